@@ -1,0 +1,211 @@
+/*
+ * sagecal_b200.h -- C ABI of libsagecal_b200.so
+ *
+ * The data-parallel hot path of SAGECal direction-dependent calibration
+ * (arXiv 1910.13908; the problem statement is BASELINE.json:5 "north_star",
+ * the paper itself, only says "a single calibration solution will
+ * be derived for each cluster") as hand-written CUDA for one NVIDIA B200
+ * (sm_100a).  Readings of everything the paper leaves open: DESIGN.md §3.
+ *
+ * Conventions
+ *   N stations, B = N(N-1)/2 baselines (p<q, no autocorrelations), T time
+ *   slots, F channels, K clusters.  rows = T*B, samples = rows*F.
+ *   Canonical row order: row r = t*B + b, b(p,q) = p*N - p(p+1)/2 + (q-p-1).
+ *   Complex numbers are interleaved {re, im} doubles (sagecal_c128, bit
+ *   compatible with cuDoubleComplex / torch.complex128 / C99 double complex).
+ *   A 2x2 matrix is row-major [XX, XY, YX, YY].
+ *   Visibilities, residuals:  [rows][F][4] c128 (64 B per sample).
+ *   Coherencies of K clusters, chosen by `coh_format`:
+ *     SAGECAL_COH_FULL   [K][rows][F][4] c128  (general 2x2, 64 B/sample)
+ *     SAGECAL_COH_SCALAR [K][rows][F]    c128  (C = c*I2, exact when every
+ *                         source has Q=U=V=0; 16 B/sample)
+ *   Jones matrices: [K][N][4] c128.
+ *
+ * Pointers
+ *   "dev"  = device pointer owned by the caller (e.g. a torch tensor); must be
+ *            32-byte aligned (torch allocations are 512-byte aligned).
+ *   "host" = host pointer, read during the call (small descriptors only),
+ *            may be freed on return.
+ *   The library never allocates caller-visible memory: scratch comes from the
+ *   caller's `workspace` (dev, 256-byte aligned), sized by
+ *   sagecal_workspace_bytes().  `stream` is a cudaStream_t (NULL = default
+ *   stream).  Every call is asynchronous on `stream` and never synchronises
+ *   the device; scalar results are device pointers.
+ *
+ * Errors
+ *   Every function returns 0 on success or a negative SAGECAL_E* code; nothing
+ *   is enqueued when argument validation fails.  No exceptions, no aborts.
+ */
+#ifndef SAGECAL_B200_H
+#define SAGECAL_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { double re, im; } sagecal_c128;
+
+#define SAGECAL_OK            0
+#define SAGECAL_EINVAL       (-1)  /* bad shape, NULL pointer, misaligned pointer, bad enum */
+#define SAGECAL_EWORKSPACE   (-2)  /* workspace NULL or smaller than sagecal_workspace_bytes() */
+#define SAGECAL_ECUDA        (-3)  /* a CUDA call failed: see sagecal_last_cuda_error() */
+#define SAGECAL_EUNSUPPORTED (-4)  /* valid request this build does not implement */
+
+#define SAGECAL_COH_FULL   0
+#define SAGECAL_COH_SCALAR 1
+
+/* `what` of sagecal_workspace_bytes */
+#define SAGECAL_WS_LM_PASS   1
+#define SAGECAL_WS_CALIBRATE 2
+
+/* Speed of light used to turn uvw in metres into wavelengths (m/s). */
+#define SAGECAL_C0 299792458.0
+
+const char* sagecal_strerror(int code);
+/* cudaError_t of the last failing CUDA call made by this library on this host thread (0 = none). */
+int sagecal_last_cuda_error(void);
+/* "major.minor.patch" of the library. */
+const char* sagecal_version(void);
+
+/* Bytes of device scratch the call named by `what` needs for this shape (0 if none).
+ * Returns 0 for invalid arguments as well; the call itself then reports SAGECAL_EINVAL. */
+size_t sagecal_workspace_bytes(int what, int nstations, int ntime, int nchan, int nclus);
+
+/*
+ * Coherency prediction (BASELINE.json:5 "The first is per-cluster model prediction";
+ * SURVEY.md §8(a) rows 8a-0, 8a-1; DESIGN.md §3 readings Q2, Q4, Q5):
+ *
+ *   C_k[r][c] = sum_{s in cluster k} B_s(f_c) * exp(-2 pi i (f_c/c0) (u_r l_s + v_r m_s + w_r (n_s - 1)))
+ *   B_s(f)    = (f/f0)^alpha_s * [[I+Q, U+iV], [U-iV, I-Q]],     n_s - 1 = -(l^2+m^2)/(1+sqrt(1-l^2-m^2))
+ *
+ * nstations, ntime : N, T; rows = T*N(N-1)/2 (N >= 2, T >= 1).
+ * freqs_host [F]   : channel frequencies in Hz (host), F >= 1.  Uniformly spaced
+ *                    channels use a per-channel phasor recurrence; anything else one sincos per channel.
+ * f0               : reference frequency of the flux law, Hz (> 0).
+ * uvw              : dev [rows][3] f64, metres, for the baseline as ordered (p, q).
+ * nclus, cluster_offset_host [K+1] : sources of cluster k are [offset[k], offset[k+1]) (host, non-decreasing,
+ *                    offset[0] = 0).  An empty cluster yields zeros.
+ * src_l, src_m, src_I, src_alpha : dev [S_tot] f64.  src_Q/U/V : dev [S_tot] or all three NULL = unpolarised.
+ * coh_format       : SAGECAL_COH_FULL, or SAGECAL_COH_SCALAR (then Q/U/V must be NULL).
+ * coh              : dev out, layout per coh_format.
+ * precision        : 0 = float64 throughout (parity 1e-10); 1 = mixed: float64 phase and range reduction,
+ *                    float32 sincos polynomial and flux product, float64 accumulation (parity 1e-5).
+ * workspace        : dev scratch >= sagecal_predict_workspace_bytes(F, S_tot) (the prepared source table).
+ * Limits: F <= 512, K <= 1024 (descriptors travel as kernel parameters, so the call needs no host->device copy).
+ */
+size_t sagecal_predict_workspace_bytes(int nchan, int nsrc_total);
+int sagecal_predict_coherencies(
+    int nstations, int ntime, int nchan,
+    const double* freqs_host, double f0,
+    const double* uvw,
+    int nclus, const int* cluster_offset_host,
+    const double* src_l, const double* src_m,
+    const double* src_I, const double* src_Q, const double* src_U, const double* src_V,
+    const double* src_alpha,
+    int coh_format, sagecal_c128* coh, int precision,
+    void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Jones corruption and subtraction (BASELINE.json:5 "the Jones-corrupted residual V_pq - J_p C_pq J_q^H";
+ * SURVEY.md §8(a) rows 8a-2, 8a-3, 8a-6):
+ *
+ *   vis_out = vis_in + sign * sum_{k : mask[k]} J_{p,k} C_k J_{q,k}^H        (clusters added in index order)
+ *
+ * coh              : dev, all K clusters, layout per coh_format.
+ * jones            : dev [K][N][4].
+ * cluster_mask_host: host [K] bytes, non-zero = include; NULL = all clusters.
+ * sign             : -1 subtracts the corrupted model (residual), +1 adds it (simulate / E-step add-back).
+ * vis_in, vis_out  : dev [rows][F][4]; vis_out may alias vis_in exactly (in place), no partial overlap.
+ *                    vis_in may be NULL = zeros (pure model).
+ */
+int sagecal_corrupt_subtract(
+    int nstations, int ntime, int nchan, int nclus,
+    int coh_format, const sagecal_c128* coh, const sagecal_c128* jones,
+    const uint8_t* cluster_mask_host, double sign,
+    const sagecal_c128* vis_in, sagecal_c128* vis_out, void* stream);
+
+/*
+ * One fused Levenberg-Marquardt evaluation pass for ONE cluster (BASELINE.json:5 "the cost, and the gradient
+ * and per-station-block J^H J accumulation over all N(N-1)/2 baselines"):
+ *
+ *   E = x - J_p C J_q^H,   T1 = J_p C,   A = C J_q^H          per sample on baseline (p, q)
+ *   cost    = sum ||E||_F^2
+ *   grad[p] = sum_{q>p} E A^H  + sum_{q<p} E_{qp}^H T1_{qp}     (d cost = -2 Re sum_p tr(grad[p]^H dJ_p))
+ *   jtj[p]  = sum_{q>p} A A^H  + sum_{q<p} T1_{qp}^H T1_{qp}     (2x2 Hermitian PSD; the (p,p) diagonal 8x8 real
+ *                                                                block of J^T J acts on a perturbation D as D*jtj[p])
+ *
+ * x      : dev [rows][F][4]: data with the other clusters' models subtracted.
+ * coh_k  : dev, this cluster's coherencies ([rows][F][4] or [rows][F]).
+ * jones_k: dev [N][4].
+ * cost   : dev out [1] f64.   grad, jtj : dev out [N][4] c128.
+ * Sums are formed without global atomics in a fixed order: results are bit-reproducible run to run.
+ */
+int sagecal_lm_cost_grad_jtj(
+    int nstations, int ntime, int nchan,
+    const sagecal_c128* x, int coh_format, const sagecal_c128* coh_k,
+    const sagecal_c128* jones_k,
+    double* cost, sagecal_c128* grad, sagecal_c128* jtj,
+    void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * SAGE expectation-maximisation over K clusters with a block-diagonal Levenberg-Marquardt M-step kept entirely on
+ * the device (BASELINE.json:5 "the SAGE-EM / Levenberg-Marquardt inner loop run per cluster against the residual
+ * with the other clusters' J_p C J_q^H subtracted", item (e)):
+ *
+ *   R = vis - sum_k J_k C_k J_k^H
+ *   for em < n_em, for k < K:   x_k = R + J_k C_k J_k^H
+ *       mu = tau * max_p max(M_p[0][0], M_p[1][1]),  nu = 2
+ *       n_lm times: dJ_p = G_p (M_p + mu I)^-1;  J' = J + dJ;  rho = (phi(J) - phi(J')) / sum_p [Re tr(G_p^H dJ_p) + mu ||dJ_p||^2]
+ *                   accept iff rho > 0 (all finite): J = J', mu *= max(1/3, 1-(2 rho-1)^3), nu = 2;  else mu *= nu, nu *= 2
+ *       R = x_k - J_k C_k J_k^H
+ *
+ * vis     : dev [rows][F][4] (read only).     coh : dev, K clusters.
+ * jones   : dev [K][N][4], in = start values, out = solution.
+ * residual: dev out [rows][F][4]; must not alias vis.
+ * tau     : initial damping factor (1e-3 in all configs).
+ * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
+ * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
+ * No device->host transfer or synchronisation happens inside the call.
+ */
+int sagecal_sage_calibrate(
+    int nstations, int ntime, int nchan, int nclus,
+    const sagecal_c128* vis, int coh_format, const sagecal_c128* coh,
+    sagecal_c128* jones, sagecal_c128* residual,
+    int n_em, int n_lm, double tau,
+    double* cost_per_cluster, double* cost_trace,
+    void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * Whole-interval convenience entry with HOST buffers (used for end-to-end timing): copies uvw, the source table,
+ * the visibilities and the start Jones to the device, runs predict + calibrate, copies Jones, residual and costs
+ * back.  Allocates and frees its own device memory (cudaMallocAsync on `stream`) and synchronises `stream` before
+ * returning.  All array pointers are host pointers (pinned memory recommended).  residual_host / cost_trace_host
+ * may be NULL (not copied back).
+ */
+int sagecal_calibrate_interval_host(
+    int nstations, int ntime, int nchan,
+    const double* freqs_host, double f0, const double* uvw_host,
+    int nclus, const int* cluster_offset_host,
+    const double* src_l, const double* src_m, const double* src_I,
+    const double* src_Q, const double* src_U, const double* src_V, const double* src_alpha,
+    int coh_format,
+    const sagecal_c128* vis_host, sagecal_c128* jones_host, sagecal_c128* residual_host,
+    int n_em, int n_lm, double tau,
+    double* cost_per_cluster_host, double* cost_trace_host, void* stream);
+
+/*
+ * Test hook, host only, no device needed: replays the work decomposition of the LM pass kernel.
+ * cover : host out [T*B] int32, must be zeroed by the caller; on return every entry must be 1 (each baseline and
+ *         time slot visited by exactly one thread of one CTA).
+ * info  : host out [8] int64 = {TQ, nchunk, ncols, TC, tlen, nslots, R, U}.
+ * Returns 0, SAGECAL_EINVAL, or a positive bit mask naming the violated bookkeeping invariant.
+ */
+int sagecal_debug_pass_cover(int nstations, int ntime, int nchan, int32_t* cover, int64_t* info);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAGECAL_B200_H */

@@ -1,0 +1,26 @@
+"""sagecal-b200: the data-parallel hot path of SAGECal direction-dependent calibration on one NVIDIA B200.
+
+Thin ctypes binding of libsagecal_b200.so (C ABI: include/sagecal_b200.h).  The functions here have the names of
+the C entry points and only marshal arguments: torch is used for device memory and streams, every step of the path
+runs in the library's CUDA kernels.  There is no CPU fallback: if the shared library is missing the import of any
+entry point raises.
+"""
+from ._binding import (  # noqa: F401
+    COH_FULL,
+    COH_SCALAR,
+    SagecalError,
+    calibrate_interval_host,
+    corrupt_subtract,
+    lib_path,
+    lm_cost_grad_jtj,
+    load_library,
+    predict_coherencies,
+    sage_calibrate,
+    version,
+    workspace_bytes,
+)
+
+__all__ = [
+    "COH_FULL", "COH_SCALAR", "SagecalError", "calibrate_interval_host", "corrupt_subtract", "lib_path",
+    "lm_cost_grad_jtj", "load_library", "predict_coherencies", "sage_calibrate", "version", "workspace_bytes",
+]

@@ -1,0 +1,260 @@
+"""ctypes marshalling for libsagecal_b200.so.  No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+import torch
+
+COH_FULL = 0
+COH_SCALAR = 1
+WS_LM_PASS = 1
+WS_CALIBRATE = 2
+
+_PKG = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_PKG, "libsagecal_b200.so")
+_lib = None
+
+
+class SagecalError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        L = load_library()
+        msg = L.sagecal_strerror(code).decode()
+        extra = f" (cudaError {L.sagecal_last_cuda_error()})" if code == -3 else ""
+        super().__init__(f"{where}: {msg}{extra} [code {code}]")
+        self.code = code
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def load_library():
+    """dlopen the C-ABI library.  Raises if it has not been built: there is no fallback path."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(_LIB_PATH):
+        raise ImportError(
+            f"{_LIB_PATH} is missing: build it with `python -m paper_1910_13908_b200.build` "
+            "(nvcc, sm_100a).  sagecal-b200 has no CPU or PyTorch fallback.")
+    L = ctypes.CDLL(_LIB_PATH)
+    i, d, vp, sz = ctypes.c_int, ctypes.c_double, ctypes.c_void_p, ctypes.c_size_t
+    L.sagecal_strerror.restype = ctypes.c_char_p
+    L.sagecal_strerror.argtypes = [i]
+    L.sagecal_last_cuda_error.restype = i
+    L.sagecal_version.restype = ctypes.c_char_p
+    L.sagecal_workspace_bytes.restype = sz
+    L.sagecal_workspace_bytes.argtypes = [i, i, i, i, i]
+    L.sagecal_predict_workspace_bytes.restype = sz
+    L.sagecal_predict_workspace_bytes.argtypes = [i, i]
+    L.sagecal_predict_coherencies.restype = i
+    L.sagecal_predict_coherencies.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, i, vp, sz, vp]
+    L.sagecal_corrupt_subtract.restype = i
+    L.sagecal_corrupt_subtract.argtypes = [i, i, i, i, i, vp, vp, vp, d, vp, vp, vp]
+    L.sagecal_lm_cost_grad_jtj.restype = i
+    L.sagecal_lm_cost_grad_jtj.argtypes = [i, i, i, vp, i, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sagecal_sage_calibrate.restype = i
+    L.sagecal_sage_calibrate.argtypes = [i, i, i, i, vp, i, vp, vp, vp, i, i, d, vp, vp, vp, sz, vp]
+    L.sagecal_calibrate_interval_host.restype = i
+    L.sagecal_calibrate_interval_host.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp,
+                                                  i, i, d, vp, vp, vp]
+    _lib = L
+    return L
+
+
+def version() -> str:
+    return load_library().sagecal_version().decode()
+
+
+def workspace_bytes(what: int, N: int, T: int, F: int, K: int = 1) -> int:
+    return int(load_library().sagecal_workspace_bytes(what, N, T, F, K))
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise SagecalError(code, where)
+
+
+def _stream(stream) -> int:
+    s = torch.cuda.current_stream() if stream is None else stream
+    return int(s.cuda_stream)
+
+
+def _dev(t: Optional[torch.Tensor], dtype, name: str) -> Optional[int]:
+    if t is None:
+        return None
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dtype and t.is_contiguous()):
+        raise TypeError(f"{name}: expected a contiguous CUDA tensor of dtype {dtype}")
+    return t.data_ptr()
+
+
+def _workspace(nbytes: int, device) -> torch.Tensor:
+    return torch.empty(max(int(nbytes), 256), dtype=torch.uint8, device=device)
+
+
+def _rows(N: int, T: int) -> int:
+    return T * (N * (N - 1) // 2)
+
+
+def predict_coherencies(N: int, T: int, freqs: Sequence[float], f0: float, uvw: torch.Tensor,
+                        cluster_offset: Sequence[int], src_l: torch.Tensor, src_m: torch.Tensor, src_I: torch.Tensor,
+                        src_alpha: torch.Tensor, src_Q: Optional[torch.Tensor] = None,
+                        src_U: Optional[torch.Tensor] = None, src_V: Optional[torch.Tensor] = None,
+                        coh_format: int = COH_FULL, precision: int = 0, out: Optional[torch.Tensor] = None,
+                        stream=None) -> torch.Tensor:
+    """sagecal_predict_coherencies: coh [K, rows, F, 4] (COH_FULL) or [K, rows, F] (COH_SCALAR), complex128."""
+    L = load_library()
+    fr = np.ascontiguousarray(freqs, dtype=np.float64)
+    co = np.ascontiguousarray(cluster_offset, dtype=np.int32)
+    F, K, rows = int(fr.size), int(co.size) - 1, _rows(N, T)
+    shape = (K, rows, F, 4) if coh_format == COH_FULL else (K, rows, F)
+    if out is None:
+        out = torch.empty(shape, dtype=torch.complex128, device=uvw.device)
+    elif tuple(out.shape) != shape:
+        raise ValueError(f"out: expected shape {shape}")
+    if tuple(uvw.shape) != (rows, 3):
+        raise ValueError(f"uvw: expected shape {(rows, 3)}")
+    S = int(co[-1]) if co.size else 0
+    for name, t in (("src_l", src_l), ("src_m", src_m), ("src_I", src_I), ("src_alpha", src_alpha),
+                    ("src_Q", src_Q), ("src_U", src_U), ("src_V", src_V)):
+        if t is not None and t.numel() != S:
+            raise ValueError(f"{name}: expected {S} elements")
+    wsb = int(L.sagecal_predict_workspace_bytes(F, S))
+    ws = _workspace(wsb, uvw.device)
+    f64 = torch.float64
+    rc = L.sagecal_predict_coherencies(
+        N, T, F, fr.ctypes.data, float(f0), _dev(uvw, f64, "uvw"), K, co.ctypes.data,
+        _dev(src_l, f64, "src_l"), _dev(src_m, f64, "src_m"), _dev(src_I, f64, "src_I"),
+        _dev(src_Q, f64, "src_Q"), _dev(src_U, f64, "src_U"), _dev(src_V, f64, "src_V"),
+        _dev(src_alpha, f64, "src_alpha"), coh_format, _dev(out, torch.complex128, "out"), precision,
+        ws.data_ptr(), wsb, _stream(stream))
+    _check(rc, "sagecal_predict_coherencies")
+    return out
+
+
+def _coh_check(coh: torch.Tensor, coh_format: int, K: int, rows: int, F: int, name="coh"):
+    shape = (K, rows, F, 4) if coh_format == COH_FULL else (K, rows, F)
+    if tuple(coh.shape) != shape:
+        raise ValueError(f"{name}: expected shape {shape}, got {tuple(coh.shape)}")
+
+
+def corrupt_subtract(N: int, T: int, F: int, coh: torch.Tensor, jones: torch.Tensor,
+                     vis_in: Optional[torch.Tensor], sign: float = -1.0, cluster_mask: Optional[Sequence[int]] = None,
+                     coh_format: int = COH_FULL, out: Optional[torch.Tensor] = None, stream=None) -> torch.Tensor:
+    """sagecal_corrupt_subtract: out = vis_in + sign * sum_k J_p C_k J_q^H.  out may be vis_in (in place)."""
+    L = load_library()
+    K, rows = int(jones.shape[0]), _rows(N, T)
+    c128 = torch.complex128
+    if K:
+        _coh_check(coh, coh_format, K, rows, F)
+    if tuple(jones.shape[:2]) != (K, N) or jones.numel() != K * N * 4:
+        raise ValueError("jones: expected shape [K, N, 2, 2]")
+    if out is None:
+        out = torch.empty((rows, F, 4), dtype=c128, device=jones.device)
+    if out.numel() != rows * F * 4 or (vis_in is not None and vis_in.numel() != rows * F * 4):
+        raise ValueError("vis: expected rows*F*4 elements")
+    mask = None
+    if cluster_mask is not None:
+        mask = np.ascontiguousarray(cluster_mask, dtype=np.uint8)
+        if mask.size != K:
+            raise ValueError("cluster_mask: expected K entries")
+    rc = L.sagecal_corrupt_subtract(N, T, F, K, coh_format, _dev(coh, c128, "coh") if K else None,
+                                    _dev(jones, c128, "jones") if K else None,
+                                    mask.ctypes.data if mask is not None else None, float(sign),
+                                    _dev(vis_in, c128, "vis_in"), _dev(out, c128, "out"), _stream(stream))
+    _check(rc, "sagecal_corrupt_subtract")
+    return out
+
+
+def lm_cost_grad_jtj(N: int, T: int, F: int, x: torch.Tensor, coh_k: torch.Tensor, jones_k: torch.Tensor,
+                     coh_format: int = COH_FULL, stream=None):
+    """sagecal_lm_cost_grad_jtj: returns (cost [1] f64, grad [N,2,2] c128, jtj [N,2,2] c128) device tensors."""
+    L = load_library()
+    rows = _rows(N, T)
+    c128 = torch.complex128
+    if x.numel() != rows * F * 4 or coh_k.numel() != rows * F * (4 if coh_format == COH_FULL else 1):
+        raise ValueError("x / coh_k: wrong number of elements")
+    if jones_k.numel() != N * 4:
+        raise ValueError("jones_k: expected [N, 2, 2]")
+    dev = x.device
+    cost = torch.empty(1, dtype=torch.float64, device=dev)
+    grad = torch.empty((N, 2, 2), dtype=c128, device=dev)
+    jtj = torch.empty((N, 2, 2), dtype=c128, device=dev)
+    wsb = workspace_bytes(WS_LM_PASS, N, T, F)
+    ws = _workspace(wsb, dev)
+    rc = L.sagecal_lm_cost_grad_jtj(N, T, F, _dev(x, c128, "x"), coh_format, _dev(coh_k, c128, "coh_k"),
+                                    _dev(jones_k, c128, "jones_k"), cost.data_ptr(), grad.data_ptr(), jtj.data_ptr(),
+                                    ws.data_ptr(), wsb, _stream(stream))
+    _check(rc, "sagecal_lm_cost_grad_jtj")
+    return cost, grad, jtj
+
+
+def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor, jones: torch.Tensor,
+                   n_em: int, n_lm: int, tau: float = 1e-3, coh_format: int = COH_FULL,
+                   residual: Optional[torch.Tensor] = None, trace: bool = True, workspace: Optional[torch.Tensor] = None,
+                   stream=None):
+    """sagecal_sage_calibrate.  `jones` [K,N,2,2] is updated in place.
+    Returns dict(jones, residual, cost_per_cluster [K], cost_trace [n_em*K+1] or None), all device tensors."""
+    L = load_library()
+    K, rows = int(jones.shape[0]), _rows(N, T)
+    c128 = torch.complex128
+    if K:
+        _coh_check(coh, coh_format, K, rows, F)
+    if vis.numel() != rows * F * 4:
+        raise ValueError("vis: expected rows*F*4 elements")
+    if jones.numel() != K * N * 4:
+        raise ValueError("jones: expected [K, N, 2, 2]")
+    dev = vis.device
+    if residual is None:
+        residual = torch.empty((rows, F, 4), dtype=c128, device=dev)
+    cpc = torch.zeros(max(K, 1), dtype=torch.float64, device=dev)
+    tr = torch.zeros(n_em * K + 1, dtype=torch.float64, device=dev) if trace else None
+    wsb = workspace_bytes(WS_CALIBRATE, N, T, F, K)
+    ws = workspace if workspace is not None else _workspace(wsb, dev)
+    if ws.numel() < wsb:
+        raise ValueError("workspace too small")
+    rc = L.sagecal_sage_calibrate(N, T, F, K, _dev(vis, c128, "vis"), coh_format,
+                                  _dev(coh, c128, "coh") if K else None, _dev(jones, c128, "jones") if K else None,
+                                  _dev(residual, c128, "residual"), int(n_em), int(n_lm), float(tau),
+                                  cpc.data_ptr(), tr.data_ptr() if tr is not None else None,
+                                  ws.data_ptr(), ws.numel(), _stream(stream))
+    _check(rc, "sagecal_sage_calibrate")
+    return dict(jones=jones, residual=residual, cost_per_cluster=cpc[:K], cost_trace=tr)
+
+
+def _host(a, dtype, name):
+    if a is None:
+        return None, None
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != dtype or not a.is_contiguous():
+            raise TypeError(f"{name}: expected a contiguous CPU tensor of dtype {dtype}")
+        return a.data_ptr(), a
+    raise TypeError(f"{name}: expected a CPU torch tensor (pinned memory recommended)")
+
+
+def calibrate_interval_host(N: int, T: int, freqs: Sequence[float], f0: float, uvw: torch.Tensor,
+                            cluster_offset: Sequence[int], src_l, src_m, src_I, src_alpha, vis: torch.Tensor,
+                            jones: torch.Tensor, n_em: int, n_lm: int, tau: float = 1e-3, src_Q=None, src_U=None,
+                            src_V=None, coh_format: int = COH_FULL, residual: Optional[torch.Tensor] = None,
+                            cost_per_cluster: Optional[torch.Tensor] = None, stream=None):
+    """sagecal_calibrate_interval_host: predict + calibrate from HOST tensors (copies inside the call).
+    `jones` (CPU, [K,N,2,2]) is updated in place; `residual` (CPU) is filled if given."""
+    L = load_library()
+    fr = np.ascontiguousarray(freqs, dtype=np.float64)
+    co = np.ascontiguousarray(cluster_offset, dtype=np.int32)
+    F, K = int(fr.size), int(co.size) - 1
+    f64, c128 = torch.float64, torch.complex128
+    if cost_per_cluster is None:
+        cost_per_cluster = torch.zeros(K, dtype=f64)
+    ptrs = [_host(t, f64, n)[0] for n, t in (("src_l", src_l), ("src_m", src_m), ("src_I", src_I), ("src_Q", src_Q),
+                                            ("src_U", src_U), ("src_V", src_V), ("src_alpha", src_alpha))]
+    rc = L.sagecal_calibrate_interval_host(
+        N, T, F, fr.ctypes.data, float(f0), _host(uvw, f64, "uvw")[0], K, co.ctypes.data, *ptrs, coh_format,
+        _host(vis, c128, "vis")[0], _host(jones, c128, "jones")[0], _host(residual, c128, "residual")[0],
+        int(n_em), int(n_lm), float(tau), _host(cost_per_cluster, f64, "cost_per_cluster")[0], None,
+        _stream(stream))
+    _check(rc, "sagecal_calibrate_interval_host")
+    return dict(jones=jones, residual=residual, cost_per_cluster=cost_per_cluster)

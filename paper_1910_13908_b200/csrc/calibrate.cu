@@ -1,0 +1,360 @@
+// sagecal_sage_calibrate: SAGE-EM over clusters with a block-diagonal Levenberg-Marquardt M-step, the whole loop
+// enqueued on one stream with every decision taken on the device (SURVEY.md §8(a) rows 8a-3, 8a-5..8a-7,
+// §8(c) A7-A8).  No device->host traffic, no synchronisation inside an interval.
+#include <math.h>
+#include <string.h>
+#include "lm_pass.cuh"
+
+namespace sgc {
+
+int corrupt_range(int N, int T, int F, int coh_format, const sagecal_c128* coh, const sagecal_c128* jones, int k0,
+                  int k1, double sign, const sagecal_c128* vis_in, sagecal_c128* vis_out, cudaStream_t st);
+
+thread_local int g_last_cuda_error = 0;
+
+int num_sms() {
+    static int cached = 0;
+    if (cached) return cached;
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        return 148;  // B200; only reached without a device (workspace sizing on a CPU-only box)
+    }
+    cached = n;
+    return n;
+}
+
+// ---- LM control (8a-5): damping, 2x2 solves, accept/reject, all on device --------------------------------------
+struct LmScalars {
+    double phi;      // cost at the accepted Jones
+    double phi_try;  // cost at the trial Jones (written by the pass)
+    double mu, nu;   // Nielsen damping state
+    double pred;     // predicted reduction of the pending trial step
+    double pad[3];
+};
+
+constexpr int LM_THREADS = 256;
+
+__device__ __forceinline__ double block_sum(double v, double* s_buf) {  // fixed-order tree, all threads get the sum
+    const int tid = threadIdx.x;
+    s_buf[tid] = v;
+    __syncthreads();
+    for (int o = LM_THREADS / 2; o > 0; o >>= 1) {
+        if (tid < o) s_buf[tid] += s_buf[tid + o];
+        __syncthreads();
+    }
+    const double r = s_buf[0];
+    __syncthreads();
+    return r;
+}
+__device__ __forceinline__ double block_max(double v, double* s_buf) {
+    const int tid = threadIdx.x;
+    s_buf[tid] = v;
+    __syncthreads();
+    for (int o = LM_THREADS / 2; o > 0; o >>= 1) {
+        if (tid < o) s_buf[tid] = fmax(s_buf[tid], s_buf[tid + o]);
+        __syncthreads();
+    }
+    const double r = s_buf[0];
+    __syncthreads();
+    return r;
+}
+
+// INIT:   (phi, G, M) were just evaluated at J.  mu = tau*max_p max(M_p00, M_p11), nu = 2; first trial step.
+// !INIT:  (phi_try, G_try, M_try) were just evaluated at J_try.  rho test, accept/reject, damping update; next
+//         trial step.  dJ_p = G_p (M_p + mu I)^-1, J_try = J + dJ, pred = sum_p Re tr(G_p^H dJ_p) + mu ||dJ_p||^2.
+template <bool INIT>
+__global__ void __launch_bounds__(LM_THREADS)
+lm_step_kernel(int N, double tau, LmScalars* __restrict__ sc, sagecal_c128* __restrict__ J,
+               sagecal_c128* __restrict__ G, sagecal_c128* __restrict__ M, const sagecal_c128* __restrict__ G_try,
+               const sagecal_c128* __restrict__ M_try, sagecal_c128* __restrict__ J_try,
+               double* __restrict__ cost_out, double* __restrict__ trace_out) {
+    __shared__ double s_buf[LM_THREADS];
+    const int tid = threadIdx.x;
+    double phi = sc->phi, mu, nu;
+    bool accept = false;
+    if (INIT) {
+        double mmax = 0.0;
+        for (int p = tid; p < N; p += LM_THREADS) mmax = fmax(mmax, fmax(M[4 * p].re, M[4 * p + 3].re));
+        mmax = block_max(mmax, s_buf);
+        mu = tau * mmax;
+        nu = 2.0;
+    } else {
+        const double phin = sc->phi_try, pred = sc->pred;
+        mu = sc->mu; nu = sc->nu;
+        const double rho = (phi - phin) / pred;
+        accept = isfinite(phin) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
+        if (accept) {
+            phi = phin;
+            const double s = 2.0 * rho - 1.0;
+            mu *= fmax(1.0 / 3.0, 1.0 - s * s * s);
+            nu = 2.0;
+        } else {
+            mu *= nu;
+            nu *= 2.0;
+        }
+    }
+    if (!(mu >= 1e-300)) mu = 1e-300;
+    if (mu > 1e300) mu = 1e300;
+    if (nu > 0x1p60) nu = 0x1p60;
+
+    double pred_part = 0.0;
+    for (int p = tid; p < N; p += LM_THREADS) {
+        cplx g[4], m[4], j[4];
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+            if (accept) {
+                g[i] = mk(G_try[4 * p + i].re, G_try[4 * p + i].im);
+                m[i] = mk(M_try[4 * p + i].re, M_try[4 * p + i].im);
+                j[i] = mk(J_try[4 * p + i].re, J_try[4 * p + i].im);
+                G[4 * p + i].re = g[i].re; G[4 * p + i].im = g[i].im;
+                M[4 * p + i].re = m[i].re; M[4 * p + i].im = m[i].im;
+                J[4 * p + i].re = j[i].re; J[4 * p + i].im = j[i].im;
+            } else {
+                g[i] = mk(G[4 * p + i].re, G[4 * p + i].im);
+                m[i] = mk(M[4 * p + i].re, M[4 * p + i].im);
+                j[i] = mk(J[4 * p + i].re, J[4 * p + i].im);
+            }
+        }
+        // (M_p + mu I)^-1 of the Hermitian 2x2 [[a, b], [conj b, d]]
+        const double a = m[0].re + mu, d = m[3].re + mu;
+        const cplx b = m[1];
+        const double det = a * d - (b.re * b.re + b.im * b.im);
+        const cplx inv[4] = {mk(d / det, 0.0), mk(-b.re / det, -b.im / det), mk(-b.re / det, b.im / det),
+                             mk(a / det, 0.0)};
+        cplx dj[4];
+        dj[0] = cfma(g[1], inv[2], cmul(g[0], inv[0]));
+        dj[1] = cfma(g[1], inv[3], cmul(g[0], inv[1]));
+        dj[2] = cfma(g[3], inv[2], cmul(g[2], inv[0]));
+        dj[3] = cfma(g[3], inv[3], cmul(g[2], inv[1]));
+#pragma unroll
+        for (int i = 0; i < 4; i++) {
+            J_try[4 * p + i].re = j[i].re + dj[i].re;
+            J_try[4 * p + i].im = j[i].im + dj[i].im;
+            pred_part += g[i].re * dj[i].re + g[i].im * dj[i].im;
+            pred_part += mu * (dj[i].re * dj[i].re + dj[i].im * dj[i].im);
+        }
+    }
+    const double pred = block_sum(pred_part, s_buf);
+    if (tid == 0) {
+        sc->phi = phi; sc->mu = mu; sc->nu = nu; sc->pred = pred;
+        if (cost_out) *cost_out = phi;
+        if (trace_out) *trace_out = phi;
+    }
+}
+
+// ---- ||R||_F^2 for cost_trace[0] -------------------------------------------------------------------------------
+constexpr int NORM_THREADS = 256;
+__global__ void __launch_bounds__(NORM_THREADS)
+norm2_partial_kernel(const double* __restrict__ v, int64_t n4, double* __restrict__ partial) {
+    __shared__ double s_buf[NORM_THREADS];
+    double acc = 0.0;
+    for (int64_t i = (int64_t)blockIdx.x * NORM_THREADS + threadIdx.x; i < n4; i += (int64_t)gridDim.x * NORM_THREADS) {
+        const d4 a = ldg256_stream(v + 4 * i);
+        acc = fma(a.x, a.x, fma(a.y, a.y, fma(a.z, a.z, fma(a.w, a.w, acc))));
+    }
+    s_buf[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = NORM_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s_buf[threadIdx.x] += s_buf[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) partial[blockIdx.x] = s_buf[0];
+}
+__global__ void __launch_bounds__(NORM_THREADS)
+norm2_final_kernel(const double* __restrict__ partial, int n, double* __restrict__ out) {
+    __shared__ double s_buf[NORM_THREADS];
+    double acc = 0.0;
+    for (int i = threadIdx.x; i < n; i += NORM_THREADS) acc += partial[i];
+    s_buf[threadIdx.x] = acc;
+    __syncthreads();
+    for (int o = NORM_THREADS / 2; o > 0; o >>= 1) {
+        if (threadIdx.x < o) s_buf[threadIdx.x] += s_buf[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *out = s_buf[0];
+}
+constexpr int NORM_BLOCKS = 1024;
+
+struct CalWorkspace {
+    PassWorkspace pass;
+    LmScalars* sc;
+    sagecal_c128 *G, *M, *G_try, *M_try, *J_try;
+    double* norm_partial;
+};
+static size_t cal_extra_bytes(int N) {
+    return 256 + 5 * round_up((size_t)N * 64, 256) + round_up(sizeof(double) * NORM_BLOCKS, 256);
+}
+static CalWorkspace carve_cal(const PassGeom& g, void* ws) {
+    CalWorkspace w;
+    w.pass = carve_pass_workspace(g, ws);
+    char* p = (char*)ws + pass_workspace_bytes(g);
+    w.sc = (LmScalars*)p; p += 256;
+    const size_t nj = round_up((size_t)g.N * 64, 256);
+    w.G = (sagecal_c128*)p; p += nj;
+    w.M = (sagecal_c128*)p; p += nj;
+    w.G_try = (sagecal_c128*)p; p += nj;
+    w.M_try = (sagecal_c128*)p; p += nj;
+    w.J_try = (sagecal_c128*)p; p += nj;
+    w.norm_partial = (double*)p;
+    return w;
+}
+
+}  // namespace sgc
+
+using namespace sgc;
+
+extern "C" const char* sagecal_strerror(int code) {
+    switch (code) {
+        case SAGECAL_OK: return "ok";
+        case SAGECAL_EINVAL: return "invalid argument (shape, NULL or misaligned pointer, enum)";
+        case SAGECAL_EWORKSPACE: return "workspace missing, misaligned or too small";
+        case SAGECAL_ECUDA: return "CUDA call failed (see sagecal_last_cuda_error)";
+        case SAGECAL_EUNSUPPORTED: return "valid request not implemented by this build";
+        default: return "unknown sagecal error code";
+    }
+}
+extern "C" int sagecal_last_cuda_error(void) { return g_last_cuda_error; }
+extern "C" const char* sagecal_version(void) { return "0.1.0"; }
+
+extern "C" size_t sagecal_workspace_bytes(int what, int N, int T, int F, int K) {
+    (void)K;
+    if (N < 2 || T < 1 || F < 1) return 0;
+    const PassGeom g = make_pass_geom(N, T, F);
+    switch (what) {
+        case SAGECAL_WS_LM_PASS: return pass_workspace_bytes(g);
+        case SAGECAL_WS_CALIBRATE: return pass_workspace_bytes(g) + cal_extra_bytes(N);
+        default: return 0;
+    }
+}
+
+extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_c128* vis, int coh_format,
+                                      const sagecal_c128* coh, sagecal_c128* jones, sagecal_c128* residual, int n_em,
+                                      int n_lm, double tau, double* cost_per_cluster, double* cost_trace,
+                                      void* workspace, size_t workspace_bytes, void* stream) {
+    if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
+    if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    if (!vis || !residual || vis == residual || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
+    if (K > 0 && (!coh || !jones || !cost_per_cluster)) return SAGECAL_EINVAL;
+    if (K > 0 && (!aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32) || !aligned(jones, 16))) return SAGECAL_EINVAL;
+    if (!(tau > 0.0) || !isfinite(tau)) return SAGECAL_EINVAL;
+    const PassGeom g = make_pass_geom(N, T, F);
+    if (!workspace || !aligned(workspace, 256) || workspace_bytes < pass_workspace_bytes(g) + cal_extra_bytes(N))
+        return SAGECAL_EWORKSPACE;
+    const CalWorkspace w = carve_cal(g, workspace);
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t samples = (int64_t)T * g.B * F;
+    const size_t cstride = coh_format == SAGECAL_COH_SCALAR ? (size_t)samples : (size_t)samples * 4;
+    int rc;
+
+    // R = V - sum_k J_k C_k J_k^H
+    if (K > 0) {
+        if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, 0, K, -1.0, vis, residual, st))) return rc;
+    } else {
+        SGC_CUDA(cudaMemcpyAsync(residual, vis, (size_t)samples * 64, cudaMemcpyDeviceToDevice, st));
+    }
+    if (cost_trace) {
+        norm2_partial_kernel<<<NORM_BLOCKS, NORM_THREADS, 0, st>>>((const double*)residual, samples * 2, w.norm_partial);
+        SGC_LAUNCH_CHECK();
+        norm2_final_kernel<<<1, NORM_THREADS, 0, st>>>(w.norm_partial, NORM_BLOCKS, cost_trace);
+        SGC_LAUNCH_CHECK();
+    }
+    int it = 1;
+    for (int em = 0; em < n_em; em++) {
+        for (int k = 0; k < K; k++, it++) {
+            const sagecal_c128* Ck = coh + (size_t)k * cstride;
+            sagecal_c128* Jk = jones + (size_t)k * N * 4;
+            // E-step: x_k = R + J_k C_k J_k^H (in place: `residual` holds x_k during the M-step)
+            if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, +1.0, residual, residual, st))) return rc;
+            // M-step: n_lm trial steps of block-diagonal LM
+            if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, Jk, &w.sc->phi, w.G, w.M, st))) return rc;
+            lm_step_kernel<true><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
+                                                         cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
+            SGC_LAUNCH_CHECK();
+            for (int i = 0; i < n_lm; i++) {
+                if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, w.J_try, &w.sc->phi_try, w.G_try, w.M_try, st))) return rc;
+                lm_step_kernel<false><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
+                                                              cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
+                SGC_LAUNCH_CHECK();
+            }
+            // R = x_k - J_k C_k J_k^H at the new J_k
+            if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, -1.0, residual, residual, st))) return rc;
+        }
+    }
+    return SAGECAL_OK;
+}
+
+extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double* freqs_host, double f0,
+                                               const double* uvw_host, int K, const int* cluster_offset_host,
+                                               const double* src_l, const double* src_m, const double* src_I,
+                                               const double* src_Q, const double* src_U, const double* src_V,
+                                               const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
+                                               sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
+                                               int n_lm, double tau, double* cost_per_cluster_host,
+                                               double* cost_trace_host, void* stream) {
+    if (N < 2 || T < 1 || F < 1 || K < 1 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
+    if (!freqs_host || !uvw_host || !cluster_offset_host || !vis_host || !jones_host || !cost_per_cluster_host)
+        return SAGECAL_EINVAL;
+    if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    const int S = cluster_offset_host[K];
+    if (S < 0 || (S > 0 && (!src_l || !src_m || !src_I || !src_alpha))) return SAGECAL_EINVAL;
+    const bool pol = src_Q || src_U || src_V;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t B = (int64_t)N * (N - 1) / 2, rows = (int64_t)T * B, samples = rows * F;
+    const size_t vis_bytes = (size_t)samples * 64;
+    const size_t coh_bytes = (size_t)K * samples * (coh_format == SAGECAL_COH_SCALAR ? 16 : 64);
+    const size_t ws_pred = sagecal_predict_workspace_bytes(F, S);
+    const size_t ws_cal = sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE, N, T, F, K);
+    const size_t ntrace = (size_t)n_em * K + 1;
+    const size_t sS = round_up(sizeof(double) * (size_t)(S > 0 ? S : 1), 256);
+
+    // one arena: uvw | 7 source columns | vis | residual | coh | jones | costs | trace | workspaces
+    size_t off = 0;
+    auto take = [&](size_t n) { size_t o = off; off += round_up(n, 256); return o; };
+    const size_t o_uvw = take((size_t)rows * 24), o_src = take(7 * sS), o_vis = take(vis_bytes), o_res = take(vis_bytes),
+                 o_coh = take(coh_bytes), o_jon = take((size_t)K * N * 64), o_cpc = take(sizeof(double) * K),
+                 o_trc = take(sizeof(double) * ntrace), o_wsp = take(ws_pred), o_wsc = take(ws_cal);
+    char* arena = nullptr;
+    SGC_CUDA(cudaMallocAsync((void**)&arena, off, st));
+    int rc = SAGECAL_OK;
+    auto h2d = [&](size_t o, const void* src, size_t n) {
+        if (rc == SAGECAL_OK && src && n) {
+            cudaError_t e = cudaMemcpyAsync(arena + o, src, n, cudaMemcpyHostToDevice, st);
+            if (e != cudaSuccess) rc = cuda_fail(e);
+        }
+    };
+    h2d(o_uvw, uvw_host, (size_t)rows * 24);
+    const double* cols[7] = {src_l, src_m, src_I, src_alpha, src_Q, src_U, src_V};
+    double* dcol[7];
+    for (int i = 0; i < 7; i++) {
+        dcol[i] = (double*)(arena + o_src + i * sS);
+        h2d(o_src + i * sS, cols[i], sizeof(double) * (size_t)S);
+    }
+    h2d(o_vis, vis_host, vis_bytes);
+    h2d(o_jon, jones_host, (size_t)K * N * 64);
+    if (rc == SAGECAL_OK)
+        rc = sagecal_predict_coherencies(N, T, F, freqs_host, f0, (const double*)(arena + o_uvw), K, cluster_offset_host,
+                                         dcol[0], dcol[1], dcol[2], pol ? dcol[4] : nullptr, pol ? dcol[5] : nullptr,
+                                         pol ? dcol[6] : nullptr, dcol[3], coh_format, (sagecal_c128*)(arena + o_coh), 0,
+                                         arena + o_wsp, ws_pred, st);
+    if (rc == SAGECAL_OK)
+        rc = sagecal_sage_calibrate(N, T, F, K, (const sagecal_c128*)(arena + o_vis), coh_format,
+                                    (const sagecal_c128*)(arena + o_coh), (sagecal_c128*)(arena + o_jon),
+                                    (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, (double*)(arena + o_cpc),
+                                    cost_trace_host ? (double*)(arena + o_trc) : nullptr, arena + o_wsc, ws_cal, st);
+    auto d2h = [&](void* dst, size_t o, size_t n) {
+        if (rc == SAGECAL_OK && dst && n) {
+            cudaError_t e = cudaMemcpyAsync(dst, arena + o, n, cudaMemcpyDeviceToHost, st);
+            if (e != cudaSuccess) rc = cuda_fail(e);
+        }
+    };
+    d2h(jones_host, o_jon, (size_t)K * N * 64);
+    d2h(residual_host, o_res, vis_bytes);
+    d2h(cost_per_cluster_host, o_cpc, sizeof(double) * K);
+    d2h(cost_trace_host, o_trc, sizeof(double) * ntrace);
+    cudaError_t e1 = cudaFreeAsync(arena, st);
+    cudaError_t e2 = cudaStreamSynchronize(st);
+    if (rc == SAGECAL_OK && e1 != cudaSuccess) rc = cuda_fail(e1);
+    if (rc == SAGECAL_OK && e2 != cudaSuccess) rc = cuda_fail(e2);
+    return rc;
+}

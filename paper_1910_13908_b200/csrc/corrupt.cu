@@ -1,0 +1,107 @@
+// sagecal_corrupt_subtract: vis_out = vis_in + sign * sum_k J_{p,k} C_k J_{q,k}^H.
+//
+// HBM-bound, one pass over the visibilities: one thread owns one sample (64 B, two 256-bit accesses), walks the
+// requested clusters in index order streaming C_k (no L1 allocation) while the per-station Jones come through the
+// read-only L1 path (K*N*64 B, L2 resident).  In place is safe: a thread reads its sample before writing it.
+#include "common.cuh"
+
+namespace sgc {
+
+constexpr int COR_THREADS = 256;
+
+template <bool SCALAR, bool HAS_IN>
+__global__ void __launch_bounds__(COR_THREADS)
+corrupt_kernel(int N, int F, int64_t B, int64_t samples_per_slot, int64_t samples, int k0, int k1,
+               const sagecal_c128* __restrict__ coh, const sagecal_c128* __restrict__ jones, double sign,
+               const sagecal_c128* vis_in, sagecal_c128* vis_out) {
+    const int64_t i = (int64_t)blockIdx.x * COR_THREADS + threadIdx.x;
+    if (i >= samples) return;
+    const int64_t b = (i % samples_per_slot) / F;
+    int p, q;
+    bl_stations(N, b, p, q);
+    m22 acc;
+    if (HAS_IN) load_m22(vis_in + 4 * i, acc);
+    else { acc.a[0] = acc.a[1] = acc.a[2] = acc.a[3] = mk(0.0, 0.0); }
+
+    const size_t cstride = SCALAR ? (size_t)samples : (size_t)samples * 4;
+    const sagecal_c128* cp = coh + (size_t)k0 * cstride + (SCALAR ? (size_t)i : (size_t)i * 4);
+#pragma unroll 2
+    for (int k = k0; k < k1; k++, cp += cstride) {
+        m22 Jp, Jq, model;
+        load_jones(jones + ((size_t)k * N + p) * 4, Jp);
+        load_jones(jones + ((size_t)k * N + q) * 4, Jq);
+        if (SCALAR) {
+            const cplx c = ldg128_stream(cp);
+            m22 P;
+            mmh(Jp, Jq, P);                        // J_p J_q^H
+#pragma unroll
+            for (int j = 0; j < 4; j++) model.a[j] = cmul(c, P.a[j]);
+        } else {
+            m22 C, T1;
+            load_m22_stream(cp, C);
+            mm(Jp, C, T1);                         // T1 = J_p C
+            mmh(T1, Jq, model);                    // T1 J_q^H
+        }
+#pragma unroll
+        for (int j = 0; j < 4; j++) {
+            acc.a[j].re = fma(sign, model.a[j].re, acc.a[j].re);
+            acc.a[j].im = fma(sign, model.a[j].im, acc.a[j].im);
+        }
+    }
+    store_m22(vis_out + 4 * i, acc);
+}
+
+// enqueue vis_out = vis_in + sign * sum_{k0<=k<k1} model_k
+int corrupt_range(int N, int T, int F, int coh_format, const sagecal_c128* coh, const sagecal_c128* jones, int k0,
+                  int k1, double sign, const sagecal_c128* vis_in, sagecal_c128* vis_out, cudaStream_t st) {
+    const int64_t B = (int64_t)N * (N - 1) / 2;
+    const int64_t samples = (int64_t)T * B * F;
+    const unsigned grid = (unsigned)((samples + COR_THREADS - 1) / COR_THREADS);
+    const bool scalar = coh_format == SAGECAL_COH_SCALAR;
+    if (scalar) {
+        if (vis_in) corrupt_kernel<true, true><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);
+        else corrupt_kernel<true, false><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);
+    } else {
+        if (vis_in) corrupt_kernel<false, true><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);
+        else corrupt_kernel<false, false><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);
+    }
+    SGC_LAUNCH_CHECK();
+    return SAGECAL_OK;
+}
+
+}  // namespace sgc
+
+using namespace sgc;
+
+extern "C" int sagecal_corrupt_subtract(int N, int T, int F, int K, int coh_format, const sagecal_c128* coh,
+                                        const sagecal_c128* jones, const uint8_t* cluster_mask_host, double sign,
+                                        const sagecal_c128* vis_in, sagecal_c128* vis_out, void* stream) {
+    if (N < 2 || T < 1 || F < 1 || K < 0) return SAGECAL_EINVAL;
+    if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    if (!vis_out || !aligned(vis_out, 32) || (vis_in && !aligned(vis_in, 32))) return SAGECAL_EINVAL;
+    if (K > 0 && (!coh || !jones || !aligned(jones, 16))) return SAGECAL_EINVAL;
+    if (K > 0 && !aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32)) return SAGECAL_EINVAL;
+    if (!(sign == sign)) return SAGECAL_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int64_t samples = (int64_t)T * ((int64_t)N * (N - 1) / 2) * F;
+
+    // runs of consecutive selected clusters, in index order; the first run reads vis_in, later runs vis_out
+    bool first = true;
+    int k = 0;
+    while (k < K) {
+        if (cluster_mask_host && !cluster_mask_host[k]) { k++; continue; }
+        int k1 = k + 1;
+        while (k1 < K && (!cluster_mask_host || cluster_mask_host[k1])) k1++;
+        int rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k1, sign, first ? vis_in : vis_out, vis_out, st);
+        if (rc) return rc;
+        first = false;
+        k = k1;
+    }
+    if (first) {  // nothing selected: vis_out = vis_in (or zeros)
+        if (vis_in && vis_in != vis_out)
+            SGC_CUDA(cudaMemcpyAsync(vis_out, vis_in, (size_t)samples * 64, cudaMemcpyDeviceToDevice, st));
+        else if (!vis_in)
+            SGC_CUDA(cudaMemsetAsync(vis_out, 0, (size_t)samples * 64, st));
+    }
+    return SAGECAL_OK;
+}

@@ -1,0 +1,256 @@
+// sagecal_predict_coherencies: point-source coherency prediction.
+//
+//   C_k[r][c] = sum_s B_s(f_c) exp(-2 pi i (f_c/c0)(u_r l_s + v_r m_s + w_r (n_s-1)))         (BASELINE.json:5)
+//
+// FP64-pipe bound.  One thread owns one uvw row and a register tile of FT channels; the cluster's sources are
+// staged through shared memory in tiles and broadcast to the whole CTA.  For uniformly spaced channels the phasor
+// of channel c+1 is the phasor of channel c times exp(-2 pi i ph df/c0): two sincospi per (row, source, channel
+// tile) instead of FT, re-anchored at every tile so the recurrence never runs longer than FT-1 steps.
+// The phase is kept in cycles, so range reduction (inside sincospi) is exact.
+#include "common.cuh"
+
+namespace sgc {
+
+constexpr int PRED_THREADS = 128;
+constexpr int PRED_MAXF = 512;
+constexpr int PRED_MAXK = 1024;
+
+struct PredFreqs { double kf[PRED_MAXF]; };          // f_c / c0  [1/m]
+struct PredClusters { int off[PRED_MAXK + 1]; };
+
+// ---- 8a-0: source-table preparation ---------------------------------------------------------------------------
+// nm1[s] = -(l^2+m^2)/(1+sqrt(1-l^2-m^2));  flux[s][c][NFL] = (f_c/f0)^alpha_s * {I} or {I+Q, I-Q, U, V}
+template <int NFL>
+__global__ void predict_prep_kernel(int S, int F, int Fpad, PredFreqs fr, double c0_over_f0,
+                                    const double* __restrict__ l, const double* __restrict__ m,
+                                    const double* __restrict__ sI, const double* __restrict__ sQ,
+                                    const double* __restrict__ sU, const double* __restrict__ sV,
+                                    const double* __restrict__ alpha, double* __restrict__ nm1,
+                                    double* __restrict__ flux) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= S * Fpad) return;
+    int s = i / Fpad, c = i - s * Fpad;
+    if (c == 0) {
+        double r2 = fma(l[s], l[s], m[s] * m[s]);
+        nm1[s] = -r2 / (1.0 + sqrt(1.0 - r2));
+    }
+    double sc = (c < F) ? pow(fr.kf[c] * c0_over_f0, alpha[s]) : 0.0;  // padded channels contribute nothing
+    double* o = flux + (size_t)i * NFL;
+    if (NFL == 1) {
+        o[0] = sc * sI[s];
+    } else {
+        o[0] = sc * (sI[s] + sQ[s]);
+        o[1] = sc * (sI[s] - sQ[s]);
+        o[2] = sc * sU[s];
+        o[3] = sc * sV[s];
+    }
+}
+
+// ---- 8a-1: the predict kernel ---------------------------------------------------------------------------------
+// FT      channels per register tile
+// POL     polarised sources (4 flux values, general 2x2 output) / unpolarised (C = c*I2)
+// UNIFORM channel recurrence / one sincospi per channel
+// SCALAR  output format SAGECAL_COH_SCALAR (only with !POL)
+template <int FT, bool POL, bool UNIFORM, bool SCALAR>
+__global__ void __launch_bounds__(PRED_THREADS)
+predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClusters cl,
+               const double* __restrict__ uvw, const double* __restrict__ src_l,
+               const double* __restrict__ src_m, const double* __restrict__ nm1_g,
+               const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh) {
+    constexpr int NFL = POL ? 4 : 1;
+    constexpr int NACC = POL ? 4 : 1;            // complex accumulators per channel
+    constexpr int ST = POL ? 32 : 128;           // sources per shared-memory tile
+    __shared__ double s_l[ST], s_m[ST], s_n[ST];
+    __shared__ __align__(16) double s_fl[ST * FT * NFL];
+
+    const int k = blockIdx.y;
+    const int s_begin = cl.off[k], s_end = cl.off[k + 1];
+    const int64_t r = (int64_t)blockIdx.x * PRED_THREADS + threadIdx.x;
+    const bool live = r < rows;
+    double u = 0, v = 0, w = 0;
+    if (live) { u = uvw[3 * r]; v = uvw[3 * r + 1]; w = uvw[3 * r + 2]; }
+
+    for (int c0 = 0; c0 < Fpad; c0 += FT) {
+        cplx acc[FT][NACC];
+#pragma unroll
+        for (int c = 0; c < FT; c++)
+#pragma unroll
+            for (int j = 0; j < NACC; j++) acc[c][j] = mk(0.0, 0.0);
+
+        for (int sb = s_begin; sb < s_end; sb += ST) {
+            const int ns = min(ST, s_end - sb);
+            __syncthreads();
+            for (int i = threadIdx.x; i < ns; i += PRED_THREADS) {
+                s_l[i] = src_l[sb + i]; s_m[i] = src_m[sb + i]; s_n[i] = nm1_g[sb + i];
+            }
+            for (int i = threadIdx.x; i < ns * FT * NFL; i += PRED_THREADS) {
+                int s = i / (FT * NFL), rem = i - s * (FT * NFL);
+                s_fl[i] = flux_g[((size_t)(sb + s) * Fpad + c0) * NFL + rem];
+            }
+            __syncthreads();
+#pragma unroll 2
+            for (int s = 0; s < ns; s++) {
+                const double ph = fma(w, s_n[s], fma(v, s_m[s], u * s_l[s]));  // metres
+                const double* fl = s_fl + s * (FT * NFL);
+                double er, ei, dr = 1.0, di = 0.0;
+                if (UNIFORM) {
+                    double sn, cs;
+                    sincospi(2.0 * (ph * fr.kf[c0]), &sn, &cs);
+                    er = cs; ei = -sn;
+                    if (FT > 1) { sincospi(2.0 * (ph * dkf), &sn, &cs); dr = cs; di = -sn; }
+                }
+#pragma unroll
+                for (int c = 0; c < FT; c++) {
+                    if (!UNIFORM) {
+                        double sn, cs;
+                        sincospi(2.0 * (ph * fr.kf[min(c0 + c, PRED_MAXF - 1)]), &sn, &cs);
+                        er = cs; ei = -sn;
+                    }
+                    if (!POL) {
+                        const double f = fl[c];
+                        acc[c][0].re = fma(f, er, acc[c][0].re);
+                        acc[c][0].im = fma(f, ei, acc[c][0].im);
+                    } else {
+                        const double fa = fl[4 * c], fd = fl[4 * c + 1], fu = fl[4 * c + 2], fv = fl[4 * c + 3];
+                        acc[c][0].re = fma(fa, er, acc[c][0].re);   // XX = (I+Q) e
+                        acc[c][0].im = fma(fa, ei, acc[c][0].im);
+                        acc[c][3].re = fma(fd, er, acc[c][3].re);   // YY = (I-Q) e
+                        acc[c][3].im = fma(fd, ei, acc[c][3].im);
+                        // XY = (U+iV) e,  YX = (U-iV) e,  e = er + i ei
+                        acc[c][1].re = fma(-fv, ei, fma(fu, er, acc[c][1].re));
+                        acc[c][1].im = fma(fv, er, fma(fu, ei, acc[c][1].im));
+                        acc[c][2].re = fma(fv, ei, fma(fu, er, acc[c][2].re));
+                        acc[c][2].im = fma(-fv, er, fma(fu, ei, acc[c][2].im));
+                    }
+                    if (UNIFORM && c + 1 < FT) {
+                        const double nr = fma(-ei, di, er * dr), ni = fma(ei, dr, er * di);
+                        er = nr; ei = ni;
+                    }
+                }
+            }
+        }
+        if (live) {
+            if (SCALAR) {
+                sagecal_c128* o = coh + ((size_t)k * rows + r) * F + c0;
+#pragma unroll
+                for (int c = 0; c < FT; c++)
+                    if (c0 + c < F) { o[c].re = acc[c][0].re; o[c].im = acc[c][0].im; }
+            } else {
+                sagecal_c128* o = coh + (((size_t)k * rows + r) * F + c0) * 4;
+#pragma unroll
+                for (int c = 0; c < FT; c++) {
+                    if (c0 + c < F) {
+                        if (!POL) {
+                            stg256(o + 4 * c, acc[c][0].re, acc[c][0].im, 0.0, 0.0);
+                            stg256(o + 4 * c + 2, 0.0, 0.0, acc[c][0].re, acc[c][0].im);
+                        } else {
+                            stg256(o + 4 * c, acc[c][0].re, acc[c][0].im, acc[c][1].re, acc[c][1].im);
+                            stg256(o + 4 * c + 2, acc[c][2].re, acc[c][2].im, acc[c][3].re, acc[c][3].im);
+                        }
+                    }
+                }
+            }
+        }
+    }
+}
+
+template <int FT, bool POL, bool UNIFORM, bool SCALAR>
+static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
+                          const PredClusters& cl, const double* uvw, const double* l, const double* m,
+                          const double* nm1, const double* flux, sagecal_c128* coh) {
+    predict_kernel<FT, POL, UNIFORM, SCALAR><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m,
+                                                                          nm1, flux, coh);
+    SGC_LAUNCH_CHECK();
+    return SAGECAL_OK;
+}
+
+static int pick_ft(int F) { return F >= 8 ? 8 : F >= 4 ? 4 : F >= 2 ? 2 : 1; }
+
+}  // namespace sgc
+
+using namespace sgc;
+
+extern "C" size_t sagecal_predict_workspace_bytes(int nchan, int nsrc_total) {
+    if (nchan < 1 || nchan > PRED_MAXF || nsrc_total < 0) return 0;
+    const int ft = pick_ft(nchan);
+    const size_t Fpad = round_up((size_t)nchan, ft);
+    // nm1[S] + flux[S][Fpad][4]
+    return round_up(sizeof(double) * (size_t)nsrc_total, 256) + round_up(sizeof(double) * (size_t)nsrc_total * Fpad * 4, 256) + 256;
+}
+
+extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* freqs_host, double f0,
+                                           const double* uvw, int K, const int* cluster_offset_host,
+                                           const double* src_l, const double* src_m, const double* src_I,
+                                           const double* src_Q, const double* src_U, const double* src_V,
+                                           const double* src_alpha, int coh_format, sagecal_c128* coh,
+                                           int precision, void* workspace, size_t workspace_bytes, void* stream) {
+    if (N < 2 || T < 1 || F < 1 || F > PRED_MAXF || K < 0 || K > PRED_MAXK) return SAGECAL_EINVAL;
+    if (!freqs_host || !(f0 > 0.0) || !cluster_offset_host) return SAGECAL_EINVAL;
+    if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    if (precision != 0 && precision != 1) return SAGECAL_EINVAL;
+    const bool pol = src_Q || src_U || src_V;
+    if (pol && !(src_Q && src_U && src_V)) return SAGECAL_EINVAL;
+    if (pol && coh_format == SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    if (K == 0) return SAGECAL_OK;
+    if (cluster_offset_host[0] != 0) return SAGECAL_EINVAL;
+    for (int k = 0; k < K; k++)
+        if (cluster_offset_host[k + 1] < cluster_offset_host[k]) return SAGECAL_EINVAL;
+    const int S = cluster_offset_host[K];
+    if (!uvw || !coh || !aligned(coh, 32) || !aligned(uvw, 8)) return SAGECAL_EINVAL;
+    if (S > 0 && (!src_l || !src_m || !src_I || !src_alpha)) return SAGECAL_EINVAL;
+    for (int c = 0; c < F; c++)
+        if (!(freqs_host[c] > 0.0)) return SAGECAL_EINVAL;
+    if (precision == 1) return SAGECAL_EUNSUPPORTED;
+    if (!workspace || !aligned(workspace, 256) || workspace_bytes < sagecal_predict_workspace_bytes(F, S))
+        return SAGECAL_EWORKSPACE;
+
+    cudaStream_t st = (cudaStream_t)stream;
+    const int ft = pick_ft(F);
+    const int Fpad = (int)round_up((size_t)F, ft);
+    const int64_t rows = (int64_t)T * ((int64_t)N * (N - 1) / 2);
+
+    PredFreqs fr;
+    for (int c = 0; c < PRED_MAXF; c++) fr.kf[c] = 0.0;
+    for (int c = 0; c < F; c++) fr.kf[c] = freqs_host[c] / SAGECAL_C0;
+    // uniform spacing (to 1e-13 of the band centre) enables the channel recurrence
+    bool uniform = true;
+    double df = F > 1 ? (freqs_host[F - 1] - freqs_host[0]) / (F - 1) : 0.0;
+    for (int c = 0; c < F; c++)
+        if (fabs(freqs_host[c] - (freqs_host[0] + c * df)) > 1e-13 * fabs(freqs_host[0])) uniform = false;
+    const double dkf = df / SAGECAL_C0;
+    for (int c = F; c < Fpad; c++) fr.kf[c] = fr.kf[0] + c * dkf;  // padded channels: harmless phases, zero flux
+    PredClusters cl;
+    for (int k = 0; k <= PRED_MAXK; k++) cl.off[k] = cluster_offset_host[k <= K ? k : K];
+
+    double* nm1 = (double*)workspace;
+    double* flux = (double*)((char*)workspace + round_up(sizeof(double) * (size_t)S, 256));
+    if (S > 0) {
+        const int n = S * Fpad, tb = 256;
+        if (pol)
+            predict_prep_kernel<4><<<(n + tb - 1) / tb, tb, 0, st>>>(S, F, Fpad, fr, SAGECAL_C0 / f0, src_l, src_m, src_I,
+                                                                   src_Q, src_U, src_V, src_alpha, nm1, flux);
+        else
+            predict_prep_kernel<1><<<(n + tb - 1) / tb, tb, 0, st>>>(S, F, Fpad, fr, SAGECAL_C0 / f0, src_l, src_m, src_I,
+                                                                   nullptr, nullptr, nullptr, src_alpha, nm1, flux);
+        SGC_LAUNCH_CHECK();
+    }
+    dim3 grid((unsigned)((rows + PRED_THREADS - 1) / PRED_THREADS), (unsigned)K);
+    const bool scalar = coh_format == SAGECAL_COH_SCALAR;
+#define SGC_PRED(FT_, POL_, UNI_, SC_)                                                                              \
+    return launch_predict<FT_, POL_, UNI_, SC_>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l, src_m, nm1, flux, coh)
+#define SGC_PRED_FT(FT_)                                            \
+    do {                                                            \
+        if (pol) { if (uniform) SGC_PRED(FT_, true, true, false); else SGC_PRED(FT_, true, false, false); } \
+        else if (scalar) { if (uniform) SGC_PRED(FT_, false, true, true); else SGC_PRED(FT_, false, false, true); } \
+        else { if (uniform) SGC_PRED(FT_, false, true, false); else SGC_PRED(FT_, false, false, false); } \
+    } while (0)
+    switch (ft) {
+        case 8: SGC_PRED_FT(8); break;
+        case 4: SGC_PRED_FT(4); break;
+        case 2: SGC_PRED_FT(2); break;
+        default: SGC_PRED_FT(1); break;
+    }
+#undef SGC_PRED_FT
+#undef SGC_PRED
+    return SAGECAL_OK;
+}

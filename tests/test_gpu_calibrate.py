@@ -1,0 +1,172 @@
+"""-m gpu parity: sagecal_sage_calibrate (CUDA, device-resident EM/LM loop) against oracle.sage on the same seeded
+inputs and the same fixed iteration counts.  Tolerance: 1e-8 relative on the final per-cluster cost
+(BASELINE.json:5); the same bound is applied to the Jones, the residual and the cost trace.  A parity seed is only
+valid if no accept/reject decision sat within rounding of zero (DESIGN.md §3 Q18): min |rho| > 1e-6."""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from sagecal_inputs import make_config, make_problem
+from tests.helpers import rel_l2, rel_max
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-8
+
+
+def _run_both(p, n_em, n_lm, coh_format=None, polarised=False):
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, host
+
+    fmt = sg.COH_FULL if coh_format is None else coh_format
+    coh = oracle.predict(p)
+    V = oracle.simulate(p, coh)                       # the oracle's V feeds both sides (never the other way round)
+    want = oracle.sage(p.N, p.T, p.F, V, coh, p.jones_init(), n_em, n_lm, p.tau)
+    assert want["min_abs_rho"] > 1e-6, "seed has an accept/reject decision within rounding of 0: not a parity seed"
+    coh_d = gpu_predict(p, fmt)                        # the CUDA path predicts its own coherencies
+    got = sg.sage_calibrate(p.N, p.T, p.F, dev(V), coh_d, dev(p.jones_init()), n_em, n_lm, p.tau, coh_format=fmt)
+    return want, {k: (None if v is None else host(v)) for k, v in got.items()}, V, coh
+
+
+def _compare(want, got):
+    cpc_err = np.max(np.abs(got["cost_per_cluster"] - want["cost_per_cluster"]) / want["cost_per_cluster"])
+    assert cpc_err < TOL, cpc_err
+    assert rel_max(got["cost_trace"], want["cost_trace"]) < TOL
+    assert rel_l2(got["jones"], want["jones"]) < TOL
+    assert rel_l2(got["residual"], want["residual"]) < TOL
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_calibrate_configs(cuda_device, cfg):
+    """configs[0..2] with their own iteration budget (3 EM x 10 LM)."""
+    p = make_config(cfg)
+    want, got, V, coh = _run_both(p, p.n_em, p.n_lm)
+    _compare(want, got)
+    tr = got["cost_trace"]
+    assert np.all(np.diff(tr) <= 1e-12 * tr[:-1])            # P11 on the CUDA path
+
+
+def test_calibrate_scalar_format(cuda_device):
+    import paper_1910_13908_b200 as sg
+    p = make_config(2, K=6)
+    want, got, _, _ = _run_both(p, 2, 6, coh_format=sg.COH_SCALAR)
+    _compare(want, got)
+
+
+def test_calibrate_polarised_small(cuda_device):
+    p = make_problem(10, 4, 3, 3, 4, seed=31, sigma=0.05, layout="disc:3000", field_deg=4.0, patch_deg=0.5,
+                     polarised=True)
+    want, got, _, _ = _run_both(p, 3, 5)
+    _compare(want, got)
+
+
+def test_calibrate_cfg3_multi_tile(cuda_device):
+    """configs[3] shape (N=256, F=4: 8 column tiles, time-chunked units), K cut to 4 and 1 EM x 5 LM so the oracle
+    finishes in seconds."""
+    p = make_config(3, K=4)
+    want, got, _, _ = _run_both(p, 1, 5)
+    _compare(want, got)
+
+
+def test_calibrate_noiseless_recovery_on_gpu(cuda_device):
+    """P10 on the CUDA path: noiseless single-cluster data, the cost falls below 1e-20 relative and the true Jones
+    are recovered up to a unitary matrix."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+    from tests.helpers import procrustes_err
+
+    p = make_config(0, sigma=0.0)
+    coh_d = gpu_predict(p)
+    V = gpu_simulate(p, coh_d, noise=False)
+    phi0 = float((V.abs() ** 2).sum())
+    got = sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 1, 60, p.tau)
+    assert float(got["cost_per_cluster"][0]) / phi0 < 1e-20
+    assert procrustes_err(host(got["jones"])[0], p.jones_true[0]) < 1e-12
+
+
+def test_calibrate_full_size_properties(cuda_device):
+    """configs[4] (N=512, T=20, F=8, K=50 x 40 sources) in the launch configuration bench.py times, scalar
+    coherencies, 1 EM x 2 LM to bound the time.  The oracle cannot run this size inside a test, so: sampled outputs
+    (the residual on random rows, recomputed by the oracle from the returned Jones; the gradient of one LM pass for
+    sampled stations, by the oracle on those stations' baselines) and properties that hold at any size
+    (P11 monotone trace, P13 residual bookkeeping, cost == ||residual||^2)."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from sagecal_inputs import baseline_index, noise_rows
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+
+    p = make_config(4)
+    N, T, F, K = p.N, p.T, p.F, p.K
+    coh_d = gpu_predict(p, sg.COH_SCALAR)
+    V = gpu_simulate(p, coh_d, sg.COH_SCALAR)
+    J0 = dev(p.jones_init())
+    got = sg.sage_calibrate(N, T, F, V, coh_d, J0, 1, 2, p.tau, coh_format=sg.COH_SCALAR)
+    tr = host(got["cost_trace"])
+    assert np.all(np.isfinite(tr)) and np.all(np.diff(tr) <= 1e-12 * tr[:-1])
+    # cost_per_cluster[K-1] is ||R||^2 after the last M-step
+    r2 = float((got["residual"].abs() ** 2).sum())
+    assert abs(r2 - tr[-1]) < 1e-9 * r2
+    assert abs(float(got["cost_per_cluster"][-1]) - tr[-1]) <= 1e-15 * tr[-1]
+    # P13 / sampled parity: residual rows recomputed from scratch by the oracle from the returned Jones
+    rng = np.random.default_rng(44)
+    rows = np.sort(rng.choice(p.rows, 64, replace=False))
+    rows_d = torch.from_numpy(rows).to(V.device)
+    coh_rows = oracle.predict(p, rows=rows)                       # [K, 64, F, 4]
+    Jt, Jn = p.jones_true, host(got["jones"])
+    P_, Q_ = np.triu_indices(N, 1)
+    bidx = rows % p.B
+    def model(J):
+        C = coh_rows.reshape(K, rows.size, F, 2, 2)
+        return np.einsum("krij,krfjl,krml->rfim", J[:, P_[bidx]], C, J[:, Q_[bidx]].conj()).reshape(rows.size, F, 4)
+    v_rows = model(Jt) + noise_rows(p, rows)
+    assert rel_l2(host(V[rows_d]), v_rows) < 1e-10
+    assert rel_l2(host(got["residual"][rows_d]), v_rows - model(Jn)) < 1e-9
+    # one LM pass at full size: gradient / J^H J of sampled stations against the oracle on their baselines
+    x = V  # any data serves
+    cost, grad, jtj = sg.lm_cost_grad_jtj(N, T, F, x, coh_d[7], got["jones"][7], coh_format=sg.COH_SCALAR)
+    for s in (0, 255, 511):
+        others = [o for o in range(N) if o != s]
+        bl = np.array([baseline_index(N, min(s, o), max(s, o)) for o in others])
+        rr = (np.arange(T)[:, None] * p.B + bl[None, :]).reshape(-1)
+        rr_d = torch.from_numpy(rr).to(V.device)
+        xs = host(x[rr_d]).reshape(T, N - 1, F, 4)
+        cs = host(coh_d[7][rr_d]).reshape(T, N - 1, F)
+        Js = Jn[7]
+        G = np.zeros((2, 2), complex)
+        M = np.zeros((2, 2), complex)
+        for j, o in enumerate(others):
+            Xm = xs[:, j].reshape(-1, 2, 2)
+            c = cs[:, j].reshape(-1)
+            if s < o:   # s is the row station p
+                A = c[:, None, None] * Js[o].conj().T[None]
+                E = Xm - Js[s][None] @ A
+                G += np.einsum("nij,nkj->ik", E, A.conj())
+                M += np.einsum("nij,nkj->ik", A, A.conj())
+            else:       # s is the column station q
+                T1 = c[:, None, None] * Js[o][None]
+                E = Xm - T1 @ Js[s].conj().T[None]
+                G += np.einsum("nji,njk->ik", E.conj(), T1)
+                M += np.einsum("nji,njk->ik", T1.conj(), T1)
+        assert rel_l2(host(grad[s]), G) < 1e-10
+        assert rel_l2(host(jtj[s]), M) < 1e-10
+    del coh_d, V
+    torch.cuda.empty_cache()
+
+
+def test_calibrate_host_entry(cuda_device):
+    """sagecal_calibrate_interval_host (host buffers, copies inside) gives the same answer as the device API."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, host
+
+    p = make_config(1)
+    coh = oracle.predict(p)
+    V = oracle.simulate(p, coh)
+    ref = sg.sage_calibrate(p.N, p.T, p.F, dev(V), gpu_predict(p), dev(p.jones_init()), 2, 4, p.tau)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    J = t(p.jones_init())
+    R = torch.empty((p.rows, p.F, 4), dtype=torch.complex128).pin_memory()
+    out = sg.calibrate_interval_host(p.N, p.T, p.freqs, p.f0, t(p.uvw), p.cluster_offset, t(p.src_l), t(p.src_m),
+                                     t(p.src_I), t(p.src_alpha), t(V), J, 2, 4, p.tau, residual=R)
+    assert np.array_equal(J.numpy(), host(ref["jones"]))
+    assert np.array_equal(R.numpy(), host(ref["residual"]))
+    assert np.array_equal(out["cost_per_cluster"].numpy(), host(ref["cost_per_cluster"]))

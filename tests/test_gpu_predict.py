@@ -1,0 +1,122 @@
+"""-m gpu parity: sagecal_predict_coherencies (CUDA, through the C ABI) against oracle.predict on the same seeded
+inputs.  Tolerance: 1e-10 relative (BASELINE.json:5 'to within 1e-10 relative for float64'), measured as in
+DESIGN.md §3 Q16: ||gpu-oracle||_2/||oracle||_2 and max|gpu-oracle|/max|oracle| over the whole array."""
+import numpy as np
+import pytest
+
+from oracle import oracle
+from sagecal_inputs import make_config, make_problem
+from tests.helpers import rel_l2, rel_max
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+def _check(got, want, tol=TOL):
+    assert got.shape == want.shape
+    assert rel_l2(got, want) < tol, rel_l2(got, want)
+    assert rel_max(got, want) < tol, rel_max(got, want)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_predict_configs_full_and_scalar(cuda_device, cfg):
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host
+
+    p = make_config(cfg)
+    want = oracle.predict(p)                                  # [K, rows, F, 4]
+    got = host(gpu_predict(p, sg.COH_FULL))
+    _check(got, want)
+    # unpolarised: XY = YX = 0 exactly, XX = YY
+    assert np.all(got[..., 1] == 0) and np.all(got[..., 2] == 0) and np.array_equal(got[..., 0], got[..., 3])
+    got_s = host(gpu_predict(p, sg.COH_SCALAR))
+    assert np.array_equal(got_s, got[..., 0])                 # the scalar format is the same numbers
+
+
+@pytest.mark.parametrize("F,uniform", [(1, True), (3, True), (5, False), (9, True), (13, False)])
+def test_predict_polarised_ragged(cuda_device, F, uniform):
+    """Polarised sources (general 2x2 brightness), rows not a multiple of the CTA size, channel counts that are not
+    a multiple of the register tile, non-uniform channel spacing (no recurrence), clusters of unequal size
+    including an empty one."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, host
+
+    rng = np.random.default_rng(100 + F)
+    freqs = np.linspace(120e6, 170e6, F) if uniform else np.sort(rng.uniform(120e6, 170e6, F))
+    if F == 1:
+        freqs = np.array([143.7e6])
+    p = make_problem(11, 3, F, 4, 7, seed=55 + F, polarised=True, layout="disc:20000", field_deg=5.0,
+                     patch_deg=0.7, freqs=freqs)
+    # ragged clusters: sizes 7, 0, 12, 9
+    off = np.array([0, 7, 7, 19, 28], dtype=np.int32)
+    p.cluster_offset = off
+    p.K = 4
+    want = oracle.predict(p)
+    d = {k: dev(getattr(p, k)) for k in ("src_l", "src_m", "src_I", "src_alpha", "src_Q", "src_U", "src_V")}
+    got = host(sg.predict_coherencies(p.N, p.T, p.freqs, p.f0, dev(p.uvw), off, d["src_l"], d["src_m"], d["src_I"],
+                                      d["src_alpha"], d["src_Q"], d["src_U"], d["src_V"]))
+    _check(got, want)
+    assert np.all(got[1] == 0)                                # empty cluster
+
+
+def test_predict_closed_forms_on_gpu(cuda_device):
+    """P1/P2 on the CUDA path itself: a source at the phase centre gives C = B_s (f/f0)^alpha on every row;
+    negating uvw gives the Hermitian transpose."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, host
+
+    p = make_problem(9, 2, 4, 1, 1, seed=9, polarised=True, layout="disc:30000")
+    p.src_l[:] = 0.0
+    p.src_m[:] = 0.0
+    d = {k: dev(getattr(p, k)) for k in ("src_l", "src_m", "src_I", "src_alpha", "src_Q", "src_U", "src_V")}
+    args = (p.N, p.T, p.freqs, p.f0)
+    got = host(sg.predict_coherencies(*args, dev(p.uvw), p.cluster_offset, d["src_l"], d["src_m"], d["src_I"],
+                                      d["src_alpha"], d["src_Q"], d["src_U"], d["src_V"]))[0]
+    sc = (p.freqs / p.f0) ** p.src_alpha[0]
+    I, Q, U, V = p.src_I[0], p.src_Q[0], p.src_U[0], p.src_V[0]
+    Bm = np.array([I + Q, U + 1j * V, U - 1j * V, I - Q])
+    want = np.broadcast_to(sc[None, :, None] * Bm[None, None, :], got.shape)
+    assert rel_max(got, want) < 1e-14
+    # Hermitian symmetry under uvw -> -uvw with sources off centre
+    p2 = make_problem(9, 2, 4, 1, 6, seed=10, polarised=True, layout="disc:30000", field_deg=4.0)
+    d = {k: dev(getattr(p2, k)) for k in ("src_l", "src_m", "src_I", "src_alpha", "src_Q", "src_U", "src_V")}
+    a = host(sg.predict_coherencies(*args, dev(p2.uvw), p2.cluster_offset, d["src_l"], d["src_m"], d["src_I"],
+                                    d["src_alpha"], d["src_Q"], d["src_U"], d["src_V"]))[0]
+    b = host(sg.predict_coherencies(*args, dev(-p2.uvw), p2.cluster_offset, d["src_l"], d["src_m"], d["src_I"],
+                                    d["src_alpha"], d["src_Q"], d["src_U"], d["src_V"]))[0]
+    bh = b.reshape(-1, 4, 2, 2).conj().transpose(0, 1, 3, 2).reshape(b.shape)
+    assert rel_max(a, bh) < 1e-14
+
+
+def test_predict_full_size_sampled(cuda_device):
+    """configs[4] (N=512, T=20, F=8, K=50, S=40) in the launch configuration bench.py times: all 4.19e10 vis*src
+    predicted on the device (scalar format, 16.7 GB), a random sample of rows checked against the oracle."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host
+
+    p = make_config(4)
+    coh = gpu_predict(p, sg.COH_SCALAR)                       # [K, rows, F]
+    rng = np.random.default_rng(4)
+    rows = np.sort(rng.choice(p.rows, 192, replace=False))
+    rows[0], rows[-1] = 0, p.rows - 1
+    want = oracle.predict(p, rows=rows)[..., 0]               # [K, 192, F]
+    import torch
+    got = host(coh[:, torch.from_numpy(rows).to(coh.device), :])
+    _check(got, want)
+    del coh
+    torch.cuda.empty_cache()
+
+
+def test_predict_errors(cuda_device):
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev
+
+    p = make_config(0)
+    d = {k: dev(getattr(p, k)) for k in ("src_l", "src_m", "src_I", "src_alpha")}
+    with pytest.raises(sg.SagecalError) as e:   # bad reference frequency
+        sg.predict_coherencies(p.N, p.T, p.freqs, -1.0, dev(p.uvw), p.cluster_offset, d["src_l"], d["src_m"],
+                               d["src_I"], d["src_alpha"])
+    assert e.value.code == -1
+    with pytest.raises(sg.SagecalError):        # offsets must start at 0 and not decrease
+        sg.predict_coherencies(p.N, p.T, p.freqs, p.f0, dev(p.uvw), [3, 0, 3], d["src_l"], d["src_m"],
+                               d["src_I"], d["src_alpha"])
