@@ -1,0 +1,418 @@
+#!/usr/bin/env python
+"""bench.py -- one calibration interval per step on one B200 (replicas on N GPUs).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--coh full|scalar] [--impl ours|reference]
+
+A step is one pass of the whole hot path over one synthetic interval:
+sagecal_predict_coherencies for all K clusters, then sagecal_sage_calibrate (initial residual, n_em x K x
+[add-back, (n_lm+1) fused cost/gradient/J^H J passes with the device-side LM control, write-back]).
+Workload: BASELINE.json configs[4] (N=512, T=20, F=8, K=50 x 40 sources, 3 EM x 10 LM), the configuration
+north_star's target is quoted on; it fits one GPU (67 GB of 2x2 coherencies).  Inputs are seeded and synthetic
+(sagecal_inputs, recipe in DESIGN.md §4); the visibilities are built on the device by the CUDA path itself.
+
+Prints ONE JSON line (rank 0).  `value` = seconds per interval with inputs resident in HBM; `e2e` = the same through
+sagecal_calibrate_interval_host with pinned HOST buffers (copies inside the timed region); `roofline` = the fused LM
+pass kernel (the dominant kernel: 1650 launches per step) against the measured HBM copy rate, its launch durations
+taken live with CUDA events on the launching stream inside the timed region; `cpu_baseline` = the oracle, as it
+stands, on a bounded sample of the same workload on the host cores.
+
+--impl reference times the oracle (the only other place bench.py executes oracle/) and prints the same line shape.
+Multi-GPU: the path does not shard ("replicas only"): under torchrun every rank calibrates its own
+interval, no data-path collective; time = max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "calib_wall_time_per_interval"
+UNIT = "s"
+FALLBACK_HBM_GBS = 6650.0   # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
+PASS_BYTES_PER_SAMPLE = {"full": 128, "scalar": 80}   # x (64 B) + C (64 B or 16 B): SURVEY.md §8(d), DESIGN.md §6
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# helpers without a GPU in them (covered by tests/test_bench_host.py)
+# ---------------------------------------------------------------------------------------------------------------
+def workload_name(p, coh: str) -> str:
+    return (f"{p.name}: N={p.N} stations, B={p.B} baselines, T={p.T}, F={p.F}, K={p.K} clusters x "
+            f"{p.S_tot // max(p.K, 1)} sources, {p.n_em} EM x {p.n_lm} LM, float64, coherencies {coh}")
+
+
+def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
+    """Fused LM evaluation passes in one interval: n_em * K * (n_lm + 1)  (SURVEY.md §8 size table)."""
+    return n_em * K * (n_lm + 1)
+
+
+def expected_launches(K: int, n_em: int, n_lm: int, trace: bool) -> int:
+    """Kernels one step launches: predict (prep + predict), initial residual, optional ||R||^2 (2),
+    per (em, k): add-back, write-back, (n_lm+1) x (pass, station reduction, LM control)."""
+    return 2 + 1 + (2 if trace else 0) + n_em * K * (2 + 3 * (n_lm + 1))
+
+
+def max_over_ranks(ms: float, world_size: int, device=None) -> float:
+    """Step time of the job = the slowest rank's (all-reduce MAX over the default process group)."""
+    if world_size <= 1:
+        return ms
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device if device is not None else "cpu")
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def seconds_per_interval(ms_per_step: float, n_gpus: int) -> float:
+    """Replicas: every rank finishes one interval per step, so the job finishes n_gpus intervals per step time."""
+    return ms_per_step / 1000.0 / max(n_gpus, 1)
+
+
+def load_peaks() -> tuple[float, str]:
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    try:
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def load_traffic(coh: str):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the LM pass kernel at the bench workload, from the
+    committed ncu --set full summary (profiles/lm_pass_traffic.csv: coh,bytes_read,bytes_write), else None."""
+    path = os.path.join(ROOT, "profiles", "lm_pass_traffic.csv")
+    try:
+        rows = [l.strip().split(",") for l in open(path) if l.strip() and not l.startswith("#")]
+        for r in rows:
+            if r[0] == coh:
+                return float(r[1]) + float(r[2])
+    except Exception:
+        pass
+    return None
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu_index = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.gpu_index), f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line)
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        return parse_clock_lines(self.lines)
+
+
+def parse_clock_lines(lines) -> dict:
+    sm, smax, power, reasons = [], [], [], set()
+    names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+    for line in lines:
+        f = [x.strip() for x in line.split(",")]
+        if len(f) < 9:
+            continue
+        try:
+            sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+        except ValueError:
+            continue
+        for n, v in zip(names, f[5:9]):
+            if v.lower() == "active":
+                reasons.add(n)
+    if not sm:
+        return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+    return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(smax)), "power_w_max": float(max(power)),
+            "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the oracle on a bounded sample of the workload (cpu_baseline leg and --impl reference)
+# ---------------------------------------------------------------------------------------------------------------
+SAMPLE = dict(T=2, K=3, n_em=1, n_lm=3)   # of configs[4]; smaller configs are clipped to their own sizes
+
+
+def oracle_sample(p, sample=None):
+    """Runs the oracle, as it stands, on the first T_s time slots and first K_s clusters of problem `p` with
+    n_em_s x n_lm_s iterations, and scales the measured time to one full interval: predict by samples*sources,
+    calibration by time slots x (corrupt + pass) sweeps.  Returns (seconds_per_interval, description, parts)."""
+    from oracle import oracle
+    from sagecal_inputs import noise_rows
+    s = dict(SAMPLE if sample is None else sample)
+    Ts, Ks = min(s["T"], p.T), min(s["K"], p.K)
+    n_em_s, n_lm_s = min(s["n_em"], p.n_em), min(s["n_lm"], p.n_lm)
+    rows = np.arange(Ts * p.B)                           # row r = t*B + b: the first T_s time slots
+    t0 = time.perf_counter()
+    coh = oracle.predict(p, rows=rows, clusters=range(Ks))
+    t_pred = time.perf_counter() - t0
+    vis = np.zeros((rows.size, p.F, 4), np.complex128)   # input preparation, not timed
+    for k in range(Ks):
+        oracle.corrupt_accumulate(p.N, Ts, p.F, coh[k], p.jones_true[k], +1.0, vis)
+    vis += noise_rows(p, rows)
+    t0 = time.perf_counter()
+    oracle.sage(p.N, Ts, p.F, vis, coh, p.jones_init()[:Ks], n_em_s, n_lm_s, p.tau)
+    t_cal = time.perf_counter() - t0
+    S = p.S_tot // max(p.K, 1)
+    sweeps = lambda K, n_em, n_lm: K + n_em * K * (2 + n_lm + 1)   # initial residual + add-back/write-back + passes
+    f_pred = (p.T / Ts) * (p.K / Ks)
+    f_cal = (p.T / Ts) * sweeps(p.K, p.n_em, p.n_lm) / sweeps(Ks, n_em_s, n_lm_s)
+    total = t_pred * f_pred + t_cal * f_cal
+    desc = (f"first {Ts} of {p.T} time slots x first {Ks} of {p.K} clusters ({S} sources each), predict + "
+            f"{n_em_s} EM x {n_lm_s} LM; measured {t_pred:.2f} s predict + {t_cal:.2f} s calibrate, scaled x{f_pred:.0f} "
+            f"(samples x sources) and x{f_cal:.1f} (time slots x corrupt/pass sweeps) to one interval")
+    return total, desc, dict(predict_s=t_pred, calibrate_s=t_cal, predict_scale=f_pred, calibrate_scale=f_cal)
+
+
+def run_reference(args):
+    """--impl reference: the oracle on the host cores, each step one bounded sample.  Rank 0 only."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return 0
+    from oracle import oracle
+    from sagecal_inputs import make_config
+    oracle.build()
+    p = make_config(args.config)
+    for _ in range(args.warmup):
+        oracle_sample(p)
+    vals, desc = [], ""
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        v, desc, _ = oracle_sample(p)
+        vals.append(v)
+    wall_ms = (time.perf_counter() - t0) * 1000.0 / max(args.steps, 1)
+    value = float(np.mean(vals))
+    cores = oracle.num_threads()
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": wall_ms, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(p, "full"), "note": "each step is a bounded sample scaled to one interval"},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+    return 0
+
+
+# ---------------------------------------------------------------------------------------------------------------
+# the CUDA path
+# ---------------------------------------------------------------------------------------------------------------
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    import paper_1910_13908_b200 as sg
+    from sagecal_inputs import make_config
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the CUDA path has no CPU fallback)")
+    sg.load_library()                                   # raises if libsagecal_b200.so was not built
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    if world != args.gpus and rank == 0:
+        print(f"bench.py: --gpus {args.gpus} but WORLD_SIZE={world}; using WORLD_SIZE", file=sys.stderr)
+
+    # ---- inputs: replicas, every rank its own interval (seed offset by rank) ----
+    p = make_config(args.config, seed=191013908 + args.config + 1000 * rank)
+    fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
+    N, T, F, K = p.N, p.T, p.F, p.K
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    uvw, sl, sm_, sI, sa = t(p.uvw), t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha)
+    coh_shape = (K, p.rows, F, 4) if fmt == sg.COH_FULL else (K, p.rows, F)
+    coh = torch.empty(coh_shape, dtype=torch.complex128, device=dev)
+    predict = lambda: sg.predict_coherencies(N, T, p.freqs, p.f0, uvw, p.cluster_offset, sl, sm_, sI, sa,
+                                             coh_format=fmt, out=coh)
+    predict()
+    noise_host = torch.from_numpy(p.noise()).pin_memory()
+    vis = sg.corrupt_subtract(N, T, F, coh, t(p.jones_true), noise_host.to(dev), sign=+1.0, coh_format=fmt)
+    jones0 = t(p.jones_init())
+    jones = jones0.clone()
+    residual = torch.empty_like(vis)
+    ws = torch.empty(sg.workspace_bytes(2, N, T, F, K), dtype=torch.uint8, device=dev)
+
+    def step():
+        predict()
+        jones.copy_(jones0)
+        return sg.sage_calibrate(N, T, F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+                                 residual=residual, trace=True, workspace=ws)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        out = step()
+    barrier()
+
+    # ---- timed region: device-resident, the LM pass kernel's launches timed live by the library's event pairs ----
+    sg.profile_read()
+    sg.profile_enable(["lm_pass"])
+    launches0 = sg.launch_count()
+    clocks = ClockSampler(local_rank)
+    clocks.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        out = step()
+    e1.record()
+    barrier()
+    ms_per_step = max_over_ranks(e0.elapsed_time(e1) / max(args.steps, 1), world, dev)
+    clk = clocks.stop()
+    gpu_launches = sg.launch_count() - launches0
+    prof = sg.profile_read()
+    sg.profile_enable([])
+    cost_sum = float(out["cost_per_cluster"].sum())
+    trace_last = float(out["cost_trace"][-1])
+
+    # ---- one extra untimed step with every kernel kind timed: where the step's device time goes ----
+    sg.profile_enable(sg.kernel_kinds())
+    step()
+    torch.cuda.synchronize()
+    breakdown = {k: round(v["ms"], 3) for k, v in sg.profile_read().items()}
+    sg.profile_enable([])
+
+    npass = prof["lm_pass"]["timed"]
+    pass_ms = prof["lm_pass"]["ms"] / max(npass, 1)
+    pass_bytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
+    peak, peak_src = load_peaks()
+    achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
+    roofline = {"bound": "hbm", "kernel": "lm_pass_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": load_traffic(args.coh), "peak_source": peak_src,
+                "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,
+                "share_of_step": prof["lm_pass"]["ms"] / max(args.steps, 1) / ms_per_step}
+
+    # ---- end to end: HOST buffers in, HOST buffers out, through sagecal_calibrate_interval_host ----
+    if args.no_e2e:
+        e2e, e2e_cost_sum = None, None
+        return _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown,
+                       pass_bytes, cost_sum, trace_last)
+    vis_host = torch.empty(vis.shape, dtype=vis.dtype).pin_memory()
+    vis_host.copy_(vis)
+    del coh, vis, residual, ws, out, noise_host
+    torch.cuda.empty_cache()
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    h_uvw, h_l, h_m, h_I, h_a = pin(p.uvw), pin(p.src_l), pin(p.src_m), pin(p.src_I), pin(p.src_alpha)
+    h_j0 = pin(p.jones_init())
+    h_j = torch.empty_like(h_j0).pin_memory()
+    h_res = torch.empty(vis_host.shape, dtype=vis_host.dtype).pin_memory()
+    h_cpc = torch.zeros(K, dtype=torch.float64).pin_memory()
+    nbytes = lambda *ts: int(sum(x.numel() * x.element_size() for x in ts))
+    h2d = nbytes(h_uvw, h_l, h_m, h_I, h_a, vis_host, h_j)
+    d2h = nbytes(h_j, h_res, h_cpc)
+
+    def e2e_step():
+        h_j.copy_(h_j0)
+        sg.calibrate_interval_host(N, T, p.freqs, p.f0, h_uvw, p.cluster_offset, h_l, h_m, h_I, h_a, vis_host, h_j,
+                                   p.n_em, p.n_lm, p.tau, coh_format=fmt, residual=h_res, cost_per_cluster=h_cpc)
+
+    for _ in range(args.warmup):
+        e2e_step()
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        e2e_step()                                      # synchronises its stream before returning
+    torch.cuda.synchronize()
+    e2e_ms = max_over_ranks((time.perf_counter() - t0) * 1000.0 / max(args.steps, 1), world, dev)
+    e2e_cost_sum = float(h_cpc.sum())
+    e2e = {"value": seconds_per_interval(e2e_ms, world), "unit": UNIT, "h2d_bytes_per_step": h2d,
+           "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
+           "api": "sagecal_calibrate_interval_host (pinned host buffers in and out)"}
+
+    return _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown,
+                   pass_bytes, cost_sum, trace_last)
+
+
+def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown, pass_bytes,
+            cost_sum, trace_last):
+    import torch.distributed as dist
+    from sagecal_inputs import make_config
+    K = p.K
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- the oracle on the host cores, bounded sample (rank 0, N=1 only) ----
+    cpu_baseline = None
+    if world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle
+        oracle.build()
+        v, desc, _ = oracle_sample(make_config(args.config))
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": desc}
+
+    predict_ms = breakdown.get("predict", 0.0) + breakdown.get("predict_prep", 0.0)
+    line = {
+        "metric": METRIC, "value": seconds_per_interval(ms_per_step, world), "unit": UNIT, "n_gpus": world,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": workload_name(p, args.coh), "parallelism": "replicas only (one interval per GPU)",
+                   "l2": "inputs larger than L2 (per-pass working set %.2f GB vs 126 MB)" % (pass_bytes / 1e9),
+                   "seed": p.seed},
+        "clocks": clk, "e2e": e2e, "gpu_launches": int(gpu_launches),
+        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True),
+        "roofline": roofline, "cpu_baseline": cpu_baseline,
+        "breakdown_ms_one_step": breakdown,
+        "predict_gvis_src_per_s": p.vis_src / (predict_ms * 1e-3) / 1e9 if predict_ms > 0 else None,
+        "check": {"sum_cost_per_cluster": cost_sum, "cost_trace_last": trace_last, "e2e_sum_cost_per_cluster": e2e_cost_sum},
+    }
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+    return 0
+
+
+def main(argv=None):
+    ap = argparse.ArgumentParser(description=__doc__.split("\n\n")[0])
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
+    ap.add_argument("--coh", choices=["full", "scalar"], default="full")
+    ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
+    args = ap.parse_args(argv)
+    if args.impl == "reference":
+        return run_reference(args)
+    return run_ours(args)
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -197,6 +197,22 @@ int sagecal_calibrate_interval_host(
     double* cost_per_cluster_host, double* cost_trace_host, void* stream);
 
 /*
+ * Measurement plumbing (no effect on results).  Every kernel the library launches is counted by kind;
+ * kinds are 0..sagecal_kernel_kinds()-1, named by sagecal_kernel_kind_name() ("predict", "corrupt", "lm_pass", ...).
+ * sagecal_launch_count : kernels launched by this process since the library was loaded (all kinds).
+ * sagecal_profile_enable(mask): from now on bracket every launch whose kind bit is set in `mask` with a CUDA-event
+ *                        pair recorded on the launching stream (mask 0 switches timing off).
+ * sagecal_profile_read : waits for the recorded events, then fills (each host [sagecal_kernel_kinds()], may be NULL)
+ *                        ms_host = summed device time per kind, timed_host = launches timed per kind (both since the
+ *                        previous read), launches_host = launches per kind since load.  Returns 0 or SAGECAL_ECUDA.
+ */
+long long sagecal_launch_count(void);
+int sagecal_kernel_kinds(void);
+const char* sagecal_kernel_kind_name(int kind);
+int sagecal_profile_enable(unsigned kind_mask);
+int sagecal_profile_read(double* ms_host, long long* timed_host, long long* launches_host);
+
+/*
  * Test hook, host only, no device needed: replays the work decomposition of the LM pass kernel.
  * cover : host out [T*B] int32, must be zeroed by the caller; on return every entry must be 1 (each baseline and
  *         time slot visited by exactly one thread of one CTA).

@@ -11,16 +11,21 @@ from ._binding import (  # noqa: F401
     SagecalError,
     calibrate_interval_host,
     corrupt_subtract,
+    kernel_kinds,
+    launch_count,
     lib_path,
     lm_cost_grad_jtj,
     load_library,
     predict_coherencies,
+    profile_enable,
+    profile_read,
     sage_calibrate,
     version,
     workspace_bytes,
 )
 
 __all__ = [
-    "COH_FULL", "COH_SCALAR", "SagecalError", "calibrate_interval_host", "corrupt_subtract", "lib_path",
-    "lm_cost_grad_jtj", "load_library", "predict_coherencies", "sage_calibrate", "version", "workspace_bytes",
+    "COH_FULL", "COH_SCALAR", "SagecalError", "calibrate_interval_host", "corrupt_subtract", "kernel_kinds",
+    "launch_count", "lib_path", "lm_cost_grad_jtj", "load_library", "predict_coherencies", "profile_enable",
+    "profile_read", "sage_calibrate", "version", "workspace_bytes",
 ]

@@ -61,8 +61,46 @@ def load_library():
     L.sagecal_calibrate_interval_host.restype = i
     L.sagecal_calibrate_interval_host.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp,
                                                   i, i, d, vp, vp, vp]
+    L.sagecal_launch_count.restype = ctypes.c_longlong
+    L.sagecal_kernel_kinds.restype = i
+    L.sagecal_kernel_kind_name.restype = ctypes.c_char_p
+    L.sagecal_kernel_kind_name.argtypes = [i]
+    L.sagecal_profile_enable.restype = i
+    L.sagecal_profile_enable.argtypes = [ctypes.c_uint]
+    L.sagecal_profile_read.restype = i
+    L.sagecal_profile_read.argtypes = [vp, vp, vp]
     _lib = L
     return L
+
+
+def launch_count() -> int:
+    """sagecal_launch_count: kernels this process has launched through the library."""
+    return int(load_library().sagecal_launch_count())
+
+
+def kernel_kinds():
+    L = load_library()
+    return [L.sagecal_kernel_kind_name(k).decode() for k in range(L.sagecal_kernel_kinds())]
+
+
+def profile_enable(kinds: Sequence[str] = ()) -> None:
+    """sagecal_profile_enable: time every launch of the named kernel kinds with CUDA events (empty = off)."""
+    names = kernel_kinds()
+    mask = 0
+    for k in kinds:
+        mask |= 1 << names.index(k)
+    _check(load_library().sagecal_profile_enable(mask), "sagecal_profile_enable")
+
+
+def profile_read() -> dict:
+    """sagecal_profile_read: {kind: dict(ms, timed, launches)}; waits for the recorded events."""
+    L = load_library()
+    names = kernel_kinds()
+    ms = np.zeros(len(names), np.float64)
+    timed = np.zeros(len(names), np.int64)
+    launches = np.zeros(len(names), np.int64)
+    _check(L.sagecal_profile_read(ms.ctypes.data, timed.ctypes.data, launches.ctypes.data), "sagecal_profile_read")
+    return {n: dict(ms=float(ms[k]), timed=int(timed[k]), launches=int(launches[k])) for k, n in enumerate(names)}
 
 
 def version() -> str:

@@ -254,10 +254,16 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
         SGC_CUDA(cudaMemcpyAsync(residual, vis, (size_t)samples * 64, cudaMemcpyDeviceToDevice, st));
     }
     if (cost_trace) {
-        norm2_partial_kernel<<<NORM_BLOCKS, NORM_THREADS, 0, st>>>((const double*)residual, samples * 2, w.norm_partial);
-        SGC_LAUNCH_CHECK();
-        norm2_final_kernel<<<1, NORM_THREADS, 0, st>>>(w.norm_partial, NORM_BLOCKS, cost_trace);
-        SGC_LAUNCH_CHECK();
+        {
+            LaunchScope ls(KK_NORM, st);
+            norm2_partial_kernel<<<NORM_BLOCKS, NORM_THREADS, 0, st>>>((const double*)residual, samples * 2, w.norm_partial);
+            SGC_LAUNCH_CHECK();
+        }
+        {
+            LaunchScope ls(KK_NORM, st);
+            norm2_final_kernel<<<1, NORM_THREADS, 0, st>>>(w.norm_partial, NORM_BLOCKS, cost_trace);
+            SGC_LAUNCH_CHECK();
+        }
     }
     int it = 1;
     for (int em = 0; em < n_em; em++) {
@@ -268,11 +274,15 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
             if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, +1.0, residual, residual, st))) return rc;
             // M-step: n_lm trial steps of block-diagonal LM
             if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, Jk, &w.sc->phi, w.G, w.M, st))) return rc;
-            lm_step_kernel<true><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
-                                                         cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
-            SGC_LAUNCH_CHECK();
+            {
+                LaunchScope ls(KK_LMSTEP, st);
+                lm_step_kernel<true><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
+                                                             cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
+                SGC_LAUNCH_CHECK();
+            }
             for (int i = 0; i < n_lm; i++) {
                 if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, w.J_try, &w.sc->phi_try, w.G_try, w.M_try, st))) return rc;
+                LaunchScope ls(KK_LMSTEP, st);
                 lm_step_kernel<false><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
                                                               cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
                 SGC_LAUNCH_CHECK();
@@ -315,6 +325,14 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
                  o_coh = take(coh_bytes), o_jon = take((size_t)K * N * 64), o_cpc = take(sizeof(double) * K),
                  o_trc = take(sizeof(double) * ntrace), o_wsp = take(ws_pred), o_wsc = take(ws_cal);
     char* arena = nullptr;
+    {   // keep the arena in the device's default pool between calls (intervals arrive back to back)
+        int dev = 0;
+        cudaMemPool_t pool;
+        SGC_CUDA(cudaGetDevice(&dev));
+        SGC_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
+        uint64_t keep = UINT64_MAX;
+        SGC_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
+    }
     SGC_CUDA(cudaMallocAsync((void**)&arena, off, st));
     int rc = SAGECAL_OK;
     auto h2d = [&](size_t o, const void* src, size_t n) {

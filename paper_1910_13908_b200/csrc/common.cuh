@@ -21,6 +21,17 @@ inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_
 inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 int num_sms();  // SM count of the current device (cached)
 
+// ---- launch accounting and optional per-kernel CUDA-event timing (profile.cu; sagecal_profile_* in the ABI) ----
+enum KernelKind { KK_PREP = 0, KK_PREDICT, KK_CORRUPT, KK_PASS, KK_REDUCE, KK_LMSTEP, KK_NORM, KK_COUNT };
+// Brackets one kernel launch: counts it, and when timing of its kind is enabled records an event pair on `st`.
+struct LaunchScope {
+    int kind;
+    cudaStream_t st;
+    bool timed;
+    LaunchScope(int kind, cudaStream_t st);
+    ~LaunchScope();
+};
+
 // ---- complex scalars and 2x2 matrices (row-major [XX, XY, YX, YY]) --------------------------------------------
 struct __align__(16) cplx { double re, im; };
 struct __align__(32) d4 { double x, y, z, w; };

@@ -58,6 +58,7 @@ int corrupt_range(int N, int T, int F, int coh_format, const sagecal_c128* coh, 
     const int64_t samples = (int64_t)T * B * F;
     const unsigned grid = (unsigned)((samples + COR_THREADS - 1) / COR_THREADS);
     const bool scalar = coh_format == SAGECAL_COH_SCALAR;
+    LaunchScope ls(KK_CORRUPT, st);
     if (scalar) {
         if (vis_in) corrupt_kernel<true, true><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);
         else corrupt_kernel<true, false><<<grid, COR_THREADS, 0, st>>>(N, F, B, B * F, samples, k0, k1, coh, jones, sign, vis_in, vis_out);

@@ -308,13 +308,19 @@ lm_reduce_kernel(PassGeom g, const double* __restrict__ Ppart, const double* __r
 int enqueue_pass(const PassGeom& g, const PassWorkspace& w, const sagecal_c128* x, int coh_format,
                  const sagecal_c128* coh_k, const sagecal_c128* jones, double* cost, sagecal_c128* grad,
                  sagecal_c128* jtj, cudaStream_t st) {
-    if (coh_format == SAGECAL_COH_SCALAR)
-        lm_pass_kernel<true><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
-    else
-        lm_pass_kernel<false><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
-    SGC_LAUNCH_CHECK();
-    lm_reduce_kernel<<<g.N + 1, RED_THREADS, 0, st>>>(g, w.Ppart, w.Pcost, w.Qpart, cost, grad, jtj);
-    SGC_LAUNCH_CHECK();
+    {
+        LaunchScope ls(KK_PASS, st);
+        if (coh_format == SAGECAL_COH_SCALAR)
+            lm_pass_kernel<true><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
+        else
+            lm_pass_kernel<false><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
+        SGC_LAUNCH_CHECK();
+    }
+    {
+        LaunchScope ls(KK_REDUCE, st);
+        lm_reduce_kernel<<<g.N + 1, RED_THREADS, 0, st>>>(g, w.Ppart, w.Pcost, w.Qpart, cost, grad, jtj);
+        SGC_LAUNCH_CHECK();
+    }
     return SAGECAL_OK;
 }
 

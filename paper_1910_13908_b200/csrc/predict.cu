@@ -158,6 +158,7 @@ template <int FT, bool POL, bool UNIFORM, bool SCALAR>
 static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
                           const PredClusters& cl, const double* uvw, const double* l, const double* m,
                           const double* nm1, const double* flux, sagecal_c128* coh) {
+    LaunchScope ls(KK_PREDICT, st);
     predict_kernel<FT, POL, UNIFORM, SCALAR><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m,
                                                                           nm1, flux, coh);
     SGC_LAUNCH_CHECK();
@@ -226,6 +227,7 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
     double* flux = (double*)((char*)workspace + round_up(sizeof(double) * (size_t)S, 256));
     if (S > 0) {
         const int n = S * Fpad, tb = 256;
+        LaunchScope ls(KK_PREP, st);
         if (pol)
             predict_prep_kernel<4><<<(n + tb - 1) / tb, tb, 0, st>>>(S, F, Fpad, fr, SAGECAL_C0 / f0, src_l, src_m, src_I,
                                                                    src_Q, src_U, src_V, src_alpha, nm1, flux);

@@ -1,0 +1,82 @@
+// Launch accounting and optional per-kernel CUDA-event timing (sagecal_launch_count, sagecal_profile_*).
+// Measurement plumbing for bench.py's `roofline` and `gpu_launches` keys: every kernel launch of the library goes
+// through a LaunchScope, which always counts it and, when timing of its kind is enabled, brackets it with an event
+// pair recorded on the launching stream.  Nothing here touches the data path.
+#include <atomic>
+#include <mutex>
+#include <vector>
+#include "common.cuh"
+
+namespace sgc {
+
+static std::atomic<long long> g_launches[KK_COUNT];
+static std::atomic<unsigned> g_timed_mask{0};
+static std::mutex g_mu;
+struct EvPair { cudaEvent_t a, b; int kind; };
+static std::vector<EvPair> g_pairs;    // recorded since the last read
+static std::vector<EvPair> g_free;     // event pairs ready for reuse
+
+LaunchScope::LaunchScope(int kind_, cudaStream_t st_) : kind(kind_), st(st_), timed(false) {
+    g_launches[kind].fetch_add(1, std::memory_order_relaxed);
+    if (g_timed_mask.load(std::memory_order_relaxed) & (1u << kind)) {
+        std::lock_guard<std::mutex> lk(g_mu);
+        EvPair p;
+        if (!g_free.empty()) { p = g_free.back(); g_free.pop_back(); }
+        else if (cudaEventCreate(&p.a) != cudaSuccess || cudaEventCreate(&p.b) != cudaSuccess) { (void)cudaGetLastError(); return; }
+        p.kind = kind;
+        if (cudaEventRecord(p.a, st) != cudaSuccess) { (void)cudaGetLastError(); g_free.push_back(p); return; }
+        g_pairs.push_back(p);
+        timed = true;
+    }
+}
+LaunchScope::~LaunchScope() {
+    if (timed) {
+        std::lock_guard<std::mutex> lk(g_mu);
+        (void)cudaEventRecord(g_pairs.back().b, st);
+    }
+}
+
+}  // namespace sgc
+
+using namespace sgc;
+
+extern "C" long long sagecal_launch_count(void) {
+    long long n = 0;
+    for (int k = 0; k < KK_COUNT; k++) n += g_launches[k].load();
+    return n;
+}
+
+extern "C" int sagecal_kernel_kinds(void) { return KK_COUNT; }
+
+extern "C" const char* sagecal_kernel_kind_name(int kind) {
+    static const char* names[KK_COUNT] = {"predict_prep", "predict", "corrupt", "lm_pass", "lm_reduce", "lm_step", "norm2"};
+    return kind >= 0 && kind < KK_COUNT ? names[kind] : "?";
+}
+
+extern "C" int sagecal_profile_enable(unsigned kind_mask) {
+    g_timed_mask.store(kind_mask & ((1u << KK_COUNT) - 1));
+    return SAGECAL_OK;
+}
+
+extern "C" int sagecal_profile_read(double* ms_host, long long* timed_host, long long* launches_host) {
+    std::lock_guard<std::mutex> lk(g_mu);
+    for (int k = 0; k < KK_COUNT; k++) {
+        if (ms_host) ms_host[k] = 0.0;
+        if (timed_host) timed_host[k] = 0;
+        if (launches_host) launches_host[k] = g_launches[k].load();
+    }
+    int rc = SAGECAL_OK;
+    for (EvPair& p : g_pairs) {
+        float ms = 0.f;
+        cudaError_t e = cudaEventSynchronize(p.b);
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, p.a, p.b);
+        if (e != cudaSuccess) { rc = cuda_fail(e); (void)cudaGetLastError(); }
+        else {
+            if (ms_host) ms_host[p.kind] += (double)ms;
+            if (timed_host) timed_host[p.kind]++;
+        }
+        g_free.push_back(p);
+    }
+    g_pairs.clear();
+    return rc;
+}
