@@ -40,14 +40,19 @@ METRIC = "calib_wall_time_per_interval"
 UNIT = "s"
 FALLBACK_HBM_GBS = 6650.0   # B200_PROFILING.md fallback, used only if MEASURED_PEAKS.json is absent
 PASS_BYTES_PER_SAMPLE = {"full": 128, "scalar": 80}   # x (64 B) + C (64 B or 16 B): SURVEY.md §8(d), DESIGN.md §6
+# compressed mode's streaming kernel (write-back of the previous cluster + statistics for the next):
+# read R (64 B) + C_prev + C_next (64 B or 16 B each), write R (64 B)
+WBSTAT_BYTES_PER_SAMPLE = {"full": 256, "scalar": 160}
+LM_RECENTRE = 10                                       # SAGECAL_LM_RECENTRE of include/sagecal_b200.h
 
 
 # ---------------------------------------------------------------------------------------------------------------
 # helpers without a GPU in them (covered by tests/test_bench_host.py)
 # ---------------------------------------------------------------------------------------------------------------
-def workload_name(p, coh: str) -> str:
+def workload_name(p, coh: str, lm: str = "") -> str:
     return (f"{p.name}: N={p.N} stations, B={p.B} baselines, T={p.T}, F={p.F}, K={p.K} clusters x "
-            f"{p.S_tot // max(p.K, 1)} sources, {p.n_em} EM x {p.n_lm} LM, float64, coherencies {coh}")
+            f"{p.S_tot // max(p.K, 1)} sources, {p.n_em} EM x {p.n_lm} LM, float64, coherencies {coh}"
+            + (f", lm {lm}" if lm else ""))
 
 
 def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
@@ -55,10 +60,16 @@ def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
     return n_em * K * (n_lm + 1)
 
 
-def expected_launches(K: int, n_em: int, n_lm: int, trace: bool) -> int:
-    """Kernels one step launches: predict (prep + predict), initial residual, optional ||R||^2 (2),
-    per (em, k): add-back, write-back, (n_lm+1) x (pass, station reduction, LM control)."""
-    return 2 + 1 + (2 if trace else 0) + n_em * K * (2 + 3 * (n_lm + 1))
+def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "direct") -> int:
+    """Kernels one step launches: predict (prep + predict), initial residual, optional ||R||^2 (2), then
+    direct:     per (em, k): add-back, write-back, (n_lm+1) x (pass, station reduction, LM control);
+    compressed: gram of the coherencies, per (em, k) and per chunk of LM_RECENTRE trial steps one write-back+statistics
+                kernel and one extra evaluation, (cpass, creduce, LM control) per evaluation, one final write-back."""
+    head = 2 + 1 + (2 if trace else 0)
+    if lm == "direct":
+        return head + n_em * K * (2 + 3 * (n_lm + 1))
+    chunks = max(1, -(-n_lm // LM_RECENTRE))
+    return head + 1 + n_em * K * (chunks + 3 * (n_lm + chunks)) + 1
 
 
 def max_over_ranks(ms: float, world_size: int, device=None) -> float:
@@ -86,10 +97,10 @@ def load_peaks() -> tuple[float, str]:
         return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md 6.65 TB/s)"
 
 
-def load_traffic(coh: str):
-    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the LM pass kernel at the bench workload, from the
-    committed ncu --set full summary (profiles/lm_pass_traffic.csv: coh,bytes_read,bytes_write), else None."""
-    path = os.path.join(ROOT, "profiles", "lm_pass_traffic.csv")
+def load_traffic(coh: str, kernel: str = "lm_pass"):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the named kernel at the bench workload, from the
+    committed ncu --set full summary (profiles/<kernel>_traffic.csv: coh,bytes_read,bytes_write), else None."""
+    path = os.path.join(ROOT, "profiles", f"{kernel}_traffic.csv")
     try:
         rows = [l.strip().split(",") for l in open(path) if l.strip() and not l.startswith("#")]
         for r in rows:
@@ -250,6 +261,9 @@ def run_ours(args):
     # ---- inputs: replicas, every rank its own interval (seed offset by rank) ----
     p = make_config(args.config, seed=191013908 + args.config + 1000 * rank)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
+    lm_mode = sg.LM_COMPRESSED if args.lm == "compressed" else sg.LM_DIRECT
+    # the dominant kernel of the step, the one `roofline` describes
+    top = "wbstat" if args.lm == "compressed" else "lm_pass"
     N, T, F, K = p.N, p.T, p.F, p.K
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     uvw, sl, sm_, sI, sa = t(p.uvw), t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha)
@@ -269,7 +283,7 @@ def run_ours(args):
         predict()
         jones.copy_(jones0)
         return sg.sage_calibrate(N, T, F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
-                                 residual=residual, trace=True, workspace=ws)
+                                 residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
 
     def barrier():
         if world > 1:
@@ -282,7 +296,7 @@ def run_ours(args):
 
     # ---- timed region: device-resident, the LM pass kernel's launches timed live by the library's event pairs ----
     sg.profile_read()
-    sg.profile_enable(["lm_pass"])
+    sg.profile_enable([top])
     launches0 = sg.launch_count()
     clocks = ClockSampler(local_rank)
     clocks.start()
@@ -308,15 +322,22 @@ def run_ours(args):
     breakdown = {k: round(v["ms"], 3) for k, v in sg.profile_read().items()}
     sg.profile_enable([])
 
-    npass = prof["lm_pass"]["timed"]
-    pass_ms = prof["lm_pass"]["ms"] / max(npass, 1)
-    pass_bytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
+    npass = prof[top]["timed"]
+    pass_ms = prof[top]["ms"] / max(npass, 1)
+    if args.lm == "compressed":
+        # per step: n_em*K launches; the first has no write-back (128/80 B per sample), the last no statistics
+        # (192/144 B), the others both: algorithmic bytes per launch = the mean over the step's launches
+        wb, cb = WBSTAT_BYTES_PER_SAMPLE[args.coh], (64 if args.coh == "full" else 16)
+        n_launch = npass // max(args.steps, 1)
+        pass_bytes = ((n_launch - 2) * wb + (64 + cb) + (128 + cb)) * p.samples // max(n_launch, 1)
+    else:
+        pass_bytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
     peak, peak_src = load_peaks()
     achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": "lm_pass_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": load_traffic(args.coh), "peak_source": peak_src,
+    roofline = {"bound": "hbm", "kernel": top + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": load_traffic(args.coh, top), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,
-                "share_of_step": prof["lm_pass"]["ms"] / max(args.steps, 1) / ms_per_step}
+                "share_of_step": prof[top]["ms"] / max(args.steps, 1) / ms_per_step}
 
     # ---- end to end: HOST buffers in, HOST buffers out, through sagecal_calibrate_interval_host ----
     if args.no_e2e:
@@ -340,7 +361,8 @@ def run_ours(args):
     def e2e_step():
         h_j.copy_(h_j0)
         sg.calibrate_interval_host(N, T, p.freqs, p.f0, h_uvw, p.cluster_offset, h_l, h_m, h_I, h_a, vis_host, h_j,
-                                   p.n_em, p.n_lm, p.tau, coh_format=fmt, residual=h_res, cost_per_cluster=h_cpc)
+                                   p.n_em, p.n_lm, p.tau, coh_format=fmt, residual=h_res, cost_per_cluster=h_cpc,
+                                   lm_mode=lm_mode)
 
     for _ in range(args.warmup):
         e2e_step()
@@ -382,11 +404,11 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
         "metric": METRIC, "value": seconds_per_interval(ms_per_step, world), "unit": UNIT, "n_gpus": world,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": workload_name(p, args.coh), "parallelism": "replicas only (one interval per GPU)",
+        "config": {"workload": workload_name(p, args.coh, args.lm), "parallelism": "replicas only (one interval per GPU)",
                    "l2": "inputs larger than L2 (per-pass working set %.2f GB vs 126 MB)" % (pass_bytes / 1e9),
                    "seed": p.seed},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(gpu_launches),
-        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True),
+        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True, args.lm),
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "breakdown_ms_one_step": breakdown,
         "predict_gvis_src_per_s": p.vis_src / (predict_ms * 1e-3) / 1e9 if predict_ms > 0 else None,
@@ -405,6 +427,8 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--coh", choices=["full", "scalar"], default="full")
+    ap.add_argument("--lm", choices=["compressed", "direct"], default="compressed",
+                    help="lm_mode of sagecal_sage_calibrate (DESIGN.md §5.5); direct = every evaluation streams the samples")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")

@@ -57,6 +57,15 @@ typedef struct { double re, im; } sagecal_c128;
 #define SAGECAL_COH_FULL   0
 #define SAGECAL_COH_SCALAR 1
 
+/* `lm_mode` of sagecal_sage_calibrate: how the n_lm+1 cost/gradient/J^H J evaluations of an M-step are computed.
+ * Both follow the same LM trajectory and agree to rounding. */
+#define SAGECAL_LM_COMPRESSED 0  /* default: per-baseline time/frequency statistics of the residual, taken once per
+                                    (EM iteration, cluster) in the same streaming kernel that writes back the previous
+                                    cluster; the evaluations then read 392 B per baseline instead of 128 B per sample */
+#define SAGECAL_LM_DIRECT     1  /* every evaluation streams the cluster's T*F samples (sagecal_lm_cost_grad_jtj) */
+/* compressed mode re-takes the statistics at the accepted Jones every this many trial steps of one M-step */
+#define SAGECAL_LM_RECENTRE  10
+
 /* `what` of sagecal_workspace_bytes */
 #define SAGECAL_WS_LM_PASS   1
 #define SAGECAL_WS_CALIBRATE 2
@@ -166,6 +175,7 @@ int sagecal_lm_cost_grad_jtj(
  * jones   : dev [K][N][4], in = start values, out = solution.
  * residual: dev out [rows][F][4]; must not alias vis.
  * tau     : initial damping factor (1e-3 in all configs).
+ * lm_mode : SAGECAL_LM_COMPRESSED or SAGECAL_LM_DIRECT (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
  * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
  * No device->host transfer or synchronisation happens inside the call.
@@ -174,7 +184,7 @@ int sagecal_sage_calibrate(
     int nstations, int ntime, int nchan, int nclus,
     const sagecal_c128* vis, int coh_format, const sagecal_c128* coh,
     sagecal_c128* jones, sagecal_c128* residual,
-    int n_em, int n_lm, double tau,
+    int n_em, int n_lm, double tau, int lm_mode,
     double* cost_per_cluster, double* cost_trace,
     void* workspace, size_t workspace_bytes, void* stream);
 
@@ -193,7 +203,7 @@ int sagecal_calibrate_interval_host(
     const double* src_Q, const double* src_U, const double* src_V, const double* src_alpha,
     int coh_format,
     const sagecal_c128* vis_host, sagecal_c128* jones_host, sagecal_c128* residual_host,
-    int n_em, int n_lm, double tau,
+    int n_em, int n_lm, double tau, int lm_mode,
     double* cost_per_cluster_host, double* cost_trace_host, void* stream);
 
 /*
@@ -220,6 +230,14 @@ int sagecal_profile_read(double* ms_host, long long* timed_host, long long* laun
  * Returns 0, SAGECAL_EINVAL, or a positive bit mask naming the violated bookkeeping invariant.
  */
 int sagecal_debug_pass_cover(int nstations, int ntime, int nchan, int32_t* cover, int64_t* info);
+
+/*
+ * Test hook, host only: replays the tiling of the compressed evaluation pass and the record lists of
+ * its station reduction.  cover : host out [B] int32, zeroed by the caller; every entry must come back 1.
+ * info : host out [4] int64 = {q tiles, p blocks, live tiles, B}.  Returns 0, SAGECAL_EINVAL, or a positive bit mask
+ * (1/4: a row/column record is read but never written; 2/8: a record that carries a baseline is never read).
+ */
+int sagecal_debug_cpass_cover(int nstations, int32_t* cover, int64_t* info);
 
 #ifdef __cplusplus
 }

@@ -10,6 +10,8 @@ import torch
 
 COH_FULL = 0
 COH_SCALAR = 1
+LM_COMPRESSED = 0
+LM_DIRECT = 1
 WS_LM_PASS = 1
 WS_CALIBRATE = 2
 
@@ -57,10 +59,10 @@ def load_library():
     L.sagecal_lm_cost_grad_jtj.restype = i
     L.sagecal_lm_cost_grad_jtj.argtypes = [i, i, i, vp, i, vp, vp, vp, vp, vp, vp, sz, vp]
     L.sagecal_sage_calibrate.restype = i
-    L.sagecal_sage_calibrate.argtypes = [i, i, i, i, vp, i, vp, vp, vp, i, i, d, vp, vp, vp, sz, vp]
+    L.sagecal_sage_calibrate.argtypes = [i, i, i, i, vp, i, vp, vp, vp, i, i, d, i, vp, vp, vp, sz, vp]
     L.sagecal_calibrate_interval_host.restype = i
     L.sagecal_calibrate_interval_host.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp,
-                                                  i, i, d, vp, vp, vp]
+                                                  i, i, d, i, vp, vp, vp]
     L.sagecal_launch_count.restype = ctypes.c_longlong
     L.sagecal_kernel_kinds.restype = i
     L.sagecal_kernel_kind_name.restype = ctypes.c_char_p
@@ -233,7 +235,7 @@ def lm_cost_grad_jtj(N: int, T: int, F: int, x: torch.Tensor, coh_k: torch.Tenso
 def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor, jones: torch.Tensor,
                    n_em: int, n_lm: int, tau: float = 1e-3, coh_format: int = COH_FULL,
                    residual: Optional[torch.Tensor] = None, trace: bool = True, workspace: Optional[torch.Tensor] = None,
-                   stream=None):
+                   lm_mode: int = LM_COMPRESSED, stream=None):
     """sagecal_sage_calibrate.  `jones` [K,N,2,2] is updated in place.
     Returns dict(jones, residual, cost_per_cluster [K], cost_trace [n_em*K+1] or None), all device tensors."""
     L = load_library()
@@ -256,7 +258,7 @@ def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor,
         raise ValueError("workspace too small")
     rc = L.sagecal_sage_calibrate(N, T, F, K, _dev(vis, c128, "vis"), coh_format,
                                   _dev(coh, c128, "coh") if K else None, _dev(jones, c128, "jones") if K else None,
-                                  _dev(residual, c128, "residual"), int(n_em), int(n_lm), float(tau),
+                                  _dev(residual, c128, "residual"), int(n_em), int(n_lm), float(tau), int(lm_mode),
                                   cpc.data_ptr(), tr.data_ptr() if tr is not None else None,
                                   ws.data_ptr(), ws.numel(), _stream(stream))
     _check(rc, "sagecal_sage_calibrate")
@@ -277,7 +279,7 @@ def calibrate_interval_host(N: int, T: int, freqs: Sequence[float], f0: float, u
                             cluster_offset: Sequence[int], src_l, src_m, src_I, src_alpha, vis: torch.Tensor,
                             jones: torch.Tensor, n_em: int, n_lm: int, tau: float = 1e-3, src_Q=None, src_U=None,
                             src_V=None, coh_format: int = COH_FULL, residual: Optional[torch.Tensor] = None,
-                            cost_per_cluster: Optional[torch.Tensor] = None, stream=None):
+                            cost_per_cluster: Optional[torch.Tensor] = None, lm_mode: int = LM_COMPRESSED, stream=None):
     """sagecal_calibrate_interval_host: predict + calibrate from HOST tensors (copies inside the call).
     `jones` (CPU, [K,N,2,2]) is updated in place; `residual` (CPU) is filled if given."""
     L = load_library()
@@ -292,7 +294,7 @@ def calibrate_interval_host(N: int, T: int, freqs: Sequence[float], f0: float, u
     rc = L.sagecal_calibrate_interval_host(
         N, T, F, fr.ctypes.data, float(f0), _host(uvw, f64, "uvw")[0], K, co.ctypes.data, *ptrs, coh_format,
         _host(vis, c128, "vis")[0], _host(jones, c128, "jones")[0], _host(residual, c128, "residual")[0],
-        int(n_em), int(n_lm), float(tau), _host(cost_per_cluster, f64, "cost_per_cluster")[0], None,
+        int(n_em), int(n_lm), float(tau), int(lm_mode), _host(cost_per_cluster, f64, "cost_per_cluster")[0], None,
         _stream(stream))
     _check(rc, "sagecal_calibrate_interval_host")
     return dict(jones=jones, residual=residual, cost_per_cluster=cost_per_cluster)

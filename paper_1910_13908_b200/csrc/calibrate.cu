@@ -4,6 +4,7 @@
 #include <math.h>
 #include <string.h>
 #include "lm_pass.cuh"
+#include "compress.cuh"
 
 namespace sgc {
 
@@ -60,27 +61,40 @@ __device__ __forceinline__ double block_max(double v, double* s_buf) {
     return r;
 }
 
-// INIT:   (phi, G, M) were just evaluated at J.  mu = tau*max_p max(M_p00, M_p11), nu = 2; first trial step.
-// !INIT:  (phi_try, G_try, M_try) were just evaluated at J_try.  rho test, accept/reject, damping update; next
-//         trial step.  dJ_p = G_p (M_p + mu I)^-1, J_try = J + dJ, pred = sum_p Re tr(G_p^H dJ_p) + mu ||dJ_p||^2.
-template <bool INIT>
+// LM_INIT:     (phi, G, M) were just evaluated at J.  mu = tau*max_p max(M_p00, M_p11), nu = 2; first trial step.
+// LM_TRIAL:    (phi_try, G_try, M_try) were just evaluated at J_try.  rho test, accept/reject, damping update; next
+//              trial step.  dJ_p = G_p (M_p + mu I)^-1, J_try = J + dJ, pred = sum_p Re tr(G_p^H dJ_p) + mu ||dJ_p||^2.
+// LM_RECENTRE: (phi, G, M) were re-evaluated at the accepted J from fresh statistics (compressed mode, long
+//              M-steps); mu, nu are kept, the pending trial step is recomputed.
+// cost_st != NULL (compressed mode): the cost just evaluated is sum_p cost_st[p] (fixed-order block sum) instead of
+// sc->phi / sc->phi_try.
+enum { LM_TRIAL = 0, LM_INIT = 1, LM_RECENTRE = 2 };
+template <int MODE>
 __global__ void __launch_bounds__(LM_THREADS)
 lm_step_kernel(int N, double tau, LmScalars* __restrict__ sc, sagecal_c128* __restrict__ J,
                sagecal_c128* __restrict__ G, sagecal_c128* __restrict__ M, const sagecal_c128* __restrict__ G_try,
                const sagecal_c128* __restrict__ M_try, sagecal_c128* __restrict__ J_try,
-               double* __restrict__ cost_out, double* __restrict__ trace_out) {
+               const double* __restrict__ cost_st, double* __restrict__ cost_out, double* __restrict__ trace_out) {
     __shared__ double s_buf[LM_THREADS];
     const int tid = threadIdx.x;
-    double phi = sc->phi, mu, nu;
+    double fresh = 0.0;
+    if (cost_st) {
+        double part = 0.0;
+        for (int p = tid; p < N; p += LM_THREADS) part += cost_st[p];
+        fresh = block_sum(part, s_buf);
+    }
+    double phi = MODE == LM_TRIAL ? sc->phi : (cost_st ? fresh : sc->phi), mu, nu;
     bool accept = false;
-    if (INIT) {
+    if (MODE == LM_RECENTRE) {
+        mu = sc->mu; nu = sc->nu;
+    } else if (MODE == LM_INIT) {
         double mmax = 0.0;
         for (int p = tid; p < N; p += LM_THREADS) mmax = fmax(mmax, fmax(M[4 * p].re, M[4 * p + 3].re));
         mmax = block_max(mmax, s_buf);
         mu = tau * mmax;
         nu = 2.0;
     } else {
-        const double phin = sc->phi_try, pred = sc->pred;
+        const double phin = cost_st ? fresh : sc->phi_try, pred = sc->pred;
         mu = sc->mu; nu = sc->nu;
         const double rho = (phi - phin) / pred;
         accept = isfinite(phin) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
@@ -181,11 +195,12 @@ struct CalWorkspace {
     LmScalars* sc;
     sagecal_c128 *G, *M, *G_try, *M_try, *J_try;
     double* norm_partial;
+    CompressWorkspace cw;
 };
 static size_t cal_extra_bytes(int N) {
     return 256 + 5 * round_up((size_t)N * 64, 256) + round_up(sizeof(double) * NORM_BLOCKS, 256);
 }
-static CalWorkspace carve_cal(const PassGeom& g, void* ws) {
+static CalWorkspace carve_cal(const PassGeom& g, int K, bool scalar, void* ws) {
     CalWorkspace w;
     w.pass = carve_pass_workspace(g, ws);
     char* p = (char*)ws + pass_workspace_bytes(g);
@@ -196,8 +211,19 @@ static CalWorkspace carve_cal(const PassGeom& g, void* ws) {
     w.G_try = (sagecal_c128*)p; p += nj;
     w.M_try = (sagecal_c128*)p; p += nj;
     w.J_try = (sagecal_c128*)p; p += nj;
-    w.norm_partial = (double*)p;
+    w.norm_partial = (double*)p; p += round_up(sizeof(double) * NORM_BLOCKS, 256);
+    w.cw = carve_compress(g.N, K, scalar, p);
     return w;
+}
+
+template <int MODE>
+static int enqueue_step(int N, double tau, const CalWorkspace& w, sagecal_c128* Jk, const double* cost_st,
+                        double* cost_out, double* trace_out, cudaStream_t st) {
+    LaunchScope ls(KK_LMSTEP, st);
+    lm_step_kernel<MODE><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try, cost_st,
+                                                  cost_out, trace_out);
+    SGC_LAUNCH_CHECK();
+    return SAGECAL_OK;
 }
 
 }  // namespace sgc
@@ -215,36 +241,38 @@ extern "C" const char* sagecal_strerror(int code) {
     }
 }
 extern "C" int sagecal_last_cuda_error(void) { return g_last_cuda_error; }
-extern "C" const char* sagecal_version(void) { return "0.1.0"; }
+extern "C" const char* sagecal_version(void) { return "0.2.0"; }
 
 extern "C" size_t sagecal_workspace_bytes(int what, int N, int T, int F, int K) {
-    (void)K;
-    if (N < 2 || T < 1 || F < 1) return 0;
+    if (N < 2 || T < 1 || F < 1 || K < 0) return 0;
     const PassGeom g = make_pass_geom(N, T, F);
     switch (what) {
         case SAGECAL_WS_LM_PASS: return pass_workspace_bytes(g);
-        case SAGECAL_WS_CALIBRATE: return pass_workspace_bytes(g) + cal_extra_bytes(N);
+        // sized for either lm_mode and either coherency format (the general 2x2 statistics are the larger)
+        case SAGECAL_WS_CALIBRATE: return pass_workspace_bytes(g) + cal_extra_bytes(N) + compress_workspace_bytes(N, K, false);
         default: return 0;
     }
 }
 
 extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_c128* vis, int coh_format,
                                       const sagecal_c128* coh, sagecal_c128* jones, sagecal_c128* residual, int n_em,
-                                      int n_lm, double tau, double* cost_per_cluster, double* cost_trace,
+                                      int n_lm, double tau, int lm_mode, double* cost_per_cluster, double* cost_trace,
                                       void* workspace, size_t workspace_bytes, void* stream) {
     if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
+    if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT) return SAGECAL_EINVAL;
     if (!vis || !residual || vis == residual || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
     if (K > 0 && (!coh || !jones || !cost_per_cluster)) return SAGECAL_EINVAL;
     if (K > 0 && (!aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32) || !aligned(jones, 16))) return SAGECAL_EINVAL;
     if (!(tau > 0.0) || !isfinite(tau)) return SAGECAL_EINVAL;
     const PassGeom g = make_pass_geom(N, T, F);
-    if (!workspace || !aligned(workspace, 256) || workspace_bytes < pass_workspace_bytes(g) + cal_extra_bytes(N))
+    if (!workspace || !aligned(workspace, 256) || workspace_bytes < sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE, N, T, F, K))
         return SAGECAL_EWORKSPACE;
-    const CalWorkspace w = carve_cal(g, workspace);
+    const bool scalar = coh_format == SAGECAL_COH_SCALAR;
+    const CalWorkspace w = carve_cal(g, K, scalar, workspace);
     cudaStream_t st = (cudaStream_t)stream;
     const int64_t samples = (int64_t)T * g.B * F;
-    const size_t cstride = coh_format == SAGECAL_COH_SCALAR ? (size_t)samples : (size_t)samples * 4;
+    const size_t cstride = scalar ? (size_t)samples : (size_t)samples * 4;
     int rc;
 
     // R = V - sum_k J_k C_k J_k^H
@@ -265,31 +293,72 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
             SGC_LAUNCH_CHECK();
         }
     }
+    if (K == 0 || n_em == 0) return SAGECAL_OK;
+
+    if (lm_mode == SAGECAL_LM_DIRECT) {
+        // every LM evaluation streams the T*F samples of the cluster (rows 8a-3, 8a-4, 8a-6 as written)
+        int it = 1;
+        for (int em = 0; em < n_em; em++) {
+            for (int k = 0; k < K; k++, it++) {
+                const sagecal_c128* Ck = coh + (size_t)k * cstride;
+                sagecal_c128* Jk = jones + (size_t)k * N * 4;
+                double* tr = cost_trace ? cost_trace + it : nullptr;
+                // E-step: x_k = R + J_k C_k J_k^H (in place: `residual` holds x_k during the M-step)
+                if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, +1.0, residual, residual, st))) return rc;
+                // M-step: n_lm trial steps of block-diagonal LM
+                if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, Jk, &w.sc->phi, w.G, w.M, st))) return rc;
+                if ((rc = enqueue_step<LM_INIT>(N, tau, w, Jk, nullptr, cost_per_cluster + k, tr, st))) return rc;
+                for (int i = 0; i < n_lm; i++) {
+                    if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, w.J_try, &w.sc->phi_try, w.G_try, w.M_try, st))) return rc;
+                    if ((rc = enqueue_step<LM_TRIAL>(N, tau, w, Jk, nullptr, cost_per_cluster + k, tr, st))) return rc;
+                }
+                // R = x_k - J_k C_k J_k^H at the new J_k
+                if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, -1.0, residual, residual, st))) return rc;
+            }
+        }
+        return SAGECAL_OK;
+    }
+
+    // compressed mode: `residual` always holds R; per (em, k) one streaming kernel writes back the
+    // previous cluster and takes the statistics of the new residual against C_k, then the n_lm+1 evaluations run on
+    // the per-baseline statistics.  Statistics are re-centred every SAGECAL_LM_RECENTRE trial steps.
+    const CGeom cg = make_cgeom(N);
+    if ((rc = enqueue_gram(N, T, F, K, coh_format, coh, w.cw.Scc, st))) return rc;
+    const sagecal_c128* Cprev = nullptr;      // cluster whose write-back is pending
+    const sagecal_c128* Jprev = nullptr;
+    int par = 0;
     int it = 1;
     for (int em = 0; em < n_em; em++) {
         for (int k = 0; k < K; k++, it++) {
             const sagecal_c128* Ck = coh + (size_t)k * cstride;
             sagecal_c128* Jk = jones + (size_t)k * N * 4;
-            // E-step: x_k = R + J_k C_k J_k^H (in place: `residual` holds x_k during the M-step)
-            if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, +1.0, residual, residual, st))) return rc;
-            // M-step: n_lm trial steps of block-diagonal LM
-            if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, Jk, &w.sc->phi, w.G, w.M, st))) return rc;
-            {
-                LaunchScope ls(KK_LMSTEP, st);
-                lm_step_kernel<true><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
-                                                             cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
-                SGC_LAUNCH_CHECK();
-            }
-            for (int i = 0; i < n_lm; i++) {
-                if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, w.J_try, &w.sc->phi_try, w.G_try, w.M_try, st))) return rc;
-                LaunchScope ls(KK_LMSTEP, st);
-                lm_step_kernel<false><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try,
-                                                              cost_per_cluster + k, cost_trace ? cost_trace + it : nullptr);
-                SGC_LAUNCH_CHECK();
-            }
-            // R = x_k - J_k C_k J_k^H at the new J_k
-            if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, -1.0, residual, residual, st))) return rc;
+            const double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * cg.B;
+            double* tr = cost_trace ? cost_trace + it : nullptr;
+            int done = 0;
+            do {
+                sagecal_c128* J0 = w.cw.J0 + (size_t)par * N * 4;
+                const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
+                if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, w.cw.srr, st))) return rc;
+                SGC_CUDA(cudaMemcpyAsync(J0, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
+                if ((rc = enqueue_cpass(cg, w.cw, scalar, Scc_k, J0, J0, w.G, w.M, st))) return rc;
+                if (done == 0) rc = enqueue_step<LM_INIT>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st);
+                else rc = enqueue_step<LM_RECENTRE>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st);
+                if (rc) return rc;
+                const int chunk = n_lm - done < SAGECAL_LM_RECENTRE ? n_lm - done : SAGECAL_LM_RECENTRE;
+                for (int i = 0; i < chunk; i++) {
+                    if ((rc = enqueue_cpass(cg, w.cw, scalar, Scc_k, J0, w.J_try, w.G_try, w.M_try, st))) return rc;
+                    if ((rc = enqueue_step<LM_TRIAL>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st))) return rc;
+                }
+                done += chunk;
+                Cprev = Ck; Jprev = Jk;
+                par ^= 1;
+            } while (done < n_lm);
         }
+    }
+    // last write-back: R -= dW c of the cluster solved last
+    {
+        const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
+        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, w.cw.srr, st))) return rc;
     }
     return SAGECAL_OK;
 }
@@ -300,7 +369,7 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
                                                const double* src_Q, const double* src_U, const double* src_V,
                                                const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
                                                sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
-                                               int n_lm, double tau, double* cost_per_cluster_host,
+                                               int n_lm, double tau, int lm_mode, double* cost_per_cluster_host,
                                                double* cost_trace_host, void* stream) {
     if (N < 2 || T < 1 || F < 1 || K < 1 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (!freqs_host || !uvw_host || !cluster_offset_host || !vis_host || !jones_host || !cost_per_cluster_host)
@@ -358,7 +427,7 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     if (rc == SAGECAL_OK)
         rc = sagecal_sage_calibrate(N, T, F, K, (const sagecal_c128*)(arena + o_vis), coh_format,
                                     (const sagecal_c128*)(arena + o_coh), (sagecal_c128*)(arena + o_jon),
-                                    (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, (double*)(arena + o_cpc),
+                                    (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, lm_mode, (double*)(arena + o_cpc),
                                     cost_trace_host ? (double*)(arena + o_trc) : nullptr, arena + o_wsc, ws_cal, st);
     auto d2h = [&](void* dst, size_t o, size_t n) {
         if (rc == SAGECAL_OK && dst && n) {

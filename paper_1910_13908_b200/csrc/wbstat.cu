@@ -1,0 +1,229 @@
+// Per-baseline statistics of the compressed M-step, fused with the previous cluster's write-back
+// (SURVEY.md §8(a) rows 8a-3 / 8a-6 re-associated; formulas in compress.cuh).
+//
+//   wbstat:  R <- R - dW_prev c_prev   (write-back of the cluster just solved, dW_prev = W(J_prev) - W(J0_prev))
+//            Src = sum_tf r c_next^H,  srr = sum_tf |r|^2   (statistics of the new residual for the next cluster)
+//   gram:    Scc_k = sum_tf c_k c_k^H for every cluster (depends on the coherencies only: once per interval)
+//
+// HBM-bound streaming kernels: one thread owns one (baseline, channel) and walks the time slots, so at fixed t a
+// warp reads 32 consecutive samples (2 KB, 256-bit loads); sums stay in registers over the time loop and are
+// combined across the F lanes of a baseline with warp shuffles -- no atomics, fixed order.
+#include "compress.cuh"
+
+namespace sgc {
+
+constexpr int WS_THREADS = 128;
+
+__device__ __forceinline__ double group_sum(double v, int FP) {  // butterfly over the FP (power of two) lanes of a baseline
+    for (int o = FP >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// dW[a][c] (a = 2i+j, c = 2k+l) = D_p[i,k] conj(J0_q[j,l]) + J_p[i,k] conj(D_q[j,l])
+__device__ __forceinline__ cplx dW_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
+                                         int q, int a, int c) {
+    const int i = a >> 1, j = a & 1, k = c >> 1, l = c & 1;
+    const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
+    const sagecal_c128 jq0 = J0[4 * q + 2 * j + l], jq = J[4 * q + 2 * j + l];
+    const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
+    return cfmac(mk(jp.re, jp.im), Dq, cmulc(Dp, mk(jq0.re, jq0.im)));
+}
+// dP[a] (a = 2i+j) = (D_p J0_q^H + J_p D_q^H)[i,j]
+__device__ __forceinline__ cplx dP_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
+                                         int q, int a) {
+    const int i = a >> 1, j = a & 1;
+    cplx acc = mk(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
+        const sagecal_c128 jq0 = J0[4 * q + 2 * j + k], jq = J[4 * q + 2 * j + k];
+        const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
+        acc = cfmac(mk(jp.re, jp.im), Dq, cfmac(Dp, mk(jq0.re, jq0.im), acc));
+    }
+    return acc;
+}
+
+template <bool SCALAR, bool HAS_PREV, bool HAS_NEXT>
+__global__ void __launch_bounds__(WS_THREADS, SCALAR ? 4 : 3)
+wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ Cprev,
+              const sagecal_c128* __restrict__ J0prev, const sagecal_c128* __restrict__ Jprev,
+              const sagecal_c128* __restrict__ Cnext, double* __restrict__ Src, double* __restrict__ srr) {
+    constexpr int NW = SCALAR ? 4 : 16;                 // entries of dP / dW per baseline
+    __shared__ cplx s_dw[HAS_PREV ? NW : 1][HAS_PREV ? WS_THREADS : 1];   // [entry][baseline of this CTA]
+    const int tid = threadIdx.x;
+    const int BL = WS_THREADS / FP;                      // baselines per CTA
+    const int g = tid / FP, fl = tid - g * FP;
+    const int64_t b = (int64_t)blockIdx.x * BL + g;
+
+    if (HAS_PREV) {
+        for (int e = tid; e < BL * NW; e += WS_THREADS) {
+            const int bl = e / NW, w = e - bl * NW;
+            const int64_t bb = (int64_t)blockIdx.x * BL + bl;
+            cplx v = mk(0.0, 0.0);
+            if (bb < B) {
+                int p, q;
+                bl_stations(N, bb, p, q);
+                v = SCALAR ? dP_entry(J0prev, Jprev, p, q, w) : dW_entry(J0prev, Jprev, p, q, w >> 2, w & 3);
+            }
+            s_dw[w][bl] = v;
+        }
+        __syncthreads();
+    }
+
+    constexpr int NS = SCALAR ? 4 : 16;
+    cplx S[HAS_NEXT ? NS : 1];
+    double rr = 0.0;
+#pragma unroll
+    for (int i = 0; i < (HAS_NEXT ? NS : 1); i++) S[i] = mk(0.0, 0.0);
+
+    if (b < B) {
+        for (int f = fl; f < F; f += FP) {
+            size_t idx = (size_t)b * F + f;
+            const size_t step = (size_t)B * F;
+#pragma unroll 1
+            for (int t = 0; t < T; t++, idx += step) {
+                m22 r;
+                load_m22(R + idx * 4, r);
+                if (HAS_PREV) {
+                    if (SCALAR) {
+                        const cplx cp = ldg128_stream(Cprev + idx);
+#pragma unroll
+                        for (int a = 0; a < 4; a++) r.a[a] = cfms(s_dw[a][g], cp, r.a[a]);
+                    } else {
+                        m22 cp;
+                        load_m22_stream(Cprev + idx * 4, cp);
+#pragma unroll
+                        for (int a = 0; a < 4; a++) {
+#pragma unroll
+                            for (int c = 0; c < 4; c++) r.a[a] = cfms(s_dw[4 * a + c][g], cp.a[c], r.a[a]);
+                        }
+                    }
+                    store_m22(R + idx * 4, r);
+                }
+                if (HAS_NEXT) {
+                    if (SCALAR) {
+                        const cplx cn = ldg128_stream(Cnext + idx);
+#pragma unroll
+                        for (int a = 0; a < 4; a++) S[a] = cfmac(r.a[a], cn, S[a]);
+                    } else {
+                        m22 cn;
+                        load_m22_stream(Cnext + idx * 4, cn);
+#pragma unroll
+                        for (int a = 0; a < 4; a++) {
+#pragma unroll
+                            for (int c = 0; c < 4; c++) S[4 * a + c] = cfmac(r.a[a], cn.a[c], S[4 * a + c]);
+                        }
+                    }
+                    rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
+                }
+            }
+        }
+    }
+    if (HAS_NEXT) {
+        // all 32 lanes take part (lanes of a missing baseline carry zeros)
+#pragma unroll
+        for (int i = 0; i < NS; i++) {
+            const double re = group_sum(S[i].re, FP), im = group_sum(S[i].im, FP);
+            if (fl == 0 && b < B) {
+                Src[(size_t)(2 * i) * B + b] = re;
+                Src[(size_t)(2 * i + 1) * B + b] = im;
+            }
+        }
+        rr = group_sum(rr, FP);
+        if (fl == 0 && b < B) srr[b] = rr;
+    }
+}
+
+// Scc_k for every cluster: grid.y = cluster
+template <bool SCALAR>
+__global__ void __launch_bounds__(WS_THREADS, 4)
+gram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, double* __restrict__ Scc) {
+    const int tid = threadIdx.x;
+    const int BL = WS_THREADS / FP;
+    const int g = tid / FP, fl = tid - g * FP;
+    const int64_t b = (int64_t)blockIdx.x * BL + g;
+    const size_t samples = (size_t)T * B * F;
+    const sagecal_c128* C = coh + (size_t)blockIdx.y * samples * (SCALAR ? 1 : 4);
+    double* out = Scc + (size_t)blockIdx.y * nscc(SCALAR) * B;
+    double acc[SCALAR ? 1 : 16];
+#pragma unroll
+    for (int i = 0; i < (SCALAR ? 1 : 16); i++) acc[i] = 0.0;
+    if (b < B) {
+        for (int f = fl; f < F; f += FP) {
+            size_t idx = (size_t)b * F + f;
+            const size_t step = (size_t)B * F;
+#pragma unroll 4
+            for (int t = 0; t < T; t++, idx += step) {
+                if (SCALAR) {
+                    acc[0] = cabs2(ldg128_stream(C + idx), acc[0]);
+                } else {
+                    m22 c;
+                    load_m22_stream(C + idx * 4, c);
+#pragma unroll
+                    for (int a = 0; a < 4; a++) acc[a] = cabs2(c.a[a], acc[a]);
+                    int pr = 0;
+#pragma unroll
+                    for (int a = 0; a < 4; a++) {
+#pragma unroll
+                        for (int c2 = a + 1; c2 < 4; c2++, pr++) {
+                            const cplx s = cfmac(c.a[a], c.a[c2], mk(acc[4 + 2 * pr], acc[5 + 2 * pr]));
+                            acc[4 + 2 * pr] = s.re;
+                            acc[5 + 2 * pr] = s.im;
+                        }
+                    }
+                }
+            }
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < (SCALAR ? 1 : 16); i++) {
+        const double v = group_sum(acc[i], FP);
+        if (fl == 0 && b < B) out[(size_t)i * B + b] = v;
+    }
+}
+
+int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128* coh, double* Scc, cudaStream_t st) {
+    if (K <= 0) return SAGECAL_OK;
+    const int64_t B = (int64_t)N * (N - 1) / 2;
+    const int FP = stat_group(F), BL = WS_THREADS / FP;
+    const unsigned gx = (unsigned)((B + BL - 1) / BL);
+    // grid.y is limited to 65535 clusters; K <= 1024 by the predict ABI
+    for (int k0 = 0; k0 < K; k0 += 32768) {
+        const int kn = K - k0 < 32768 ? K - k0 : 32768;
+        LaunchScope ls(KK_GRAM, st);
+        const dim3 grid(gx, (unsigned)kn);
+        if (coh_format == SAGECAL_COH_SCALAR)
+            gram_kernel<true><<<grid, WS_THREADS, 0, st>>>(T, F, FP, B, coh + (size_t)k0 * T * B * F, Scc + (size_t)k0 * NSCC_SCALAR * B);
+        else
+            gram_kernel<false><<<grid, WS_THREADS, 0, st>>>(T, F, FP, B, coh + (size_t)k0 * T * B * F * 4, Scc + (size_t)k0 * NSCC_FULL * B);
+        SGC_LAUNCH_CHECK();
+    }
+    return SAGECAL_OK;
+}
+
+template <bool SCALAR>
+static int launch_wbstat(int N, int T, int F, sagecal_c128* R, const sagecal_c128* Cprev, const sagecal_c128* J0prev,
+                         const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src, double* srr, cudaStream_t st) {
+    const int64_t B = (int64_t)N * (N - 1) / 2;
+    const int FP = stat_group(F), BL = WS_THREADS / FP;
+    const unsigned grid = (unsigned)((B + BL - 1) / BL);
+    LaunchScope ls(KK_WBSTAT, st);
+    if (Cprev && Cnext)
+        wbstat_kernel<SCALAR, true, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+    else if (Cprev)
+        wbstat_kernel<SCALAR, true, false><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+    else
+        wbstat_kernel<SCALAR, false, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+    SGC_LAUNCH_CHECK();
+    return SAGECAL_OK;
+}
+
+int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
+                   const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
+                   double* srr, cudaStream_t st) {
+    if (!Cprev && !Cnext) return SAGECAL_OK;
+    return coh_format == SAGECAL_COH_SCALAR ? launch_wbstat<true>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, srr, st)
+                                            : launch_wbstat<false>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, srr, st);
+}
+
+}  // namespace sgc

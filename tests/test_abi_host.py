@@ -49,7 +49,7 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.sagecal_lm_cost_grad_jtj(1, 1, 1, z, 0, z, z, z, z, z, z, 0, z) == -1
     assert lib.sagecal_lm_cost_grad_jtj(4, 1, 1, z, 0, z, z, z, z, z, z, 0, z) == -1      # NULL pointers
     assert lib.sagecal_corrupt_subtract(4, 1, 1, 1, 7, z, z, z, -1.0, z, z, z) == -1      # bad coh_format
-    assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, z, z, z, 0, z) == -1
+    assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, 0, z, z, z, 0, z) == -1
     fr = (ctypes.c_double * 1)(150e6)
     off = (ctypes.c_int * 2)(0, 1)
     assert lib.sagecal_predict_coherencies(4, 1, 1, fr, 150e6, z, 1, off, z, z, z, z, z, z, z, 0, z, 0, z, 0, z) == -1
@@ -70,3 +70,29 @@ def test_pass_geometry_covers_every_baseline_once(lib, N, T, F):
     TQ, nchunk, ncols, TC, tlen, nslots, R, U = info
     assert TQ == max(1, 128 // F) and ncols == -(-N // TQ) and U == R * TC and 1 <= nslots <= U
     assert TC * tlen >= T > (TC - 1) * tlen
+
+
+@pytest.mark.parametrize("N", [2, 3, 8, 16, 17, 31, 32, 33, 34, 47, 48, 49, 64, 65, 100, 129, 256, 257, 512])
+def test_compressed_pass_tiling_covers_every_baseline_once(lib, N):
+    """cpass_kernel's (16 rows x 32 columns) tiles visit every baseline exactly once, and creduce_kernel reads exactly
+    the records that were written and carry a contribution."""
+    lib.sagecal_debug_cpass_cover.restype = ctypes.c_int
+    lib.sagecal_debug_cpass_cover.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    B = N * (N - 1) // 2
+    cover = np.zeros(B, np.int32)
+    info = np.zeros(4, np.int64)
+    rc = lib.sagecal_debug_cpass_cover(N, cover.ctypes.data, info.ctypes.data)
+    assert rc == 0, f"record bookkeeping violated: mask {rc}, info {info}"
+    assert np.all(cover == 1)
+    assert info[0] == -(-N // 32) and info[1] == -(-(N - 1) // 16) and info[3] == B
+
+
+def test_calibrate_workspace_covers_compressed_statistics(lib):
+    """SAGECAL_WS_CALIBRATE holds the per-baseline statistics of the compressed mode: K x 16 doubles (gram of the
+    coherencies) + 33 doubles per baseline, on top of the direct pass's partial sums."""
+    from paper_1910_13908_b200 import _binding as b
+    N, T, F, K = 512, 20, 8, 50
+    B = N * (N - 1) // 2
+    ws = b.workspace_bytes(b.WS_CALIBRATE, N, T, F, K)
+    assert ws >= b.workspace_bytes(b.WS_LM_PASS, N, T, F) + 8 * B * (16 * K + 33)
+    assert ws < 1.2e9

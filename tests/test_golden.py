@@ -35,7 +35,7 @@ def test_cuda_path_matches_golden_cfg0(cuda_device):
     import torch
     import paper_1910_13908_b200 as sg
     from sagecal_inputs import make_config
-    from gpu_util import dev, gpu_predict, gpu_simulate, host
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
 
     want = load_golden()
     p = make_config(0)

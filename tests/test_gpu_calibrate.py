@@ -11,9 +11,15 @@ from tests.helpers import rel_l2, rel_max
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-8
+MODES = ["compressed", "direct"]      # lm_mode of sagecal_sage_calibrate: both follow the oracle's trajectory
 
 
-def _run_both(p, n_em, n_lm, coh_format=None, polarised=False):
+def _mode(name):
+    import paper_1910_13908_b200 as sg
+    return {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT}[name]
+
+
+def _run_both(p, n_em, n_lm, coh_format=None, polarised=False, mode="compressed"):
     import paper_1910_13908_b200 as sg
     from tests.gpu_util import dev, gpu_predict, host
 
@@ -23,7 +29,8 @@ def _run_both(p, n_em, n_lm, coh_format=None, polarised=False):
     want = oracle.sage(p.N, p.T, p.F, V, coh, p.jones_init(), n_em, n_lm, p.tau)
     assert want["min_abs_rho"] > 1e-6, "seed has an accept/reject decision within rounding of 0: not a parity seed"
     coh_d = gpu_predict(p, fmt)                        # the CUDA path predicts its own coherencies
-    got = sg.sage_calibrate(p.N, p.T, p.F, dev(V), coh_d, dev(p.jones_init()), n_em, n_lm, p.tau, coh_format=fmt)
+    got = sg.sage_calibrate(p.N, p.T, p.F, dev(V), coh_d, dev(p.jones_init()), n_em, n_lm, p.tau, coh_format=fmt,
+                            lm_mode=_mode(mode))
     return want, {k: (None if v is None else host(v)) for k, v in got.items()}, V, coh
 
 
@@ -35,41 +42,82 @@ def _compare(want, got):
     assert rel_l2(got["residual"], want["residual"]) < TOL
 
 
+@pytest.mark.parametrize("mode", MODES)
 @pytest.mark.parametrize("cfg", [0, 1, 2])
-def test_calibrate_configs(cuda_device, cfg):
+def test_calibrate_configs(cuda_device, cfg, mode):
     """configs[0..2] with their own iteration budget (3 EM x 10 LM)."""
     p = make_config(cfg)
-    want, got, V, coh = _run_both(p, p.n_em, p.n_lm)
+    want, got, V, coh = _run_both(p, p.n_em, p.n_lm, mode=mode)
     _compare(want, got)
     tr = got["cost_trace"]
     assert np.all(np.diff(tr) <= 1e-12 * tr[:-1])            # P11 on the CUDA path
 
 
-def test_calibrate_scalar_format(cuda_device):
+@pytest.mark.parametrize("mode", MODES)
+def test_calibrate_scalar_format(cuda_device, mode):
     import paper_1910_13908_b200 as sg
     p = make_config(2, K=6)
-    want, got, _, _ = _run_both(p, 2, 6, coh_format=sg.COH_SCALAR)
+    want, got, _, _ = _run_both(p, 2, 6, coh_format=sg.COH_SCALAR, mode=mode)
     _compare(want, got)
 
 
-def test_calibrate_polarised_small(cuda_device):
+@pytest.mark.parametrize("mode", MODES)
+def test_calibrate_polarised_small(cuda_device, mode):
     p = make_problem(10, 4, 3, 3, 4, seed=31, sigma=0.05, layout="disc:3000", field_deg=4.0, patch_deg=0.5,
                      polarised=True)
-    want, got, _, _ = _run_both(p, 3, 5)
+    want, got, _, _ = _run_both(p, 3, 5, mode=mode)
     _compare(want, got)
 
 
-def test_calibrate_cfg3_multi_tile(cuda_device):
+@pytest.mark.parametrize("shape", [(37, 3, 3), (33, 2, 5), (70, 2, 8), (6, 2, 40)])
+def test_calibrate_compressed_ragged_shapes(cuda_device, shape):
+    """Compressed mode on shapes that leave ragged tiles everywhere: N not a multiple of the 16 x 32 station tile,
+    F not a power of two (idle lanes in a baseline's lane group) and F > 32 (a lane walks several channels);
+    polarised sources so all 16 + 16 statistics of a baseline matter."""
+    N, T, F = shape
+    p = make_problem(N, T, F, 3, 4, seed=77 + N, sigma=0.05, layout="disc:5000", field_deg=4.0, patch_deg=0.5,
+                     polarised=True)
+    want, got, _, _ = _run_both(p, 2, 4, mode="compressed")
+    _compare(want, got)
+
+
+def test_calibrate_compressed_recentres_long_msteps(cuda_device):
+    """n_lm = 25 > SAGECAL_LM_RECENTRE: the statistics are re-taken at the accepted Jones twice inside every M-step;
+    the trajectory must still be the oracle's."""
+    p = make_config(1)
+    want, got, _, _ = _run_both(p, 2, 25, mode="compressed")
+    _compare(want, got)
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_calibrate_cfg3_multi_tile(cuda_device, mode):
     """configs[3] shape (N=256, F=4: 8 column tiles, time-chunked units), K cut to 4 and 1 EM x 5 LM so the oracle
     finishes in seconds."""
     p = make_config(3, K=4)
-    want, got, _, _ = _run_both(p, 1, 5)
+    want, got, _, _ = _run_both(p, 1, 5, mode=mode)
     _compare(want, got)
 
 
-def test_calibrate_noiseless_recovery_on_gpu(cuda_device):
+def test_calibrate_modes_agree_to_rounding(cuda_device):
+    """The two lm_modes are the same sums re-associated: on the same inputs they agree far inside the parity bound."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+    p = make_config(2, K=8)
+    coh_d = gpu_predict(p)
+    V = gpu_simulate(p, coh_d)
+    out = [sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 2, 6, p.tau, lm_mode=m)
+           for m in (sg.LM_COMPRESSED, sg.LM_DIRECT)]
+    a, b = [{k: host(v) for k, v in o.items()} for o in out]
+    assert np.max(np.abs(a["cost_per_cluster"] - b["cost_per_cluster"]) / b["cost_per_cluster"]) < 1e-11
+    assert rel_l2(a["jones"], b["jones"]) < 1e-11
+    assert rel_l2(a["residual"], b["residual"]) < 1e-11
+
+
+@pytest.mark.parametrize("mode", MODES)
+def test_calibrate_noiseless_recovery_on_gpu(cuda_device, mode):
     """P10 on the CUDA path: noiseless single-cluster data, the cost falls below 1e-20 relative and the true Jones
-    are recovered up to a unitary matrix."""
+    are recovered up to a unitary matrix.  60 trial steps of one M-step; compressed mode re-centres its statistics
+    every 10 of them, which is what lets the cost fall 20 decades below the starting residual."""
     import paper_1910_13908_b200 as sg
     from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
     from tests.helpers import procrustes_err
@@ -78,12 +126,13 @@ def test_calibrate_noiseless_recovery_on_gpu(cuda_device):
     coh_d = gpu_predict(p)
     V = gpu_simulate(p, coh_d, noise=False)
     phi0 = float((V.abs() ** 2).sum())
-    got = sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 1, 60, p.tau)
+    got = sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 1, 60, p.tau, lm_mode=_mode(mode))
     assert float(got["cost_per_cluster"][0]) / phi0 < 1e-20
     assert procrustes_err(host(got["jones"])[0], p.jones_true[0]) < 1e-12
 
 
-def test_calibrate_full_size_properties(cuda_device):
+@pytest.mark.parametrize("mode", MODES)
+def test_calibrate_full_size_properties(cuda_device, mode):
     """configs[4] (N=512, T=20, F=8, K=50 x 40 sources) in the launch configuration bench.py times, scalar
     coherencies, 1 EM x 2 LM to bound the time.  The oracle cannot run this size inside a test, so: sampled outputs
     (the residual on random rows, recomputed by the oracle from the returned Jones; the gradient of one LM pass for
@@ -99,7 +148,7 @@ def test_calibrate_full_size_properties(cuda_device):
     coh_d = gpu_predict(p, sg.COH_SCALAR)
     V = gpu_simulate(p, coh_d, sg.COH_SCALAR)
     J0 = dev(p.jones_init())
-    got = sg.sage_calibrate(N, T, F, V, coh_d, J0, 1, 2, p.tau, coh_format=sg.COH_SCALAR)
+    got = sg.sage_calibrate(N, T, F, V, coh_d, J0, 1, 2, p.tau, coh_format=sg.COH_SCALAR, lm_mode=_mode(mode))
     tr = host(got["cost_trace"])
     assert np.all(np.isfinite(tr)) and np.all(np.diff(tr) <= 1e-12 * tr[:-1])
     # cost_per_cluster[K-1] is ||R||^2 after the last M-step
