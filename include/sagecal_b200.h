@@ -61,7 +61,8 @@ typedef struct { double re, im; } sagecal_c128;
  * Both follow the same LM trajectory and agree to rounding. */
 #define SAGECAL_LM_COMPRESSED 0  /* default: per-baseline time/frequency statistics of the residual, taken once per
                                     (EM iteration, cluster) in the same streaming kernel that writes back the previous
-                                    cluster; the evaluations then read 392 B per baseline instead of 128 B per sample */
+                                    cluster; the n_lm+1 evaluations and the LM control then run in one cooperative
+                                    kernel that reads 392 B per baseline instead of 128 B per sample */
 #define SAGECAL_LM_DIRECT     1  /* every evaluation streams the cluster's T*F samples (sagecal_lm_cost_grad_jtj) */
 /* compressed mode re-takes the statistics at the accepted Jones every this many trial steps of one M-step */
 #define SAGECAL_LM_RECENTRE  10
@@ -232,12 +233,13 @@ int sagecal_profile_read(double* ms_host, long long* timed_host, long long* laun
 int sagecal_debug_pass_cover(int nstations, int ntime, int nchan, int32_t* cover, int64_t* info);
 
 /*
- * Test hook, host only: replays the tiling of the compressed evaluation pass and the record lists of
- * its station reduction.  cover : host out [B] int32, zeroed by the caller; every entry must come back 1.
- * info : host out [4] int64 = {q tiles, p blocks, live tiles, B}.  Returns 0, SAGECAL_EINVAL, or a positive bit mask
- * (1/4: a row/column record is read but never written; 2/8: a record that carries a baseline is never read).
+ * Test hook, host only: replays the tiling and lane mapping of the compressed M-step kernel and the
+ * record lists of its station reduction.  cover : host out [B] int32, zeroed by the caller; every entry must come
+ * back 1.  info : host out [6] int64 = {q tiles, p blocks, tiles decoded, B, rows per tile, tiles}.  Returns 0,
+ * SAGECAL_EINVAL, or a positive bit mask (1/4: a row/column record is read but never written; 2/8: a record that
+ * carries a baseline is never read; 16/32: a tile or record index out of range).
  */
-int sagecal_debug_cpass_cover(int nstations, int32_t* cover, int64_t* info);
+int sagecal_debug_mstep_cover(int nstations, int32_t* cover, int64_t* info);
 
 #ifdef __cplusplus
 }

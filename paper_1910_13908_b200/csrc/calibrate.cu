@@ -320,35 +320,28 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     }
 
     // compressed mode: `residual` always holds R; per (em, k) one streaming kernel writes back the
-    // previous cluster and takes the statistics of the new residual against C_k, then the n_lm+1 evaluations run on
-    // the per-baseline statistics.  Statistics are re-centred every SAGECAL_LM_RECENTRE trial steps.
-    const CGeom cg = make_cgeom(N);
+    // previous cluster and takes the statistics of the new residual against C_k, then ONE cooperative kernel runs
+    // the n_lm+1 evaluations and the LM control on the per-baseline statistics.  Statistics are re-centred every
+    // SAGECAL_LM_RECENTRE trial steps.
     if ((rc = enqueue_gram(N, T, F, K, coh_format, coh, w.cw.Scc, st))) return rc;
     const sagecal_c128* Cprev = nullptr;      // cluster whose write-back is pending
     const sagecal_c128* Jprev = nullptr;
+    const int64_t B = g.B;
     int par = 0;
     int it = 1;
     for (int em = 0; em < n_em; em++) {
         for (int k = 0; k < K; k++, it++) {
             const sagecal_c128* Ck = coh + (size_t)k * cstride;
             sagecal_c128* Jk = jones + (size_t)k * N * 4;
-            const double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * cg.B;
+            const double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * B;
             double* tr = cost_trace ? cost_trace + it : nullptr;
             int done = 0;
             do {
                 sagecal_c128* J0 = w.cw.J0 + (size_t)par * N * 4;
                 const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
                 if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, w.cw.srr, st))) return rc;
-                SGC_CUDA(cudaMemcpyAsync(J0, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
-                if ((rc = enqueue_cpass(cg, w.cw, scalar, Scc_k, J0, J0, w.G, w.M, st))) return rc;
-                if (done == 0) rc = enqueue_step<LM_INIT>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st);
-                else rc = enqueue_step<LM_RECENTRE>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st);
-                if (rc) return rc;
                 const int chunk = n_lm - done < SAGECAL_LM_RECENTRE ? n_lm - done : SAGECAL_LM_RECENTRE;
-                for (int i = 0; i < chunk; i++) {
-                    if ((rc = enqueue_cpass(cg, w.cw, scalar, Scc_k, J0, w.J_try, w.G_try, w.M_try, st))) return rc;
-                    if ((rc = enqueue_step<LM_TRIAL>(N, tau, w, Jk, w.cw.cost_st, cost_per_cluster + k, tr, st))) return rc;
-                }
+                if ((rc = enqueue_mstep(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, st))) return rc;
                 done += chunk;
                 Cprev = Ck; Jprev = Jk;
                 par ^= 1;

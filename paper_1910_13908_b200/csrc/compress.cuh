@@ -1,5 +1,5 @@
 // Time/frequency-compressed M-step: shared declarations of wbstat.cu (per-baseline statistics,
-// fused with the previous cluster's write-back) and cpass.cu (cost / gradient / J^H J from those statistics).
+// fused with the previous cluster's write-back) and mstep.cu (the LM iterations of one M-step on those statistics).
 //
 // One Jones matrix per (cluster, station) holds for the whole interval (reading Q7), so for a fixed
 // baseline every (t, f) sample sees the same J_p, J_q.  With c = vec(C) (row-major [C00,C01,C10,C11]), r = vec(R)
@@ -21,11 +21,11 @@
 
 namespace sgc {
 
-// ---- statistics layout: structure of arrays over baselines, plane-major ---------------------------------------
-//   Src [NSRC][B] doubles: FULL plane 2*(4a+b) = Re, +1 = Im of Src[a][b];  SCALAR plane 2a, 2a+1 of Sr[a]
-//   srr [B]
-//   Scc [K][NSCC][B]:      FULL planes 0..3 = Scc[a][a]; planes 4+2i, 5+2i = Re, Im of the i-th upper pair in the order
-//                          (0,1) (0,2) (0,3) (1,2) (1,3) (2,3);  SCALAR plane 0 = s2
+// ---- statistics layout: one record per baseline ----------------------------------------------------------------
+//   Src  FULL   [B][4 a][4 c] complex (256 B): Src[a][c] = sum r_a conj(c_c);   SCALAR [B][4 a] complex (64 B): Sr[a]
+//   srr  [B]
+//   Scc  [K][B][NSCC] doubles: FULL 16 = Scc[0][0], [1][1], [2][2], [3][3], then Re, Im of the upper pairs in the order
+//        (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)  (128 B);  SCALAR 1 = s2
 constexpr int NSRC_FULL = 32, NSRC_SCALAR = 8;
 constexpr int NSCC_FULL = 16, NSCC_SCALAR = 1;
 __host__ __device__ constexpr int nsrc(bool scalar) { return scalar ? NSRC_SCALAR : NSRC_FULL; }
@@ -34,26 +34,41 @@ __host__ __device__ constexpr int nscc(bool scalar) { return scalar ? NSCC_SCALA
 // lanes that share one baseline in wbstat/gram: the smallest power of two >= F, at most 32
 inline int stat_group(int F) { int g = 1; while (g < F && g < 32) g <<= 1; return g; }
 
-// ---- compressed pass tiling: q tiles of 32 stations (one lane each) x p blocks of 16 rows ------------------------
-constexpr int CP_TQ = 32, CP_PB = 16, CP_THREADS = 128, CP_NP = 13, CP_NQ = 12;
-struct CGeom {
-    int N, nqt, npb;
+// ---- M-step kernel tiling (mstep.cu): tile = PB row stations p x 32 column stations q ---------------------------
+constexpr int MS_THREADS = 256, MS_WARPS = 8, MS_TQ = 32, MS_PB_MAX = 16, MS_NV = 12, MS_MAX_GRID = 2048;
+struct MGeom {
+    int N, PB, nqt, npb, ntiles;
     int64_t B;
+    // largest q of column tile qt
+    __host__ __device__ int qmax(int qt) const { int h = MS_TQ * (qt + 1); return (h < N ? h : N) - 1; }
+    // live row blocks of column tile qt: blocks pb with PB*pb < qmax(qt)
+    __host__ __device__ int nlive(int qt) const { return (qmax(qt) + PB - 1) / PB; }
 };
-inline CGeom make_cgeom(int N) {
-    CGeom g;
-    g.N = N; g.nqt = (N + CP_TQ - 1) / CP_TQ; g.npb = (N - 1 + CP_PB - 1) / CP_PB;
+inline MGeom make_mgeom(int N, int PB) {
+    MGeom g;
+    g.N = N; g.PB = PB; g.nqt = (N + MS_TQ - 1) / MS_TQ; g.npb = (N - 1 + PB - 1) / PB;
     g.B = (int64_t)N * (N - 1) / 2;
+    g.ntiles = 0;
+    for (int qt = 0; qt < g.nqt; qt++) g.ntiles += g.nlive(qt);
     return g;
 }
 
+// LM state carried between the chunks of one M-step (device memory)
+struct MstepCtl { double phi, mu, nu, pad; };
+
 struct CompressWorkspace {
-    double* Scc;      // [K][nscc][B]
-    double* Src;      // [nsrc][B]
+    double* Scc;      // [K][B][nscc]
+    double* Src;      // [B][nsrc]
     double* srr;      // [B]
-    double* Ppart;    // [nqt][N][13]  row-station partial sums (12 + cost)
-    double* Qpart;    // [npb][N][12]  column-station partial sums
-    double* cost_st;  // [N] cost summed per row station
+    double* Ppart;    // [nqt][N][12]  row-station partial sums, one record per (column tile, row)
+    double* Qpart;    // [npb(PB=2)][N][12]  column-station partial sums, one record per (row block, column)
+    double* cost_cta; // [MS_MAX_GRID] cost summed per CTA
+    double* pred_st;  // [2][N] predicted reduction per station, halves alternate by evaluation (readers of one
+                      //        evaluation must not see the next one's values)
+    double* mm_st;    // [N] max(M00, M11) per station (damping initialisation)
+    double* Htry;     // [N][4] J_try^H J_try as (h00, h11, Re h01, Im h01)
+    sagecal_c128 *G, *M, *J_try;   // [N][4] accepted gradient / J^H J, trial Jones
+    MstepCtl* ctl;
     sagecal_c128* J0; // [2][N][4] centre Jones of the current / previous statistics
 };
 size_t compress_workspace_bytes(int N, int K, bool scalar);
@@ -65,8 +80,11 @@ int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128*
 int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
                    const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
                    double* srr, cudaStream_t st);
-// (cost_st, grad, jtj) at the trial Jones Jt from the statistics centred at J0
-int enqueue_cpass(const CGeom& g, const CompressWorkspace& w, bool scalar, const double* Scc_k, const sagecal_c128* J0,
-                  const sagecal_c128* Jt, sagecal_c128* grad, sagecal_c128* jtj, cudaStream_t st);
+// One chunk of an M-step on the statistics, one cooperative launch: J0 <- Jk, evaluation at J0, then n_trial trial
+// steps with the accept/reject and damping control on the device (init: damping initialised from tau, else the
+// state in w.ctl continues).  Jk is updated in place; *cost_out (and *trace_out) receive the accepted cost.
+int enqueue_mstep(int N, bool scalar, const CompressWorkspace& w, const double* Scc_k, sagecal_c128* J0,
+                  sagecal_c128* Jk, int n_trial, bool init, double tau, double* cost_out, double* trace_out,
+                  cudaStream_t st);
 
 }  // namespace sgc

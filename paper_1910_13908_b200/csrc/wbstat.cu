@@ -125,8 +125,8 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
         for (int i = 0; i < NS; i++) {
             const double re = group_sum(S[i].re, FP), im = group_sum(S[i].im, FP);
             if (fl == 0 && b < B) {
-                Src[(size_t)(2 * i) * B + b] = re;
-                Src[(size_t)(2 * i + 1) * B + b] = im;
+                Src[(size_t)b * (2 * NS) + 2 * i] = re;
+                Src[(size_t)b * (2 * NS) + 2 * i + 1] = im;
             }
         }
         rr = group_sum(rr, FP);
@@ -178,7 +178,7 @@ gram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ co
 #pragma unroll
     for (int i = 0; i < (SCALAR ? 1 : 16); i++) {
         const double v = group_sum(acc[i], FP);
-        if (fl == 0 && b < B) out[(size_t)i * B + b] = v;
+        if (fl == 0 && b < B) out[(size_t)b * nscc(SCALAR) + i] = v;
     }
 }
 

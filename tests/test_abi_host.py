@@ -72,19 +72,22 @@ def test_pass_geometry_covers_every_baseline_once(lib, N, T, F):
     assert TC * tlen >= T > (TC - 1) * tlen
 
 
-@pytest.mark.parametrize("N", [2, 3, 8, 16, 17, 31, 32, 33, 34, 47, 48, 49, 64, 65, 100, 129, 256, 257, 512])
-def test_compressed_pass_tiling_covers_every_baseline_once(lib, N):
-    """cpass_kernel's (16 rows x 32 columns) tiles visit every baseline exactly once, and creduce_kernel reads exactly
-    the records that were written and carry a contribution."""
-    lib.sagecal_debug_cpass_cover.restype = ctypes.c_int
-    lib.sagecal_debug_cpass_cover.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+@pytest.mark.parametrize("N", [2, 3, 8, 16, 17, 31, 32, 33, 34, 47, 48, 49, 64, 65, 100, 129, 256, 257, 384, 512, 700])
+def test_mstep_tiling_covers_every_baseline_once(lib, N):
+    """mstep_kernel's tiles (PB rows x 32 columns, 4 lanes per baseline) visit every baseline exactly once, and its
+    station reduction reads exactly the records that were written and carry a contribution."""
+    lib.sagecal_debug_mstep_cover.restype = ctypes.c_int
+    lib.sagecal_debug_mstep_cover.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
     B = N * (N - 1) // 2
     cover = np.zeros(B, np.int32)
-    info = np.zeros(4, np.int64)
-    rc = lib.sagecal_debug_cpass_cover(N, cover.ctypes.data, info.ctypes.data)
+    info = np.zeros(6, np.int64)
+    rc = lib.sagecal_debug_mstep_cover(N, cover.ctypes.data, info.ctypes.data)
     assert rc == 0, f"record bookkeeping violated: mask {rc}, info {info}"
     assert np.all(cover == 1)
-    assert info[0] == -(-N // 32) and info[1] == -(-(N - 1) // 16) and info[3] == B
+    nqt, npb, seen, B_, PB, ntiles = info
+    assert nqt == -(-N // 32) and PB in (2, 4, 8, 16) and npb == -(-(N - 1) // PB) and B_ == B and seen == ntiles
+    if N == 512:
+        assert PB == 16 and ntiles == 272
 
 
 def test_calibrate_workspace_covers_compressed_statistics(lib):
