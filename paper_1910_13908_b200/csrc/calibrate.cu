@@ -339,7 +339,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
             do {
                 sagecal_c128* J0 = w.cw.J0 + (size_t)par * N * 4;
                 const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
-                if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, w.cw.srr, st))) return rc;
+                if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, st))) return rc;
                 const int chunk = n_lm - done < SAGECAL_LM_RECENTRE ? n_lm - done : SAGECAL_LM_RECENTRE;
                 if ((rc = enqueue_mstep(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, st))) return rc;
                 done += chunk;
@@ -351,7 +351,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     // last write-back: R -= dW c of the cluster solved last
     {
         const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
-        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, w.cw.srr, st))) return rc;
+        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, st))) return rc;
     }
     return SAGECAL_OK;
 }
@@ -397,12 +397,32 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     }
     SGC_CUDA(cudaMallocAsync((void**)&arena, off, st));
     int rc = SAGECAL_OK;
-    auto h2d = [&](size_t o, const void* src, size_t n) {
+    auto h2d_on = [&](cudaStream_t s, size_t o, const void* src, size_t n) {
         if (rc == SAGECAL_OK && src && n) {
-            cudaError_t e = cudaMemcpyAsync(arena + o, src, n, cudaMemcpyHostToDevice, st);
+            cudaError_t e = cudaMemcpyAsync(arena + o, src, n, cudaMemcpyHostToDevice, s);
             if (e != cudaSuccess) rc = cuda_fail(e);
         }
     };
+    auto h2d = [&](size_t o, const void* src, size_t n) { h2d_on(st, o, src, n); };
+    // the visibilities (the bulk of the input) travel on a second stream while `st` predicts the coherencies,
+    // which need only uvw and the source table; `st` joins before the calibration reads them
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev_alloc = nullptr, ev_vis = nullptr;
+    if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming) != cudaSuccess ||
+        cudaEventCreateWithFlags(&ev_vis, cudaEventDisableTiming) != cudaSuccess) {
+        rc = cuda_fail(cudaGetLastError());
+    }
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaEventRecord(ev_alloc, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_alloc, 0);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+    }
+    h2d_on(cs, o_vis, vis_host, vis_bytes);
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaEventRecord(ev_vis, cs);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+    }
     h2d(o_uvw, uvw_host, (size_t)rows * 24);
     const double* cols[7] = {src_l, src_m, src_I, src_alpha, src_Q, src_U, src_V};
     double* dcol[7];
@@ -410,13 +430,16 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
         dcol[i] = (double*)(arena + o_src + i * sS);
         h2d(o_src + i * sS, cols[i], sizeof(double) * (size_t)S);
     }
-    h2d(o_vis, vis_host, vis_bytes);
     h2d(o_jon, jones_host, (size_t)K * N * 64);
     if (rc == SAGECAL_OK)
         rc = sagecal_predict_coherencies(N, T, F, freqs_host, f0, (const double*)(arena + o_uvw), K, cluster_offset_host,
                                          dcol[0], dcol[1], dcol[2], pol ? dcol[4] : nullptr, pol ? dcol[5] : nullptr,
                                          pol ? dcol[6] : nullptr, dcol[3], coh_format, (sagecal_c128*)(arena + o_coh), 0,
                                          arena + o_wsp, ws_pred, st);
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaStreamWaitEvent(st, ev_vis, 0);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+    }
     if (rc == SAGECAL_OK)
         rc = sagecal_sage_calibrate(N, T, F, K, (const sagecal_c128*)(arena + o_vis), coh_format,
                                     (const sagecal_c128*)(arena + o_coh), (sagecal_c128*)(arena + o_jon),
@@ -432,8 +455,12 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     d2h(residual_host, o_res, vis_bytes);
     d2h(cost_per_cluster_host, o_cpc, sizeof(double) * K);
     d2h(cost_trace_host, o_trc, sizeof(double) * ntrace);
+    if (cs) (void)cudaStreamSynchronize(cs);      // on an error path the copy may still be in flight
     cudaError_t e1 = cudaFreeAsync(arena, st);
     cudaError_t e2 = cudaStreamSynchronize(st);
+    if (ev_alloc) (void)cudaEventDestroy(ev_alloc);
+    if (ev_vis) (void)cudaEventDestroy(ev_vis);
+    if (cs) (void)cudaStreamDestroy(cs);
     if (rc == SAGECAL_OK && e1 != cudaSuccess) rc = cuda_fail(e1);
     if (rc == SAGECAL_OK && e2 != cudaSuccess) rc = cuda_fail(e2);
     return rc;

@@ -22,11 +22,11 @@
 namespace sgc {
 
 // ---- statistics layout: one record per baseline ----------------------------------------------------------------
-//   Src  FULL   [B][4 a][4 c] complex (256 B): Src[a][c] = sum r_a conj(c_c);   SCALAR [B][4 a] complex (64 B): Sr[a]
-//   srr  [B]
+//   Src  FULL   [B][34]: [4 a][4 c] complex, Src[a][c] = sum r_a conj(c_c), then srr, then one pad (272 B)
+//        SCALAR [B][10]: [4 a] complex Sr[a], then srr, then one pad (80 B)
 //   Scc  [K][B][NSCC] doubles: FULL 16 = Scc[0][0], [1][1], [2][2], [3][3], then Re, Im of the upper pairs in the order
 //        (0,1) (0,2) (0,3) (1,2) (1,3) (2,3)  (128 B);  SCALAR 1 = s2
-constexpr int NSRC_FULL = 32, NSRC_SCALAR = 8;
+constexpr int NSRC_FULL = 34, NSRC_SCALAR = 10;   // doubles per record; srr sits at index NSRC-2
 constexpr int NSCC_FULL = 16, NSCC_SCALAR = 1;
 __host__ __device__ constexpr int nsrc(bool scalar) { return scalar ? NSRC_SCALAR : NSRC_FULL; }
 __host__ __device__ constexpr int nscc(bool scalar) { return scalar ? NSCC_SCALAR : NSCC_FULL; }
@@ -59,7 +59,6 @@ struct MstepCtl { double phi, mu, nu, pad; };
 struct CompressWorkspace {
     double* Scc;      // [K][B][nscc]
     double* Src;      // [B][nsrc]
-    double* srr;      // [B]
     double* Ppart;    // [nqt][N][12]  row-station partial sums, one record per (column tile, row)
     double* Qpart;    // [npb(PB=2)][N][12]  column-station partial sums, one record per (row block, column)
     double* cost_cta; // [MS_MAX_GRID] cost summed per CTA
@@ -69,6 +68,7 @@ struct CompressWorkspace {
     double* Htry;     // [N][4] J_try^H J_try as (h00, h11, Re h01, Im h01)
     sagecal_c128 *G, *M, *J_try;   // [N][4] accepted gradient / J^H J, trial Jones
     MstepCtl* ctl;
+    unsigned* bar;    // grid barrier arrive counter (zeroed before every launch)
     sagecal_c128* J0; // [2][N][4] centre Jones of the current / previous statistics
 };
 size_t compress_workspace_bytes(int N, int K, bool scalar);
@@ -76,10 +76,10 @@ CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws);
 
 // Scc of all K clusters (one pass over the coherencies)
 int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128* coh, double* Scc, cudaStream_t st);
-// R -= dW(J0prev -> Jprev) c_prev  (if Cprev), then Src, srr of the new R against Cnext (if Cnext)
+// R -= dW(J0prev -> Jprev) c_prev  (if Cprev), then the Src records (with srr) of the new R against Cnext (if Cnext)
 int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
                    const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
-                   double* srr, cudaStream_t st);
+                   cudaStream_t st);
 // One chunk of an M-step on the statistics, one cooperative launch: J0 <- Jk, evaluation at J0, then n_trial trial
 // steps with the accept/reject and damping control on the device (init: damping initialised from tau, else the
 // state in w.ctl continues).  Jk is updated in place; *cost_out (and *trace_out) receive the accepted cost.

@@ -47,7 +47,7 @@ template <bool SCALAR, bool HAS_PREV, bool HAS_NEXT>
 __global__ void __launch_bounds__(WS_THREADS, SCALAR ? 4 : 3)
 wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ Cprev,
               const sagecal_c128* __restrict__ J0prev, const sagecal_c128* __restrict__ Jprev,
-              const sagecal_c128* __restrict__ Cnext, double* __restrict__ Src, double* __restrict__ srr) {
+              const sagecal_c128* __restrict__ Cnext, double* __restrict__ Src) {
     constexpr int NW = SCALAR ? 4 : 16;                 // entries of dP / dW per baseline
     __shared__ cplx s_dw[HAS_PREV ? NW : 1][HAS_PREV ? WS_THREADS : 1];   // [entry][baseline of this CTA]
     const int tid = threadIdx.x;
@@ -125,12 +125,15 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
         for (int i = 0; i < NS; i++) {
             const double re = group_sum(S[i].re, FP), im = group_sum(S[i].im, FP);
             if (fl == 0 && b < B) {
-                Src[(size_t)b * (2 * NS) + 2 * i] = re;
-                Src[(size_t)b * (2 * NS) + 2 * i + 1] = im;
+                Src[(size_t)b * nsrc(SCALAR) + 2 * i] = re;
+                Src[(size_t)b * nsrc(SCALAR) + 2 * i + 1] = im;
             }
         }
         rr = group_sum(rr, FP);
-        if (fl == 0 && b < B) srr[b] = rr;
+        if (fl == 0 && b < B) {
+            Src[(size_t)b * nsrc(SCALAR) + 2 * NS] = rr;
+            Src[(size_t)b * nsrc(SCALAR) + 2 * NS + 1] = 0.0;
+        }
     }
 }
 
@@ -203,27 +206,27 @@ int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128*
 
 template <bool SCALAR>
 static int launch_wbstat(int N, int T, int F, sagecal_c128* R, const sagecal_c128* Cprev, const sagecal_c128* J0prev,
-                         const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src, double* srr, cudaStream_t st) {
+                         const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src, cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
     const int FP = stat_group(F), BL = WS_THREADS / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_WBSTAT, st);
     if (Cprev && Cnext)
-        wbstat_kernel<SCALAR, true, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+        wbstat_kernel<SCALAR, true, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
     else if (Cprev)
-        wbstat_kernel<SCALAR, true, false><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+        wbstat_kernel<SCALAR, true, false><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
     else
-        wbstat_kernel<SCALAR, false, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, srr);
+        wbstat_kernel<SCALAR, false, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
 }
 
 int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
                    const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
-                   double* srr, cudaStream_t st) {
+                   cudaStream_t st) {
     if (!Cprev && !Cnext) return SAGECAL_OK;
-    return coh_format == SAGECAL_COH_SCALAR ? launch_wbstat<true>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, srr, st)
-                                            : launch_wbstat<false>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, srr, st);
+    return coh_format == SAGECAL_COH_SCALAR ? launch_wbstat<true>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, st)
+                                            : launch_wbstat<false>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, st);
 }
 
 }  // namespace sgc
