@@ -418,11 +418,6 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
         if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_alloc, 0);
         if (e != cudaSuccess) rc = cuda_fail(e);
     }
-    h2d_on(cs, o_vis, vis_host, vis_bytes);
-    if (rc == SAGECAL_OK) {
-        cudaError_t e = cudaEventRecord(ev_vis, cs);
-        if (e != cudaSuccess) rc = cuda_fail(e);
-    }
     h2d(o_uvw, uvw_host, (size_t)rows * 24);
     const double* cols[7] = {src_l, src_m, src_I, src_alpha, src_Q, src_U, src_V};
     double* dcol[7];
@@ -431,6 +426,13 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
         h2d(o_src + i * sS, cols[i], sizeof(double) * (size_t)S);
     }
     h2d(o_jon, jones_host, (size_t)K * N * 64);
+    // issued after the small copies: the host-to-device copy engine serves its queue in order, and the prediction
+    // must not wait behind 1.3 GB of visibilities
+    h2d_on(cs, o_vis, vis_host, vis_bytes);
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaEventRecord(ev_vis, cs);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+    }
     if (rc == SAGECAL_OK)
         rc = sagecal_predict_coherencies(N, T, F, freqs_host, f0, (const double*)(arena + o_uvw), K, cluster_offset_host,
                                          dcol[0], dcol[1], dcol[2], pol ? dcol[4] : nullptr, pol ? dcol[5] : nullptr,
