@@ -7,6 +7,10 @@
 // of channel c+1 is the phasor of channel c times exp(-2 pi i ph df/c0): two sincospi per (row, source, channel
 // tile) instead of FT, re-anchored at every tile so the recurrence never runs longer than FT-1 steps.
 // The phase is kept in cycles, so range reduction (inside sincospi) is exact.
+// precision = 1 (MIXED): the phase in cycles and its range reduction x - rint(x) stay in
+// float64 (phases reach 3.3e3 cycles: float32 would leave 1e-4 cycles), then sincospif, the channel recurrence and
+// the flux products run in float32; products are summed in float32 over at most 32 sources and those partial sums
+// are added to the float64 accumulators.  Error ~1e-6 relative; the parity bound is 1e-5 (BASELINE.json:5).
 #include "common.cuh"
 
 namespace sgc {
@@ -51,7 +55,14 @@ __global__ void predict_prep_kernel(int S, int F, int Fpad, PredFreqs fr, double
 // POL     polarised sources (4 flux values, general 2x2 output) / unpolarised (C = c*I2)
 // UNIFORM channel recurrence / one sincospi per channel
 // SCALAR  output format SAGECAL_COH_SCALAR (only with !POL)
-template <int FT, bool POL, bool UNIFORM, bool SCALAR>
+// MIXED   float32 phasors and products (precision = 1)
+__device__ __forceinline__ void phasor_f32(double cycles, float& er, float& ei) {   // exp(-2 pi i cycles)
+    const float r = (float)(cycles - rint(cycles));          // exact reduction in float64, |r| <= 1/2
+    float sn, cs;
+    sincospif(2.0f * r, &sn, &cs);
+    er = cs; ei = -sn;
+}
+template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
 __global__ void __launch_bounds__(PRED_THREADS)
 predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClusters cl,
                const double* __restrict__ uvw, const double* __restrict__ src_l,
@@ -61,7 +72,8 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
     constexpr int NACC = POL ? 4 : 1;            // complex accumulators per channel
     constexpr int ST = POL ? 32 : 128;           // sources per shared-memory tile
     __shared__ double s_l[ST], s_m[ST], s_n[ST];
-    __shared__ __align__(16) double s_fl[ST * FT * NFL];
+    __shared__ __align__(16) double s_fl[MIXED ? 1 : ST * FT * NFL];
+    __shared__ __align__(16) float s_flf[MIXED ? ST * FT * NFL : 1];
 
     const int k = blockIdx.y;
     const int s_begin = cl.off[k], s_end = cl.off[k + 1];
@@ -85,9 +97,57 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
             }
             for (int i = threadIdx.x; i < ns * FT * NFL; i += PRED_THREADS) {
                 int s = i / (FT * NFL), rem = i - s * (FT * NFL);
-                s_fl[i] = flux_g[((size_t)(sb + s) * Fpad + c0) * NFL + rem];
+                const double f = flux_g[((size_t)(sb + s) * Fpad + c0) * NFL + rem];
+                if (MIXED) s_flf[i] = (float)f; else s_fl[i] = f;
             }
             __syncthreads();
+            if (MIXED) {
+                for (int s0 = 0; s0 < ns; s0 += 32) {
+                    float fr_[FT][NACC], fi_[FT][NACC];
+#pragma unroll
+                    for (int c = 0; c < FT; c++)
+#pragma unroll
+                        for (int j = 0; j < NACC; j++) fr_[c][j] = fi_[c][j] = 0.0f;
+                    const int s1 = min(ns, s0 + 32);
+#pragma unroll 2
+                    for (int s = s0; s < s1; s++) {
+                        const double ph = fma(w, s_n[s], fma(v, s_m[s], u * s_l[s]));  // metres
+                        const float* fl = s_flf + s * (FT * NFL);
+                        float er, ei, dr = 1.0f, di = 0.0f;
+                        if (UNIFORM) {
+                            phasor_f32(ph * fr.kf[c0], er, ei);
+                            if (FT > 1) phasor_f32(ph * dkf, dr, di);
+                        }
+#pragma unroll
+                        for (int c = 0; c < FT; c++) {
+                            if (!UNIFORM) phasor_f32(ph * fr.kf[min(c0 + c, PRED_MAXF - 1)], er, ei);
+                            if (!POL) {
+                                const float f = fl[c];
+                                fr_[c][0] = fmaf(f, er, fr_[c][0]);
+                                fi_[c][0] = fmaf(f, ei, fi_[c][0]);
+                            } else {
+                                const float fa = fl[4 * c], fd = fl[4 * c + 1], fu = fl[4 * c + 2], fv = fl[4 * c + 3];
+                                fr_[c][0] = fmaf(fa, er, fr_[c][0]);
+                                fi_[c][0] = fmaf(fa, ei, fi_[c][0]);
+                                fr_[c][3] = fmaf(fd, er, fr_[c][3]);
+                                fi_[c][3] = fmaf(fd, ei, fi_[c][3]);
+                                fr_[c][1] = fmaf(-fv, ei, fmaf(fu, er, fr_[c][1]));
+                                fi_[c][1] = fmaf(fv, er, fmaf(fu, ei, fi_[c][1]));
+                                fr_[c][2] = fmaf(fv, ei, fmaf(fu, er, fr_[c][2]));
+                                fi_[c][2] = fmaf(-fv, er, fmaf(fu, ei, fi_[c][2]));
+                            }
+                            if (UNIFORM && c + 1 < FT) {
+                                const float nr = fmaf(-ei, di, er * dr), ni = fmaf(ei, dr, er * di);
+                                er = nr; ei = ni;
+                            }
+                        }
+                    }
+#pragma unroll
+                    for (int c = 0; c < FT; c++)
+#pragma unroll
+                        for (int j = 0; j < NACC; j++) { acc[c][j].re += (double)fr_[c][j]; acc[c][j].im += (double)fi_[c][j]; }
+                }
+            } else {
 #pragma unroll 2
             for (int s = 0; s < ns; s++) {
                 const double ph = fma(w, s_n[s], fma(v, s_m[s], u * s_l[s]));  // metres
@@ -128,6 +188,7 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
                     }
                 }
             }
+            }
         }
         if (live) {
             if (SCALAR) {
@@ -154,12 +215,12 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
     }
 }
 
-template <int FT, bool POL, bool UNIFORM, bool SCALAR>
+template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
 static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
                           const PredClusters& cl, const double* uvw, const double* l, const double* m,
                           const double* nm1, const double* flux, sagecal_c128* coh) {
     LaunchScope ls(KK_PREDICT, st);
-    predict_kernel<FT, POL, UNIFORM, SCALAR><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m,
+    predict_kernel<FT, POL, UNIFORM, SCALAR, MIXED><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m,
                                                                           nm1, flux, coh);
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
@@ -201,7 +262,6 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
     if (S > 0 && (!src_l || !src_m || !src_I || !src_alpha)) return SAGECAL_EINVAL;
     for (int c = 0; c < F; c++)
         if (!(freqs_host[c] > 0.0)) return SAGECAL_EINVAL;
-    if (precision == 1) return SAGECAL_EUNSUPPORTED;
     if (!workspace || !aligned(workspace, 256) || workspace_bytes < sagecal_predict_workspace_bytes(F, S))
         return SAGECAL_EWORKSPACE;
 
@@ -238,8 +298,14 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
     }
     dim3 grid((unsigned)((rows + PRED_THREADS - 1) / PRED_THREADS), (unsigned)K);
     const bool scalar = coh_format == SAGECAL_COH_SCALAR;
-#define SGC_PRED(FT_, POL_, UNI_, SC_)                                                                              \
-    return launch_predict<FT_, POL_, UNI_, SC_>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l, src_m, nm1, flux, coh)
+    const bool mixed = precision == 1;
+#define SGC_PRED(FT_, POL_, UNI_, SC_)                                                                                  \
+    do {                                                                                                               \
+        if (mixed) return launch_predict<FT_, POL_, UNI_, SC_, true>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l,  \
+                                                                    src_m, nm1, flux, coh);                            \
+        return launch_predict<FT_, POL_, UNI_, SC_, false>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l, src_m,    \
+                                                          nm1, flux, coh);                                             \
+    } while (0)
 #define SGC_PRED_FT(FT_)                                            \
     do {                                                            \
         if (pol) { if (uniform) SGC_PRED(FT_, true, true, false); else SGC_PRED(FT_, true, false, false); } \

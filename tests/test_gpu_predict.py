@@ -120,3 +120,31 @@ def test_predict_errors(cuda_device):
     with pytest.raises(sg.SagecalError):        # offsets must start at 0 and not decrease
         sg.predict_coherencies(p.N, p.T, p.freqs, p.f0, dev(p.uvw), [3, 0, 3], d["src_l"], d["src_m"],
                                d["src_I"], d["src_alpha"])
+
+
+@pytest.mark.parametrize("case", ["cfg1", "cfg2-scalar", "polarised", "nonuniform"])
+def test_predict_mixed_precision_variant(cuda_device, case):
+    """precision=1 (float64 phase and range reduction, float32 sincos / recurrence / flux products, float64
+    accumulation of 32-source partial sums): 1e-5 relative against the float64 oracle (BASELINE.json:5), and
+    clearly not the float64 path (error above 1e-10)."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host
+    freqs = None
+    fmt = sg.COH_FULL
+    if case == "cfg1":
+        p = make_config(1)
+    elif case == "cfg2-scalar":
+        p = make_config(2, K=5)
+        fmt = sg.COH_SCALAR
+    elif case == "polarised":
+        p = make_problem(12, 3, 6, 3, 37, seed=9, layout="disc:20000", field_deg=5.0, patch_deg=0.5, polarised=True)
+    else:
+        p = make_problem(12, 3, 5, 2, 9, seed=10, layout="disc:30000", field_deg=5.0, patch_deg=0.5,
+                         freqs=np.array([120e6, 131e6, 150e6, 151e6, 178e6]))
+    want = oracle.predict(p)
+    got = host(gpu_predict(p, fmt, precision=1))
+    if fmt == sg.COH_SCALAR:
+        want = want[..., 0]
+    got = got.reshape(want.shape)
+    assert rel_l2(got, want) < 1e-5 and rel_max(got, want) < 1e-5
+    assert rel_l2(got, want) > 1e-10
