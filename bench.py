@@ -63,13 +63,13 @@ def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
 def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "direct") -> int:
     """Kernels one step launches: predict (prep + predict), initial residual, optional ||R||^2 (2), then
     direct:     per (em, k): add-back, write-back, (n_lm+1) x (pass, station reduction, LM control);
-    compressed: gram of the coherencies, per (em, k) and per chunk of LM_RECENTRE trial steps one write-back+statistics
+    compressed: per (em, k) and per chunk of LM_RECENTRE trial steps one write-back+statistics
                 kernel and one cooperative M-step kernel (all evaluations and the LM control), one final write-back."""
     head = 2 + 1 + (2 if trace else 0)
     if lm == "direct":
         return head + n_em * K * (2 + 3 * (n_lm + 1))
     chunks = max(1, -(-n_lm // LM_RECENTRE))
-    return head + 1 + n_em * K * 2 * chunks + 1
+    return head + n_em * K * 2 * chunks + 1
 
 
 def max_over_ranks(ms: float, world_size: int, device=None) -> float:

@@ -320,10 +320,10 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     }
 
     // compressed mode: `residual` always holds R; per (em, k) one streaming kernel writes back the
-    // previous cluster and takes the statistics of the new residual against C_k, then ONE cooperative kernel runs
+    // previous cluster and takes the statistics of the new residual against C_k (in the first EM iteration also the
+    // gram Scc_k of the coherencies, kept for the later ones), then ONE cooperative kernel runs
     // the n_lm+1 evaluations and the LM control on the per-baseline statistics.  Statistics are re-centred every
     // SAGECAL_LM_RECENTRE trial steps.
-    if ((rc = enqueue_gram(N, T, F, K, coh_format, coh, w.cw.Scc, st))) return rc;
     const sagecal_c128* Cprev = nullptr;      // cluster whose write-back is pending
     const sagecal_c128* Jprev = nullptr;
     const int64_t B = g.B;
@@ -333,13 +333,13 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
         for (int k = 0; k < K; k++, it++) {
             const sagecal_c128* Ck = coh + (size_t)k * cstride;
             sagecal_c128* Jk = jones + (size_t)k * N * 4;
-            const double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * B;
+            double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * B;
             double* tr = cost_trace ? cost_trace + it : nullptr;
             int done = 0;
             do {
                 sagecal_c128* J0 = w.cw.J0 + (size_t)par * N * 4;
                 const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
-                if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, st))) return rc;
+                if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, em == 0 && done == 0 ? Scc_k : nullptr, st))) return rc;
                 const int chunk = n_lm - done < SAGECAL_LM_RECENTRE ? n_lm - done : SAGECAL_LM_RECENTRE;
                 if ((rc = enqueue_mstep(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, st))) return rc;
                 done += chunk;
@@ -351,7 +351,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     // last write-back: R -= dW c of the cluster solved last
     {
         const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
-        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, st))) return rc;
+        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, nullptr, st))) return rc;
     }
     return SAGECAL_OK;
 }

@@ -74,12 +74,11 @@ struct CompressWorkspace {
 size_t compress_workspace_bytes(int N, int K, bool scalar);
 CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws);
 
-// Scc of all K clusters (one pass over the coherencies)
-int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128* coh, double* Scc, cudaStream_t st);
-// R -= dW(J0prev -> Jprev) c_prev  (if Cprev), then the Src records (with srr) of the new R against Cnext (if Cnext)
+// R -= dW(J0prev -> Jprev) c_prev  (if Cprev), then the Src records (with srr) of the new R against Cnext (if Cnext),
+// and Scc of Cnext into Scc_next if that is not NULL
 int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
                    const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
-                   cudaStream_t st);
+                   double* Scc_next, cudaStream_t st);
 // One chunk of an M-step on the statistics, one cooperative launch: J0 <- Jk, evaluation at J0, then n_trial trial
 // steps with the accept/reject and damping control on the device (init: damping initialised from tau, else the
 // state in w.ctl continues).  Jk is updated in place; *cost_out (and *trace_out) receive the accepted cost.

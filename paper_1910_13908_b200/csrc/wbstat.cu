@@ -3,7 +3,8 @@
 //
 //   wbstat:  R <- R - dW_prev c_prev   (write-back of the cluster just solved, dW_prev = W(J_prev) - W(J0_prev))
 //            Src = sum_tf r c_next^H,  srr = sum_tf |r|^2   (statistics of the new residual for the next cluster)
-//   gram:    Scc_k = sum_tf c_k c_k^H for every cluster (depends on the coherencies only: once per interval)
+//            Scc_next = sum_tf c_next c_next^H as well in the first EM iteration (it depends on the coherencies only
+//            and is kept for the rest of the interval)
 //
 // HBM-bound streaming kernels: one thread owns one (baseline, channel) and walks the time slots, so at fixed t a
 // warp reads 32 consecutive samples (2 KB, 256-bit loads); sums stay in registers over the time loop and are
@@ -43,11 +44,29 @@ __device__ __forceinline__ cplx dP_entry(const sagecal_c128* __restrict__ J0, co
     return acc;
 }
 
-template <bool SCALAR, bool HAS_PREV, bool HAS_NEXT>
-__global__ void __launch_bounds__(WS_THREADS, SCALAR ? 4 : 3)
+// Scc += c c^H in the packed Hermitian layout of compress.cuh: 4 diagonal entries, then the 6 upper pairs
+__device__ __forceinline__ void gram_add(const m22& c, double* acc) {
+#pragma unroll
+    for (int a = 0; a < 4; a++) acc[a] = cabs2(c.a[a], acc[a]);
+    int pr = 0;
+#pragma unroll
+    for (int a = 0; a < 4; a++) {
+#pragma unroll
+        for (int c2 = a + 1; c2 < 4; c2++, pr++) {
+            const cplx s = cfmac(c.a[a], c.a[c2], mk(acc[4 + 2 * pr], acc[5 + 2 * pr]));
+            acc[4 + 2 * pr] = s.re;
+            acc[5 + 2 * pr] = s.im;
+        }
+    }
+}
+
+// GRAM: also accumulate Scc of C_next (the first EM iteration; Scc depends on the coherencies only and is kept for
+// the rest of the interval)
+template <bool SCALAR, bool HAS_PREV, bool HAS_NEXT, bool GRAM>
+__global__ void __launch_bounds__(WS_THREADS, SCALAR ? 4 : (GRAM ? 2 : 3))
 wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ Cprev,
               const sagecal_c128* __restrict__ J0prev, const sagecal_c128* __restrict__ Jprev,
-              const sagecal_c128* __restrict__ Cnext, double* __restrict__ Src) {
+              const sagecal_c128* __restrict__ Cnext, double* __restrict__ Src, double* __restrict__ Scc) {
     constexpr int NW = SCALAR ? 4 : 16;                 // entries of dP / dW per baseline
     __shared__ cplx s_dw[HAS_PREV ? NW : 1][HAS_PREV ? WS_THREADS : 1];   // [entry][baseline of this CTA]
     const int tid = threadIdx.x;
@@ -75,6 +94,10 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
     double rr = 0.0;
 #pragma unroll
     for (int i = 0; i < (HAS_NEXT ? NS : 1); i++) S[i] = mk(0.0, 0.0);
+    constexpr int NG = GRAM ? (SCALAR ? NSCC_SCALAR : NSCC_FULL) : 1;
+    double gacc[NG];
+#pragma unroll
+    for (int i = 0; i < NG; i++) gacc[i] = 0.0;
 
     if (b < B) {
         for (int f = fl; f < F; f += FP) {
@@ -105,6 +128,7 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
                         const cplx cn = ldg128_stream(Cnext + idx);
 #pragma unroll
                         for (int a = 0; a < 4; a++) S[a] = cfmac(r.a[a], cn, S[a]);
+                        if (GRAM) gacc[0] = cabs2(cn, gacc[0]);
                     } else {
                         m22 cn;
                         load_m22_stream(Cnext + idx * 4, cn);
@@ -113,6 +137,7 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
 #pragma unroll
                             for (int c = 0; c < 4; c++) S[4 * a + c] = cfmac(r.a[a], cn.a[c], S[4 * a + c]);
                         }
+                        if (GRAM) gram_add(cn, gacc);
                     }
                     rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
                 }
@@ -134,99 +159,38 @@ wbstat_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sag
             Src[(size_t)b * nsrc(SCALAR) + 2 * NS] = rr;
             Src[(size_t)b * nsrc(SCALAR) + 2 * NS + 1] = 0.0;
         }
-    }
-}
-
-// Scc_k for every cluster: grid.y = cluster
-template <bool SCALAR>
-__global__ void __launch_bounds__(WS_THREADS, 4)
-gram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, double* __restrict__ Scc) {
-    const int tid = threadIdx.x;
-    const int BL = WS_THREADS / FP;
-    const int g = tid / FP, fl = tid - g * FP;
-    const int64_t b = (int64_t)blockIdx.x * BL + g;
-    const size_t samples = (size_t)T * B * F;
-    const sagecal_c128* C = coh + (size_t)blockIdx.y * samples * (SCALAR ? 1 : 4);
-    double* out = Scc + (size_t)blockIdx.y * nscc(SCALAR) * B;
-    double acc[SCALAR ? 1 : 16];
+        if (GRAM) {
 #pragma unroll
-    for (int i = 0; i < (SCALAR ? 1 : 16); i++) acc[i] = 0.0;
-    if (b < B) {
-        for (int f = fl; f < F; f += FP) {
-            size_t idx = (size_t)b * F + f;
-            const size_t step = (size_t)B * F;
-#pragma unroll 4
-            for (int t = 0; t < T; t++, idx += step) {
-                if (SCALAR) {
-                    acc[0] = cabs2(ldg128_stream(C + idx), acc[0]);
-                } else {
-                    m22 c;
-                    load_m22_stream(C + idx * 4, c);
-#pragma unroll
-                    for (int a = 0; a < 4; a++) acc[a] = cabs2(c.a[a], acc[a]);
-                    int pr = 0;
-#pragma unroll
-                    for (int a = 0; a < 4; a++) {
-#pragma unroll
-                        for (int c2 = a + 1; c2 < 4; c2++, pr++) {
-                            const cplx s = cfmac(c.a[a], c.a[c2], mk(acc[4 + 2 * pr], acc[5 + 2 * pr]));
-                            acc[4 + 2 * pr] = s.re;
-                            acc[5 + 2 * pr] = s.im;
-                        }
-                    }
-                }
+            for (int i = 0; i < NG; i++) {
+                const double v = group_sum(gacc[i], FP);
+                if (fl == 0 && b < B) Scc[(size_t)b * nscc(SCALAR) + i] = v;
             }
         }
     }
-#pragma unroll
-    for (int i = 0; i < (SCALAR ? 1 : 16); i++) {
-        const double v = group_sum(acc[i], FP);
-        if (fl == 0 && b < B) out[(size_t)b * nscc(SCALAR) + i] = v;
-    }
-}
-
-int enqueue_gram(int N, int T, int F, int K, int coh_format, const sagecal_c128* coh, double* Scc, cudaStream_t st) {
-    if (K <= 0) return SAGECAL_OK;
-    const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = stat_group(F), BL = WS_THREADS / FP;
-    const unsigned gx = (unsigned)((B + BL - 1) / BL);
-    // grid.y is limited to 65535 clusters; K <= 1024 by the predict ABI
-    for (int k0 = 0; k0 < K; k0 += 32768) {
-        const int kn = K - k0 < 32768 ? K - k0 : 32768;
-        LaunchScope ls(KK_GRAM, st);
-        const dim3 grid(gx, (unsigned)kn);
-        if (coh_format == SAGECAL_COH_SCALAR)
-            gram_kernel<true><<<grid, WS_THREADS, 0, st>>>(T, F, FP, B, coh + (size_t)k0 * T * B * F, Scc + (size_t)k0 * NSCC_SCALAR * B);
-        else
-            gram_kernel<false><<<grid, WS_THREADS, 0, st>>>(T, F, FP, B, coh + (size_t)k0 * T * B * F * 4, Scc + (size_t)k0 * NSCC_FULL * B);
-        SGC_LAUNCH_CHECK();
-    }
-    return SAGECAL_OK;
 }
 
 template <bool SCALAR>
 static int launch_wbstat(int N, int T, int F, sagecal_c128* R, const sagecal_c128* Cprev, const sagecal_c128* J0prev,
-                         const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src, cudaStream_t st) {
+                         const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src, double* Scc, cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
     const int FP = stat_group(F), BL = WS_THREADS / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_WBSTAT, st);
-    if (Cprev && Cnext)
-        wbstat_kernel<SCALAR, true, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
-    else if (Cprev)
-        wbstat_kernel<SCALAR, true, false><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
-    else
-        wbstat_kernel<SCALAR, false, true><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src);
+#define SGC_WB(P_, N_, G_) wbstat_kernel<SCALAR, P_, N_, G_><<<grid, WS_THREADS, 0, st>>>(N, T, F, FP, B, R, Cprev, J0prev, Jprev, Cnext, Src, Scc)
+    if (Cprev && Cnext) { if (Scc) SGC_WB(true, true, true); else SGC_WB(true, true, false); }
+    else if (Cprev) SGC_WB(true, false, false);
+    else { if (Scc) SGC_WB(false, true, true); else SGC_WB(false, true, false); }
+#undef SGC_WB
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
 }
 
 int enqueue_wbstat(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* Cprev,
                    const sagecal_c128* J0prev, const sagecal_c128* Jprev, const sagecal_c128* Cnext, double* Src,
-                   cudaStream_t st) {
+                   double* Scc_next, cudaStream_t st) {
     if (!Cprev && !Cnext) return SAGECAL_OK;
-    return coh_format == SAGECAL_COH_SCALAR ? launch_wbstat<true>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, st)
-                                            : launch_wbstat<false>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, st);
+    return coh_format == SAGECAL_COH_SCALAR ? launch_wbstat<true>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, Scc_next, st)
+                                            : launch_wbstat<false>(N, T, F, R, Cprev, J0prev, Jprev, Cnext, Src, Scc_next, st);
 }
 
 }  // namespace sgc

@@ -19,10 +19,10 @@ def test_pass_and_launch_counts():
     assert bench.passes_per_interval(1, 3, 10) == 33
     # prep + predict + initial residual + 2 norm kernels + per (em,k): 2 corrupts + 11 x (pass, reduce, control)
     assert bench.expected_launches(50, 3, 10, True) == 5 + 150 * (2 + 33)
-    # compressed: + gram, per (em,k) one write-back/statistics kernel + one cooperative M-step kernel, + last write-back
-    assert bench.expected_launches(50, 3, 10, True, "compressed") == 5 + 1 + 150 * 2 + 1
+    # compressed: per (em,k) one write-back/statistics kernel + one cooperative M-step kernel, + last write-back
+    assert bench.expected_launches(50, 3, 10, True, "compressed") == 5 + 150 * 2 + 1
     # n_lm = 25 re-centres twice more per M-step: 3 statistics kernels and 3 M-step kernels
-    assert bench.expected_launches(1, 2, 25, False, "compressed") == 3 + 1 + 2 * 6 + 1
+    assert bench.expected_launches(1, 2, 25, False, "compressed") == 3 + 2 * 6 + 1
     assert bench.seconds_per_interval(2000.0, 1) == 2.0
     assert bench.seconds_per_interval(2000.0, 4) == 0.5          # replicas: 4 intervals per step time
 
