@@ -433,6 +433,62 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
     return 0
 
 
+def run_grid(args):
+    """--grid: the paper's scaling experiment (runtime over stations x clusters, Figs. 1-3)
+    with this build's own timings -- configs[4]'s recipe (T=20, F=8, 40 sources per cluster, 3 EM x 10 LM) at
+    N in {64, 128, 256, 384, 512} x K in {1, 50}.  Prints one JSON object {"grid": [...]}; not the bench line."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from sagecal_inputs import make_config
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --grid: no CUDA device")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
+    lm_mode = sg.LM_COMPRESSED if args.lm == "compressed" else sg.LM_DIRECT
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    out = []
+    for N in (64, 128, 256, 384, 512):
+        for K in (1, 50):
+            p = make_config(4, N=N, K=K)
+            uvw, sl, sm_, sI, sa = t(p.uvw), t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha)
+            shape = (K, p.rows, p.F, 4) if fmt == sg.COH_FULL else (K, p.rows, p.F)
+            coh = torch.empty(shape, dtype=torch.complex128, device=dev)
+            predict = lambda: sg.predict_coherencies(N, p.T, p.freqs, p.f0, uvw, p.cluster_offset, sl, sm_, sI, sa,
+                                                     coh_format=fmt, out=coh)
+            predict()
+            vis = sg.corrupt_subtract(N, p.T, p.F, coh, t(p.jones_true), t(p.noise()), sign=+1.0, coh_format=fmt)
+            jones0 = t(p.jones_init())
+            jones = jones0.clone()
+            residual = torch.empty_like(vis)
+            ws = torch.empty(sg.workspace_bytes(2, N, p.T, p.F, K), dtype=torch.uint8, device=dev)
+
+            def step():
+                predict()
+                jones.copy_(jones0)
+                return sg.sage_calibrate(N, p.T, p.F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+                                         residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
+            for _ in range(max(args.warmup, 1)):
+                o = step()
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                o = step()
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / max(args.steps, 1)
+            tr = o["cost_trace"].cpu().numpy()
+            out.append({"N": N, "B": p.B, "K": K, "samples": p.samples, "s_per_interval": ms / 1e3,
+                        "cost_first": float(tr[0]), "cost_last": float(tr[-1]),
+                        "monotone": bool(np.all(np.diff(tr) <= 1e-12 * tr[:-1]))})
+            del coh, vis, residual, ws, o, jones, jones0
+            torch.cuda.empty_cache()
+    print(json.dumps({"grid": out, "recipe": "configs[4] layout/T/F/S, 3 EM x 10 LM, float64, coherencies " + args.coh +
+                      ", lm " + args.lm, "steps": args.steps, "warmup": max(args.warmup, 1)}), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__.split("\n\n")[0])
     ap.add_argument("--gpus", type=int, default=1)
@@ -445,7 +501,11 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
+    ap.add_argument("--grid", action="store_true",
+                    help="time the paper's stations x clusters scaling grid instead of the bench step (SURVEY.md §8(f) NEXT-4)")
     args = ap.parse_args(argv)
+    if args.grid:
+        return run_grid(args)
     if args.impl == "reference":
         return run_reference(args)
     return run_ours(args)
