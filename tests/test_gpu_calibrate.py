@@ -81,6 +81,15 @@ def test_calibrate_compressed_ragged_shapes(cuda_device, shape):
     _compare(want, got)
 
 
+def test_calibrate_compressed_more_tiles_than_ctas(cuda_device):
+    """N = 700: 500 live station tiles for at most 296 co-resident CTAs, so CTAs of the M-step kernel walk several
+    tiles (shared-memory buffers reused, per-CTA cost summed over tiles); the last column tile is ragged
+    (700 = 21*32 + 28)."""
+    p = make_problem(700, 1, 2, 2, 3, seed=123, sigma=0.05, layout="disc:20000", field_deg=4.0, patch_deg=0.5)
+    want, got, _, _ = _run_both(p, 1, 4, mode="compressed")
+    _compare(want, got)
+
+
 def test_calibrate_compressed_recentres_long_msteps(cuda_device):
     """n_lm = 25 > SAGECAL_LM_RECENTRE: the statistics are re-taken at the accepted Jones twice inside every M-step;
     the trajectory must still be the oracle's."""
