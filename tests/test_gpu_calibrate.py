@@ -228,3 +228,22 @@ def test_calibrate_host_entry(cuda_device):
     assert np.array_equal(J.numpy(), host(ref["jones"]))
     assert np.array_equal(R.numpy(), host(ref["residual"]))
     assert np.array_equal(out["cost_per_cluster"].numpy(), host(ref["cost_per_cluster"]))
+
+
+@pytest.mark.parametrize("fmt", ["full", "scalar"])
+def test_calibrate_compressed_is_bit_reproducible(cuda_device, fmt):
+    """No atomics in any sum and a fixed summation order: repeated runs on the same inputs give bit-identical Jones,
+    residual and costs (a cross-CTA race in the M-step kernel would show up here)."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+    f = sg.COH_FULL if fmt == "full" else sg.COH_SCALAR
+    p = make_config(3, K=3)
+    coh_d = gpu_predict(p, f)
+    V = gpu_simulate(p, coh_d, f)
+    runs = []
+    for _ in range(3):
+        o = sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 2, 10, p.tau, coh_format=f)
+        runs.append({k: host(v) for k, v in o.items()})
+    for r in runs[1:]:
+        for k in ("jones", "residual", "cost_per_cluster", "cost_trace"):
+            assert np.array_equal(r[k], runs[0][k]), k
