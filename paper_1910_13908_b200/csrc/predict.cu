@@ -60,7 +60,10 @@ __global__ void predict_prep_kernel(int S, int F, int Fpad, PredFreqs fr, double
 // UNIFORM channel recurrence / one sincospi per channel
 // SCALAR  output format SAGECAL_COH_SCALAR (only with !POL)
 // MIXED   float32 phasors and products (precision = 1)
-// exp(-2 pi i x), x in cycles; tab[k] = (cos, sin)(2 pi k/64)
+// exp(-2 pi i x), x in cycles; tab[8 k + c] = (cos, sin)(2 pi k/64) for c = 0..7: eight copies side by side, and
+// `tab` already points at this lane's copy (lane & 7), so the 8 lanes of a quarter-warp read 8 different 16-byte
+// columns of shared memory whatever their k: no bank conflicts (a single copy cost 1.8e9 conflict wavefronts per
+// cfg4 launch and left the FP64 pipe at 61 %).
 __device__ __forceinline__ void phasor_f64(double x, const double2* __restrict__ tab, double& er, double& ei) {
     constexpr double MAGIC = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to the nearest integer
     const double TWO_PI = 6.283185307179586476925286766559;
@@ -76,7 +79,7 @@ __device__ __forceinline__ void phasor_f64(double x, const double2* __restrict__
     const double r2 = r * r;
     const double sp = r * fma(r2, fma(r2, fma(r2, s7, s5), s3), s1);          // sin(2 pi r)
     const double cp = fma(r2, fma(r2, fma(r2, fma(r2, c8, c6), c4), c2), 1.0); // cos(2 pi r)
-    const double2 t = tab[k & 63];
+    const double2 t = tab[(k & 63) << 3];
     er = fma(-t.y, sp, t.x * cp);                                // cos(a + b)
     ei = -fma(t.x, sp, t.y * cp);                                // -sin(a + b)
 }
@@ -98,12 +101,14 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
     __shared__ double s_l[ST], s_m[ST], s_n[ST];
     __shared__ __align__(16) double s_fl[MIXED ? 1 : ST * FT * NFL];
     __shared__ __align__(16) float s_flf[MIXED ? ST * FT * NFL : 1];
-    __shared__ double2 s_tab[64];
+    __shared__ double2 s_tab_all[MIXED ? 1 : 64 * 8];
     if (!MIXED && threadIdx.x < 64) {
         double sn, cs;
         sincospi((double)threadIdx.x * 0.03125, &sn, &cs);       // 2 pi k/64 = pi k/32
-        s_tab[threadIdx.x] = make_double2(cs, sn);
+#pragma unroll
+        for (int c = 0; c < 8; c++) s_tab_all[8 * threadIdx.x + c] = make_double2(cs, sn);
     }
+    const double2* s_tab = s_tab_all + (MIXED ? 0 : (threadIdx.x & 7));
 
     const int k = blockIdx.y;
     const int s_begin = cl.off[k], s_end = cl.off[k + 1];
