@@ -69,6 +69,10 @@ def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "dire
     if lm == "direct":
         return head + n_em * K * (2 + 3 * (n_lm + 1))
     chunks = max(1, -(-n_lm // LM_RECENTRE))
+    if lm == "fullgn":
+        # per chunk: statistics kernel, evaluation (3 kernels) + control + commit, then per trial step
+        # damping/rhs, step, evaluation (3), control, commit (cuSOLVER's own kernels are not counted)
+        return head + n_em * K * (6 * chunks + 7 * n_lm) + 1
     return head + n_em * K * 2 * chunks + 1
 
 
@@ -261,9 +265,9 @@ def run_ours(args):
     # ---- inputs: replicas, every rank its own interval (seed offset by rank) ----
     p = make_config(args.config, seed=191013908 + args.config + 1000 * rank)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = sg.LM_COMPRESSED if args.lm == "compressed" else sg.LM_DIRECT
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN}[args.lm]
     # the dominant kernel of the step, the one `roofline` describes
-    top = "wbstat" if args.lm == "compressed" else "lm_pass"
+    top = "lm_pass" if args.lm == "direct" else "wbstat"
     N, T, F, K = p.N, p.T, p.F, p.K
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     uvw, sl, sm_, sI, sa = t(p.uvw), t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha)
@@ -277,7 +281,7 @@ def run_ours(args):
     jones0 = t(p.jones_init())
     jones = jones0.clone()
     residual = torch.empty_like(vis)
-    ws = torch.empty(sg.workspace_bytes(2, N, T, F, K), dtype=torch.uint8, device=dev)
+    ws = torch.empty(sg.workspace_bytes(3 if args.lm == "fullgn" else 2, N, T, F, K), dtype=torch.uint8, device=dev)
 
     def step():
         predict()
@@ -335,7 +339,7 @@ def run_ours(args):
 
     npass = prof[top]["timed"]
     pass_ms = prof[top]["ms"] / max(npass, 1)
-    if args.lm == "compressed":
+    if args.lm != "direct":
         # per step: n_em*K launches; the first has no write-back (128/80 B per sample), the last no statistics
         # (192/144 B), the others both: algorithmic bytes per launch = the mean over the step's launches
         wb, cb = WBSTAT_BYTES_PER_SAMPLE[args.coh], (64 if args.coh == "full" else 16)
@@ -445,7 +449,7 @@ def run_grid(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = sg.LM_COMPRESSED if args.lm == "compressed" else sg.LM_DIRECT
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN}[args.lm]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
     for N in (64, 128, 256, 384, 512):
@@ -461,7 +465,7 @@ def run_grid(args):
             jones0 = t(p.jones_init())
             jones = jones0.clone()
             residual = torch.empty_like(vis)
-            ws = torch.empty(sg.workspace_bytes(2, N, p.T, p.F, K), dtype=torch.uint8, device=dev)
+            ws = torch.empty(sg.workspace_bytes(3 if args.lm == "fullgn" else 2, N, p.T, p.F, K), dtype=torch.uint8, device=dev)
 
             def step():
                 predict()
@@ -496,8 +500,9 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--coh", choices=["full", "scalar"], default="full")
-    ap.add_argument("--lm", choices=["compressed", "direct"], default="compressed",
-                    help="lm_mode of sagecal_sage_calibrate (DESIGN.md §5.5); direct = every evaluation streams the samples")
+    ap.add_argument("--lm", choices=["compressed", "direct", "fullgn"], default="compressed",
+                    help="lm_mode of sagecal_sage_calibrate (DESIGN.md §5.5, §5.6); direct = every evaluation streams the "
+                         "samples; fullgn = full Gauss-Newton matrix + cuSOLVER Cholesky (a different iteration, NEXT-2)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")

@@ -64,12 +64,18 @@ typedef struct { double re, im; } sagecal_c128;
                                     cluster; the n_lm+1 evaluations and the LM control then run in one cooperative
                                     kernel that reads 392 B per baseline instead of 128 B per sample */
 #define SAGECAL_LM_DIRECT     1  /* every evaluation streams the cluster's T*F samples (sagecal_lm_cost_grad_jtj) */
+#define SAGECAL_LM_FULLGN     2  /* the other reading of "per-station-block J^H J ... small dense per-cluster solve"
+                                    (DESIGN.md §3 Q1, §5.6): the FULL 8N x 8N Gauss-Newton matrix, one off-diagonal 8x8
+                                    block per baseline, damped Cholesky with cuSOLVER, on the compressed statistics.
+                                    A different iteration (it converges in a handful of steps), not the hot path;
+                                    needs the SAGECAL_WS_CALIBRATE_FULLGN workspace (3 x (8N)^2 doubles more). */
 /* compressed mode re-takes the statistics at the accepted Jones every this many trial steps of one M-step */
 #define SAGECAL_LM_RECENTRE  10
 
 /* `what` of sagecal_workspace_bytes */
 #define SAGECAL_WS_LM_PASS   1
 #define SAGECAL_WS_CALIBRATE 2
+#define SAGECAL_WS_CALIBRATE_FULLGN 3
 
 /* Speed of light used to turn uvw in metres into wavelengths (m/s). */
 #define SAGECAL_C0 299792458.0
@@ -176,7 +182,7 @@ int sagecal_lm_cost_grad_jtj(
  * jones   : dev [K][N][4], in = start values, out = solution.
  * residual: dev out [rows][F][4]; must not alias vis.
  * tau     : initial damping factor (1e-3 in all configs).
- * lm_mode : SAGECAL_LM_COMPRESSED or SAGECAL_LM_DIRECT (above).
+ * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT or SAGECAL_LM_FULLGN (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
  * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
  * No device->host transfer or synchronisation happens inside the call.

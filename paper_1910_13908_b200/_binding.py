@@ -12,7 +12,9 @@ COH_FULL = 0
 COH_SCALAR = 1
 LM_COMPRESSED = 0
 LM_DIRECT = 1
+LM_FULLGN = 2
 WS_LM_PASS = 1
+WS_CALIBRATE_FULLGN = 3
 WS_CALIBRATE = 2
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
@@ -252,7 +254,7 @@ def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor,
         residual = torch.empty((rows, F, 4), dtype=c128, device=dev)
     cpc = torch.zeros(max(K, 1), dtype=torch.float64, device=dev)
     tr = torch.zeros(n_em * K + 1, dtype=torch.float64, device=dev) if trace else None
-    wsb = workspace_bytes(WS_CALIBRATE, N, T, F, K)
+    wsb = workspace_bytes(WS_CALIBRATE_FULLGN if lm_mode == LM_FULLGN else WS_CALIBRATE, N, T, F, K)
     ws = workspace if workspace is not None else _workspace(wsb, dev)
     if ws.numel() < wsb:
         raise ValueError("workspace too small")

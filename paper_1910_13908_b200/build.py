@@ -3,7 +3,7 @@
     python -m paper_1910_13908_b200.build [--force] [--verbose]
 
 The shared library is the product's C ABI (include/sagecal_b200.h); it links the CUDA runtime statically and has
-no other dependency.  It is git-ignored but travels to the GPU box with the repo snapshot.
+one other dependency: libcusolver (the dense Cholesky of lm_mode = SAGECAL_LM_FULLGN).  It is git-ignored but travels to the GPU box with the repo snapshot.
 """
 from __future__ import annotations
 
@@ -17,7 +17,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libsagecal_b200.so")
-SOURCES = ["predict.cu", "corrupt.cu", "lm_pass.cu", "calibrate.cu", "profile.cu", "wbstat.cu", "mstep.cu"]
+SOURCES = ["predict.cu", "corrupt.cu", "lm_pass.cu", "calibrate.cu", "profile.cu", "wbstat.cu", "mstep.cu", "fullgn.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 
@@ -61,7 +61,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
             raise RuntimeError(f"nvcc failed on {src}")
         objs.append(obj)
     tmp = LIB + f".tmp{os.getpid()}"
-    subprocess.run([nvcc, "-shared", *ARCH, "-o", tmp, *objs, "-cudart", "static"], check=True)
+    subprocess.run([nvcc, "-shared", *ARCH, "-o", tmp, *objs, "-cudart", "static", "-lcusolver"], check=True)
     os.replace(tmp, LIB)
     return LIB
 

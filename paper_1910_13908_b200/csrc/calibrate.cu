@@ -250,6 +250,8 @@ extern "C" size_t sagecal_workspace_bytes(int what, int N, int T, int F, int K) 
         case SAGECAL_WS_LM_PASS: return pass_workspace_bytes(g);
         // sized for either lm_mode and either coherency format (the general 2x2 statistics are the larger)
         case SAGECAL_WS_CALIBRATE: return pass_workspace_bytes(g) + cal_extra_bytes(N) + compress_workspace_bytes(N, K, false);
+        case SAGECAL_WS_CALIBRATE_FULLGN:
+            return pass_workspace_bytes(g) + cal_extra_bytes(N) + compress_workspace_bytes(N, K, false) + fullgn_workspace_bytes(N);
         default: return 0;
     }
 }
@@ -260,14 +262,17 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                                       void* workspace, size_t workspace_bytes, void* stream) {
     if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
-    if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT) return SAGECAL_EINVAL;
+    if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT && lm_mode != SAGECAL_LM_FULLGN) return SAGECAL_EINVAL;
     if (!vis || !residual || vis == residual || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
     if (K > 0 && (!coh || !jones || !cost_per_cluster)) return SAGECAL_EINVAL;
     if (K > 0 && (!aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32) || !aligned(jones, 16))) return SAGECAL_EINVAL;
     if (!(tau > 0.0) || !isfinite(tau)) return SAGECAL_EINVAL;
     const PassGeom g = make_pass_geom(N, T, F);
-    if (!workspace || !aligned(workspace, 256) || workspace_bytes < sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE, N, T, F, K))
+    const size_t ws_base = sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE, N, T, F, K);
+    if (!workspace || !aligned(workspace, 256) ||
+        workspace_bytes < (lm_mode == SAGECAL_LM_FULLGN ? sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE_FULLGN, N, T, F, K) : ws_base))
         return SAGECAL_EWORKSPACE;
+    void* fgn_ws = (char*)workspace + ws_base;
     const bool scalar = coh_format == SAGECAL_COH_SCALAR;
     const CalWorkspace w = carve_cal(g, K, scalar, workspace);
     cudaStream_t st = (cudaStream_t)stream;
@@ -341,7 +346,11 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                 const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
                 if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, Ck, w.cw.Src, em == 0 && done == 0 ? Scc_k : nullptr, st))) return rc;
                 const int chunk = n_lm - done < SAGECAL_LM_RECENTRE ? n_lm - done : SAGECAL_LM_RECENTRE;
-                if ((rc = enqueue_mstep(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, st))) return rc;
+                if (lm_mode == SAGECAL_LM_FULLGN)
+                    rc = enqueue_fullgn(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, fgn_ws, st);
+                else
+                    rc = enqueue_mstep(N, scalar, w.cw, Scc_k, J0, Jk, chunk, done == 0, tau, cost_per_cluster + k, tr, st);
+                if (rc) return rc;
                 done += chunk;
                 Cprev = Ck; Jprev = Jk;
                 par ^= 1;
@@ -376,7 +385,8 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     const size_t vis_bytes = (size_t)samples * 64;
     const size_t coh_bytes = (size_t)K * samples * (coh_format == SAGECAL_COH_SCALAR ? 16 : 64);
     const size_t ws_pred = sagecal_predict_workspace_bytes(F, S);
-    const size_t ws_cal = sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE, N, T, F, K);
+    const size_t ws_cal = sagecal_workspace_bytes(lm_mode == SAGECAL_LM_FULLGN ? SAGECAL_WS_CALIBRATE_FULLGN : SAGECAL_WS_CALIBRATE,
+                                                  N, T, F, K);
     const size_t ntrace = (size_t)n_em * K + 1;
     const size_t sS = round_up(sizeof(double) * (size_t)(S > 0 ? S : 1), 256);
 

@@ -86,4 +86,11 @@ int enqueue_mstep(int N, bool scalar, const CompressWorkspace& w, const double* 
                   sagecal_c128* Jk, int n_trial, bool init, double tau, double* cost_out, double* trace_out,
                   cudaStream_t st);
 
+// lm_mode = SAGECAL_LM_FULLGN (fullgn.cu): one chunk of a full Gauss-Newton M-step on the same statistics; fgn_ws is
+// device scratch of fullgn_workspace_bytes(N).
+size_t fullgn_workspace_bytes(int N);
+int enqueue_fullgn(int N, bool scalar, const CompressWorkspace& cw, const double* Scc_k, sagecal_c128* J0,
+                   sagecal_c128* Jk, int n_trial, bool init, double tau, double* cost_out, double* trace_out,
+                   void* fgn_ws, cudaStream_t st);
+
 }  // namespace sgc
