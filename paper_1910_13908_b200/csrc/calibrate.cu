@@ -61,40 +61,28 @@ __device__ __forceinline__ double block_max(double v, double* s_buf) {
     return r;
 }
 
-// LM_INIT:     (phi, G, M) were just evaluated at J.  mu = tau*max_p max(M_p00, M_p11), nu = 2; first trial step.
-// LM_TRIAL:    (phi_try, G_try, M_try) were just evaluated at J_try.  rho test, accept/reject, damping update; next
-//              trial step.  dJ_p = G_p (M_p + mu I)^-1, J_try = J + dJ, pred = sum_p Re tr(G_p^H dJ_p) + mu ||dJ_p||^2.
-// LM_RECENTRE: (phi, G, M) were re-evaluated at the accepted J from fresh statistics (compressed mode, long
-//              M-steps); mu, nu are kept, the pending trial step is recomputed.
-// cost_st != NULL (compressed mode): the cost just evaluated is sum_p cost_st[p] (fixed-order block sum) instead of
-// sc->phi / sc->phi_try.
-enum { LM_TRIAL = 0, LM_INIT = 1, LM_RECENTRE = 2 };
-template <int MODE>
+// Direct mode's LM control (compressed mode: phase B of mstep_kernel; full Gauss-Newton: fgn_control_kernel).
+// INIT:   (phi, G, M) were just evaluated at J.  mu = tau*max_p max(M_p00, M_p11), nu = 2; first trial step.
+// !INIT:  (phi_try, G_try, M_try) were just evaluated at J_try.  rho test, accept/reject, damping update; next
+//         trial step.  dJ_p = G_p (M_p + mu I)^-1, J_try = J + dJ, pred = sum_p Re tr(G_p^H dJ_p) + mu ||dJ_p||^2.
+template <bool INIT>
 __global__ void __launch_bounds__(LM_THREADS)
 lm_step_kernel(int N, double tau, LmScalars* __restrict__ sc, sagecal_c128* __restrict__ J,
                sagecal_c128* __restrict__ G, sagecal_c128* __restrict__ M, const sagecal_c128* __restrict__ G_try,
                const sagecal_c128* __restrict__ M_try, sagecal_c128* __restrict__ J_try,
-               const double* __restrict__ cost_st, double* __restrict__ cost_out, double* __restrict__ trace_out) {
+               double* __restrict__ cost_out, double* __restrict__ trace_out) {
     __shared__ double s_buf[LM_THREADS];
     const int tid = threadIdx.x;
-    double fresh = 0.0;
-    if (cost_st) {
-        double part = 0.0;
-        for (int p = tid; p < N; p += LM_THREADS) part += cost_st[p];
-        fresh = block_sum(part, s_buf);
-    }
-    double phi = MODE == LM_TRIAL ? sc->phi : (cost_st ? fresh : sc->phi), mu, nu;
+    double phi = sc->phi, mu, nu;
     bool accept = false;
-    if (MODE == LM_RECENTRE) {
-        mu = sc->mu; nu = sc->nu;
-    } else if (MODE == LM_INIT) {
+    if (INIT) {
         double mmax = 0.0;
         for (int p = tid; p < N; p += LM_THREADS) mmax = fmax(mmax, fmax(M[4 * p].re, M[4 * p + 3].re));
         mmax = block_max(mmax, s_buf);
         mu = tau * mmax;
         nu = 2.0;
     } else {
-        const double phin = cost_st ? fresh : sc->phi_try, pred = sc->pred;
+        const double phin = sc->phi_try, pred = sc->pred;
         mu = sc->mu; nu = sc->nu;
         const double rho = (phi - phin) / pred;
         accept = isfinite(phin) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
@@ -216,12 +204,12 @@ static CalWorkspace carve_cal(const PassGeom& g, int K, bool scalar, void* ws) {
     return w;
 }
 
-template <int MODE>
-static int enqueue_step(int N, double tau, const CalWorkspace& w, sagecal_c128* Jk, const double* cost_st,
-                        double* cost_out, double* trace_out, cudaStream_t st) {
+template <bool INIT>
+static int enqueue_step(int N, double tau, const CalWorkspace& w, sagecal_c128* Jk, double* cost_out, double* trace_out,
+                        cudaStream_t st) {
     LaunchScope ls(KK_LMSTEP, st);
-    lm_step_kernel<MODE><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try, cost_st,
-                                                  cost_out, trace_out);
+    lm_step_kernel<INIT><<<1, LM_THREADS, 0, st>>>(N, tau, w.sc, Jk, w.G, w.M, w.G_try, w.M_try, w.J_try, cost_out,
+                                                  trace_out);
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
 }
@@ -312,10 +300,10 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                 if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, +1.0, residual, residual, st))) return rc;
                 // M-step: n_lm trial steps of block-diagonal LM
                 if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, Jk, &w.sc->phi, w.G, w.M, st))) return rc;
-                if ((rc = enqueue_step<LM_INIT>(N, tau, w, Jk, nullptr, cost_per_cluster + k, tr, st))) return rc;
+                if ((rc = enqueue_step<true>(N, tau, w, Jk, cost_per_cluster + k, tr, st))) return rc;
                 for (int i = 0; i < n_lm; i++) {
                     if ((rc = enqueue_pass(g, w.pass, residual, coh_format, Ck, w.J_try, &w.sc->phi_try, w.G_try, w.M_try, st))) return rc;
-                    if ((rc = enqueue_step<LM_TRIAL>(N, tau, w, Jk, nullptr, cost_per_cluster + k, tr, st))) return rc;
+                    if ((rc = enqueue_step<false>(N, tau, w, Jk, cost_per_cluster + k, tr, st))) return rc;
                 }
                 // R = x_k - J_k C_k J_k^H at the new J_k
                 if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, -1.0, residual, residual, st))) return rc;
