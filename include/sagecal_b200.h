@@ -73,9 +73,10 @@ typedef struct { double re, im; } sagecal_c128;
 #define SAGECAL_LM_RECENTRE  10
 
 /* `what` of sagecal_workspace_bytes */
-#define SAGECAL_WS_LM_PASS   1
-#define SAGECAL_WS_CALIBRATE 2
-#define SAGECAL_WS_CALIBRATE_FULLGN 3
+#define SAGECAL_WS_LM_PASS   1          /* sagecal_lm_cost_grad_jtj: per-unit partial sums */
+#define SAGECAL_WS_CALIBRATE 2          /* sagecal_sage_calibrate, lm_mode COMPRESSED or DIRECT, either coherency format:
+                                           the above + K x 16 + 34 doubles per baseline of statistics (0.9 GB at N=512, K=50) */
+#define SAGECAL_WS_CALIBRATE_FULLGN 3   /* lm_mode FULLGN: the above + 3 x (8N)^2 + 58 x B doubles (0.47 GB more at N=512) */
 
 /* Speed of light used to turn uvw in metres into wavelengths (m/s). */
 #define SAGECAL_C0 299792458.0
@@ -185,7 +186,9 @@ int sagecal_lm_cost_grad_jtj(
  * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT or SAGECAL_LM_FULLGN (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
  * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
- * No device->host transfer or synchronisation happens inside the call.
+ * workspace: dev scratch >= sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE or ..._FULLGN, N, T, F, K).
+ * No device->host transfer or synchronisation happens inside the call.  (SAGECAL_LM_FULLGN additionally takes
+ * cuSOLVER's own scratch from cudaMallocAsync on `stream`: its size is only known with a device.)
  */
 int sagecal_sage_calibrate(
     int nstations, int ntime, int nchan, int nclus,
