@@ -11,9 +11,11 @@ from .synth import (  # noqa: F401
     CONFIGS,
     SEED_BASE,
     Problem,
+    RowList,
     baseline_index,
     baseline_pairs,
     make_config,
     make_problem,
+    make_rowlist,
     noise_rows,
 )

@@ -308,3 +308,43 @@ def make_config(index: int, **overrides) -> Problem:
     kw.update(overrides)
     seed = kw.pop("seed", SEED_BASE + index)
     return make_problem(seed=seed, name=f"cfg{index}", n_em=3, n_lm=10, **kw)
+
+
+# ----------------------------------------------------------------------------
+# measurement-set style row lists (second part)
+# ----------------------------------------------------------------------------
+@dataclasses.dataclass
+class RowList:
+    """The rows of one interval as a measurement set would hand them over: arbitrary order, either station
+    orientation, some (time slot, baseline) pairs absent, per-sample flags.  Index and flag arrays only -- the
+    visibilities of these rows are formed by whoever consumes them."""
+
+    ant1: np.ndarray  # [n] int32
+    ant2: np.ndarray  # [n] int32 (ant1 != ant2, either order)
+    tslot: np.ndarray  # [n] int32 in [0, T)
+    uvw: np.ndarray  # [n, 3] metres for the baseline as ordered (ant1, ant2)
+    flags: np.ndarray  # [n, F] uint8, non-zero = sample excluded
+    canonical_row: np.ndarray  # [n] int64: t*B + b(min, max) -- bookkeeping for tests
+    noise: np.ndarray  # [n, F, 4] complex128, sigma per real/imag part
+
+
+def make_rowlist(prob: Problem, *, seed: int, drop_frac: float = 0.1, swap_frac: float = 0.3,
+                 flag_frac: float = 0.05, shuffle: bool = True) -> RowList:
+    """Derive a row list from a Problem: drop `drop_frac` of the canonical rows, list the rest in random order,
+    give `swap_frac` of them as (q, p) with uvw negated, flag `flag_frac` of the samples."""
+    g = _rng(seed, 17)
+    rows = np.arange(prob.rows, dtype=np.int64)
+    keep = g.random(prob.rows) >= drop_frac
+    rows = rows[keep]
+    if shuffle:
+        rows = g.permutation(rows)
+    p, q = baseline_pairs(prob.N)
+    b = rows % prob.B
+    swap = g.random(rows.size) < swap_frac
+    a1 = np.where(swap, q[b], p[b]).astype(np.int32)
+    a2 = np.where(swap, p[b], q[b]).astype(np.int32)
+    uvw = prob.uvw[rows] * np.where(swap, -1.0, 1.0)[:, None]
+    flags = (g.random((rows.size, prob.F)) < flag_frac).astype(np.uint8)
+    noise = (g.standard_normal((rows.size, prob.F, 4)) + 1j * g.standard_normal((rows.size, prob.F, 4))) * prob.sigma
+    return RowList(ant1=a1, ant2=a2, tslot=(rows // prob.B).astype(np.int32), uvw=np.ascontiguousarray(uvw),
+                   flags=np.ascontiguousarray(flags), canonical_row=rows, noise=noise)
