@@ -217,6 +217,47 @@ int sagecal_calibrate_interval_host(
     double* cost_per_cluster_host, double* cost_trace_host, void* stream);
 
 /*
+ * Measurement-set rows <-> canonical layout, and flags (SURVEY.md §8(f) NEXT-4 "per-row station index arrays
+ * (non-canonical order, flags)").  The entry points above address a sample by arithmetic on
+ * (time slot, p, q, channel) and carry no mask.  A general row list -- any order, either station orientation, absent
+ * (time slot, baseline) pairs, per-sample flags -- is brought into that layout once per interval:
+ *
+ *   sagecal_rows_to_canonical : row r = (ant1, ant2, tslot) goes to slot tslot*B + b(min, max).  A row with
+ *       ant1 > ant2 is the Hermitian transpose of the (min, max) measurement (BASELINE.json:5 "V_qp = V_pq^H"): its
+ *       2x2 samples are conjugate-transposed and its uvw negated.  Flagged samples and slots no row maps to come
+ *       out as ZERO visibilities with flag 1 (uvw of an empty slot: 0).  Dropped rows: auto-correlations
+ *       (ant1 == ant2), indices out of range, and all but the highest-indexed of several rows on one slot.
+ *   sagecal_apply_flags       : zeroes the flagged samples of every cluster's coherencies (and of `vis` if not
+ *       NULL).  After it E = 0 - J*0*J^H = 0 at flagged samples, so they add nothing to the cost, the gradient,
+ *       J^H J or the compressed statistics in ANY entry point above, and their residual is 0 -- at no cost to
+ *       the hot loops.  Call it after sagecal_predict_coherencies (which is given the canonical uvw).
+ *   sagecal_canonical_to_rows : vis_out[r] = the canonical array's slot of row r, conjugate-transposed back if
+ *       ant1 > ant2; dropped rows (row_map < 0) are left untouched.
+ *
+ * nrows_in             : number of rows in the list (>= 0).
+ * ant1, ant2, tslot    : dev [nrows_in] int32.      uvw_in : dev [nrows_in][3] f64, metres, baseline (ant1, ant2).
+ * vis_in               : dev [nrows_in][F][4].      flag_in: dev [nrows_in][F] bytes (non-zero = excluded) or NULL.
+ * uvw, vis, flags      : dev out, canonical: [T*B][3] f64, [T*B][F][4] c128, [T*B][F] bytes (0/1).
+ * row_map              : dev out [nrows_in] int64: 2*slot + (ant1 > ant2), or -1 for a dropped row.
+ * status               : dev out [4] int32: {auto-correlations, out-of-range rows, duplicates dropped, empty slots}.
+ * workspace            : dev scratch >= sagecal_rows_workspace_bytes(N, T) (one int64 per slot).
+ * Integer atomics (slot ownership, counters) are used; the outcome does not depend on their order.
+ */
+size_t sagecal_rows_workspace_bytes(int nstations, int ntime);
+int sagecal_rows_to_canonical(
+    int nstations, int ntime, int nchan, int64_t nrows_in,
+    const int32_t* ant1, const int32_t* ant2, const int32_t* tslot,
+    const double* uvw_in, const sagecal_c128* vis_in, const uint8_t* flag_in,
+    double* uvw, sagecal_c128* vis, uint8_t* flags, int64_t* row_map, int32_t* status,
+    void* workspace, size_t workspace_bytes, void* stream);
+int sagecal_canonical_to_rows(
+    int nstations, int ntime, int nchan, int64_t nrows_in, const int64_t* row_map,
+    const sagecal_c128* vis_canonical, sagecal_c128* vis_out, void* stream);
+int sagecal_apply_flags(
+    int nstations, int ntime, int nchan, int nclus, const uint8_t* flags,
+    int coh_format, sagecal_c128* coh, sagecal_c128* vis, void* stream);
+
+/*
  * Measurement plumbing (no effect on results).  Every kernel the library launches is counted by kind;
  * kinds are 0..sagecal_kernel_kinds()-1, named by sagecal_kernel_kind_name() ("predict", "corrupt", "lm_pass", ...).
  * sagecal_launch_count : kernels launched by this process since the library was loaded (all kinds).

@@ -65,6 +65,15 @@ def load_library():
     L.sagecal_calibrate_interval_host.restype = i
     L.sagecal_calibrate_interval_host.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp,
                                                   i, i, d, i, vp, vp, vp]
+    i64 = ctypes.c_int64
+    L.sagecal_rows_workspace_bytes.restype = sz
+    L.sagecal_rows_workspace_bytes.argtypes = [i, i]
+    L.sagecal_rows_to_canonical.restype = i
+    L.sagecal_rows_to_canonical.argtypes = [i, i, i, i64, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, vp, sz, vp]
+    L.sagecal_canonical_to_rows.restype = i
+    L.sagecal_canonical_to_rows.argtypes = [i, i, i, i64, vp, vp, vp, vp]
+    L.sagecal_apply_flags.restype = i
+    L.sagecal_apply_flags.argtypes = [i, i, i, i, vp, i, vp, vp, vp]
     L.sagecal_launch_count.restype = ctypes.c_longlong
     L.sagecal_kernel_kinds.restype = i
     L.sagecal_kernel_kind_name.restype = ctypes.c_char_p
@@ -265,6 +274,67 @@ def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor,
                                   ws.data_ptr(), ws.numel(), _stream(stream))
     _check(rc, "sagecal_sage_calibrate")
     return dict(jones=jones, residual=residual, cost_per_cluster=cpc[:K], cost_trace=tr)
+
+
+def rows_to_canonical(N: int, T: int, F: int, ant1: torch.Tensor, ant2: torch.Tensor, tslot: torch.Tensor,
+                      uvw_in: torch.Tensor, vis_in: torch.Tensor, flag_in: Optional[torch.Tensor] = None, stream=None):
+    """sagecal_rows_to_canonical.  Returns dict(uvw [T*B,3], vis [T*B,F,4], flags [T*B,F] uint8,
+    row_map [n] int64, status [4] int32), all device tensors."""
+    L = load_library()
+    n, rows = int(ant1.numel()), _rows(N, T)
+    dev = vis_in.device
+    i32, f64, c128, u8 = torch.int32, torch.float64, torch.complex128, torch.uint8
+    if ant2.numel() != n or tslot.numel() != n or uvw_in.numel() != 3 * n or vis_in.numel() != n * F * 4:
+        raise ValueError("row list: ant1/ant2/tslot [n], uvw_in [n,3], vis_in [n,F,4] expected")
+    if flag_in is not None and flag_in.numel() != n * F:
+        raise ValueError("flag_in: expected [n, F]")
+    uvw = torch.empty((rows, 3), dtype=f64, device=dev)
+    vis = torch.empty((rows, F, 4), dtype=c128, device=dev)
+    flags = torch.empty((rows, F), dtype=u8, device=dev)
+    row_map = torch.empty(max(n, 1), dtype=torch.int64, device=dev)
+    status = torch.empty(4, dtype=i32, device=dev)
+    wsb = int(L.sagecal_rows_workspace_bytes(N, T))
+    ws = _workspace(wsb, dev)
+    rc = L.sagecal_rows_to_canonical(N, T, F, n, _dev(ant1, i32, "ant1"), _dev(ant2, i32, "ant2"),
+                                     _dev(tslot, i32, "tslot"), _dev(uvw_in, f64, "uvw_in"),
+                                     _dev(vis_in, c128, "vis_in"), _dev(flag_in, u8, "flag_in"), uvw.data_ptr(),
+                                     vis.data_ptr(), flags.data_ptr(), row_map.data_ptr(), status.data_ptr(),
+                                     ws.data_ptr(), wsb, _stream(stream))
+    _check(rc, "sagecal_rows_to_canonical")
+    return dict(uvw=uvw, vis=vis, flags=flags, row_map=row_map[:n], status=status)
+
+
+def canonical_to_rows(N: int, T: int, F: int, row_map: torch.Tensor, vis_canonical: torch.Tensor,
+                      out: torch.Tensor, stream=None) -> torch.Tensor:
+    """sagecal_canonical_to_rows: out[r] = the canonical slot of row r (Hermitian-transposed back for swapped rows);
+    rows with row_map < 0 are left untouched."""
+    L = load_library()
+    n = int(row_map.numel())
+    if vis_canonical.numel() != _rows(N, T) * F * 4 or out.numel() != n * F * 4:
+        raise ValueError("vis_canonical [T*B,F,4] / out [n,F,4] expected")
+    rc = L.sagecal_canonical_to_rows(N, T, F, n, _dev(row_map, torch.int64, "row_map"),
+                                     _dev(vis_canonical, torch.complex128, "vis_canonical"),
+                                     _dev(out, torch.complex128, "out"), _stream(stream))
+    _check(rc, "sagecal_canonical_to_rows")
+    return out
+
+
+def apply_flags(N: int, T: int, F: int, flags: torch.Tensor, coh: Optional[torch.Tensor], vis: Optional[torch.Tensor],
+                coh_format: int = COH_FULL, stream=None) -> None:
+    """sagecal_apply_flags: zero the flagged samples of coh [K, ...] (all clusters) and of vis, in place."""
+    L = load_library()
+    rows = _rows(N, T)
+    K = 0 if coh is None else int(coh.shape[0])
+    if flags.numel() != rows * F:
+        raise ValueError("flags: expected [T*B, F]")
+    if K:
+        _coh_check(coh, coh_format, K, rows, F)
+    if vis is not None and vis.numel() != rows * F * 4:
+        raise ValueError("vis: expected rows*F*4 elements")
+    rc = L.sagecal_apply_flags(N, T, F, K, _dev(flags, torch.uint8, "flags"), coh_format,
+                               _dev(coh, torch.complex128, "coh") if K else None,
+                               _dev(vis, torch.complex128, "vis"), _stream(stream))
+    _check(rc, "sagecal_apply_flags")
 
 
 def _host(a, dtype, name):
