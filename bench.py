@@ -44,6 +44,25 @@ PASS_BYTES_PER_SAMPLE = {"full": 128, "scalar": 80}   # x (64 B) + C (64 B or 16
 # read R (64 B) + C_prev + C_next (64 B or 16 B each), write R (64 B)
 WBSTAT_BYTES_PER_SAMPLE = {"full": 256, "scalar": 160}
 LM_RECENTRE = 10                                       # SAGECAL_LM_RECENTRE of include/sagecal_b200.h
+GRP = 4                                                # clusters per group of the streaming kernel (compress.cuh)
+
+
+def group_sizes(K: int):
+    return [min(GRP, K - k0) for k0 in range(0, K, GRP)]
+
+
+def wbgroup_bytes_per_sample(K: int, n_em: int, coh: str):
+    """Algorithmic bytes per sample of every wbgroup launch of one interval (DESIGN.md §5.5 "cluster groups"):
+    R read (64 B), R written (64 B) if a previous group is pending, one coherency sample (64 B / 16 B) per cluster of
+    the previous and of the next group.  n_em * groups + 1 launches: the first writes nothing back, the last takes
+    no statistics."""
+    cb = 64 if coh == "full" else 16
+    seq = group_sizes(K) * n_em
+    out, gp = [], 0
+    for gn in seq + [0]:
+        out.append(64 + (64 if gp else 0) + cb * (gp + gn))
+        gp = gn
+    return out
 
 
 # ---------------------------------------------------------------------------------------------------------------
@@ -60,7 +79,13 @@ def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
     return n_em * K * (n_lm + 1)
 
 
-def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "direct") -> int:
+def uses_groups(lm: str, coh: str, n_lm: int) -> bool:
+    """Which streaming kernel sagecal_sage_calibrate runs (calibrate.cu): cluster groups when forced (lm grouped) or,
+    in compressed mode, for scalar coherencies -- where that is the faster order."""
+    return n_lm <= LM_RECENTRE and (lm == "grouped" or (lm == "compressed" and coh == "scalar"))
+
+
+def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "direct", coh: str = "full") -> int:
     """Kernels one step launches: predict (prep + predict), initial residual, optional ||R||^2 (2), then
     direct:     per (em, k): add-back, write-back, (n_lm+1) x (pass, station reduction, LM control);
     compressed: per (em, k) and per chunk of LM_RECENTRE trial steps one write-back+statistics
@@ -69,6 +94,12 @@ def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "dire
     if lm == "direct":
         return head + n_em * K * (2 + 3 * (n_lm + 1))
     chunks = max(1, -(-n_lm // LM_RECENTRE))
+    if uses_groups(lm, coh, n_lm):
+        # cluster groups: per group one cross-gram kernel (first EM iteration only) and one write-back+statistics
+        # kernel per EM iteration, per cluster one M-step kernel, per cluster but the last of its group one
+        # correction kernel; one final write-back
+        gs = group_sizes(K)
+        return head + len(gs) + n_em * (len(gs) + K + sum(g - 1 for g in gs)) + 1
     if lm == "fullgn":
         # per chunk: statistics kernel, evaluation (3 kernels) + control + commit, then per trial step
         # damping/rhs, step, evaluation (3), control, commit (cuSOLVER's own kernels are not counted)
@@ -265,7 +296,7 @@ def run_ours(args):
     # ---- inputs: replicas, every rank its own interval (seed offset by rank) ----
     p = make_config(args.config, seed=191013908 + args.config + 1000 * rank)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN}[args.lm]
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "grouped": sg.LM_GROUPED}[args.lm]
     # the dominant kernel of the step, the one `roofline` describes
     top = "lm_pass" if args.lm == "direct" else "wbstat"
     N, T, F, K = p.N, p.T, p.F, p.K
@@ -339,7 +370,10 @@ def run_ours(args):
 
     npass = prof[top]["timed"]
     pass_ms = prof[top]["ms"] / max(npass, 1)
-    if args.lm != "direct":
+    if uses_groups(args.lm, args.coh, p.n_lm):
+        per = wbgroup_bytes_per_sample(K, p.n_em, args.coh)
+        pass_bytes = sum(per) * p.samples // len(per)
+    elif args.lm != "direct":
         # per step: n_em*K launches; the first has no write-back (128/80 B per sample), the last no statistics
         # (192/144 B), the others both: algorithmic bytes per launch = the mean over the step's launches
         wb, cb = WBSTAT_BYTES_PER_SAMPLE[args.coh], (64 if args.coh == "full" else 16)
@@ -349,8 +383,9 @@ def run_ours(args):
         pass_bytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
     peak, peak_src = load_peaks()
     achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
-    roofline = {"bound": "hbm", "kernel": top + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": load_traffic(args.coh, top), "peak_source": peak_src,
+    kname = "wbgroup" if uses_groups(args.lm, args.coh, p.n_lm) else top     # both are timed as kind "wbstat"
+    roofline = {"bound": "hbm", "kernel": kname + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": load_traffic(args.coh, kname), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,
                 "share_of_step": prof[top]["ms"] / max(args.steps, 1) / ms_per_step}
 
@@ -423,7 +458,7 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
                    "l2": "inputs larger than L2 (per-pass working set %.2f GB vs 126 MB)" % (pass_bytes / 1e9),
                    "seed": p.seed},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(gpu_launches),
-        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True, args.lm),
+        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True, args.lm, args.coh),
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "breakdown_ms_one_step": breakdown,
         "predict_gvis_src_per_s": p.vis_src / (predict_ms * 1e-3) / 1e9 if predict_ms > 0 else None,
@@ -449,7 +484,7 @@ def run_grid(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN}[args.lm]
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "grouped": sg.LM_GROUPED}[args.lm]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
     for N in (64, 128, 256, 384, 512):
@@ -493,6 +528,58 @@ def run_grid(args):
     return 0
 
 
+def run_rows(args):
+    """--rows: the measurement-set front end at the bench workload's size (second part):
+    a seeded row list (5 % of the rows absent, 30 % given as (q, p), 5 % of the samples flagged, random order) is
+    brought into canonical order, the flags are applied to all K clusters' coherencies, and the residual is handed
+    back in row order.  Prints one JSON object {"rows": {...}}; not the bench line."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from sagecal_inputs import make_config, make_rowlist
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --rows: no CUDA device")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
+    p = make_config(args.config)
+    rl = make_rowlist(p, seed=p.seed + 1000, drop_frac=0.05, swap_frac=0.3, flag_frac=0.05)
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
+    a1, a2, ts, uvw_in, fl_in, vis_in = t(rl.ant1), t(rl.ant2), t(rl.tslot), t(rl.uvw), t(rl.flags), t(rl.noise)
+    n = int(a1.numel())
+    shape = (p.K, p.rows, p.F, 4) if fmt == sg.COH_FULL else (p.K, p.rows, p.F)
+    coh = torch.ones(shape, dtype=torch.complex128, device=dev)
+    back = torch.empty((n, p.F, 4), dtype=torch.complex128, device=dev)
+    can = sg.rows_to_canonical(p.N, p.T, p.F, a1, a2, ts, uvw_in, vis_in, fl_in)
+    legs = {
+        "rows_to_canonical": lambda: sg.rows_to_canonical(p.N, p.T, p.F, a1, a2, ts, uvw_in, vis_in, fl_in),
+        "apply_flags": lambda: sg.apply_flags(p.N, p.T, p.F, can["flags"], coh, None, coh_format=fmt),
+        "canonical_to_rows": lambda: sg.canonical_to_rows(p.N, p.T, p.F, can["row_map"], can["vis"], back),
+    }
+    nflag = int(can["flags"].count_nonzero().item())
+    cbytes = 64 if fmt == sg.COH_FULL else 16
+    # algorithmic bytes: gather = rows read once + canonical arrays written once (+ index arrays, flags);
+    # flags = 1 B read per sample + the flagged samples' coherencies written; scatter = 64 B read + written per row sample
+    alg = {"rows_to_canonical": n * p.F * 65 + p.samples * 65 + n * 44 + p.rows * 32,
+           "apply_flags": p.samples + nflag * p.K * cbytes,
+           "canonical_to_rows": n * p.F * 128 + n * 8}
+    out = {}
+    for name, fn in legs.items():
+        for _ in range(max(args.warmup, 1)):
+            fn()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            fn()
+        e1.record()
+        torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / max(args.steps, 1)
+        out[name] = {"ms": ms, "algorithmic_bytes": alg[name], "GBps": alg[name] / ms / 1e6}
+    print(json.dumps({"rows": out, "workload": workload_name(p, args.coh), "rows_in": n, "slots": p.rows,
+                      "flagged_samples": nflag, "status": can["status"].cpu().tolist(), "steps": args.steps}), flush=True)
+    return 0
+
+
 def main(argv=None):
     ap = argparse.ArgumentParser(description=__doc__.split("\n\n")[0])
     ap.add_argument("--gpus", type=int, default=1)
@@ -500,7 +587,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--coh", choices=["full", "scalar"], default="full")
-    ap.add_argument("--lm", choices=["compressed", "direct", "fullgn"], default="compressed",
+    ap.add_argument("--lm", choices=["compressed", "direct", "fullgn", "grouped"], default="compressed",
                     help="lm_mode of sagecal_sage_calibrate (DESIGN.md §5.5, §5.6); direct = every evaluation streams the "
                          "samples; fullgn = full Gauss-Newton matrix + cuSOLVER Cholesky (a different iteration, NEXT-2)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
@@ -508,7 +595,11 @@ def main(argv=None):
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
     ap.add_argument("--grid", action="store_true",
                     help="time the paper's stations x clusters scaling grid instead of the bench step (SURVEY.md §8(f) NEXT-4)")
+    ap.add_argument("--rows", action="store_true",
+                    help="time the measurement-set front end (rows -> canonical, flags, canonical -> rows) at --config's size")
     args = ap.parse_args(argv)
+    if args.rows:
+        return run_rows(args)
     if args.grid:
         return run_grid(args)
     if args.impl == "reference":

@@ -69,13 +69,20 @@ typedef struct { double re, im; } sagecal_c128;
                                     block per baseline, damped Cholesky with cuSOLVER, on the compressed statistics.
                                     A different iteration (it converges in a handful of steps), not the hot path;
                                     needs the SAGECAL_WS_CALIBRATE_FULLGN workspace (3 x (8N)^2 doubles more). */
+#define SAGECAL_LM_GROUPED    3  /* SAGECAL_LM_COMPRESSED with the streaming kernel working on groups of 4 consecutive
+                                    clusters (one read and one write of R per group; statistics corrected inside a
+                                    group through cross grams of the coherencies; DESIGN.md §5.5 "cluster groups").
+                                    Same trajectory to rounding.  SAGECAL_LM_COMPRESSED already takes this route where
+                                    it is the faster one (scalar coherencies, n_lm <= SAGECAL_LM_RECENTRE); the value
+                                    forces it for either format.  n_lm > SAGECAL_LM_RECENTRE: SAGECAL_EUNSUPPORTED. */
 /* compressed mode re-takes the statistics at the accepted Jones every this many trial steps of one M-step */
 #define SAGECAL_LM_RECENTRE  10
 
 /* `what` of sagecal_workspace_bytes */
 #define SAGECAL_WS_LM_PASS   1          /* sagecal_lm_cost_grad_jtj: per-unit partial sums */
 #define SAGECAL_WS_CALIBRATE 2          /* sagecal_sage_calibrate, lm_mode COMPRESSED or DIRECT, either coherency format:
-                                           the above + K x 16 + 34 doubles per baseline of statistics (0.9 GB at N=512, K=50) */
+                                           the above + per baseline K x 16 + 5 x 34 doubles of statistics and 6 x 32 doubles of
+                                           cross grams per group of 4 clusters (3.7 GB at N=512, K=50) */
 #define SAGECAL_WS_CALIBRATE_FULLGN 3   /* lm_mode FULLGN: the above + 3 x (8N)^2 + 58 x B doubles (0.47 GB more at N=512) */
 
 /* Speed of light used to turn uvw in metres into wavelengths (m/s). */
@@ -183,7 +190,7 @@ int sagecal_lm_cost_grad_jtj(
  * jones   : dev [K][N][4], in = start values, out = solution.
  * residual: dev out [rows][F][4]; must not alias vis.
  * tau     : initial damping factor (1e-3 in all configs).
- * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT or SAGECAL_LM_FULLGN (above).
+ * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT, SAGECAL_LM_FULLGN or SAGECAL_LM_GROUPED (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
  * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
  * workspace: dev scratch >= sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE or ..._FULLGN, N, T, F, K).

@@ -34,6 +34,34 @@ __host__ __device__ constexpr int nscc(bool scalar) { return scalar ? NSCC_SCALA
 // lanes that share one baseline in wbstat/gram: the smallest power of two >= F, at most 32
 inline int stat_group(int F) { int g = 1; while (g < F && g < 32) g <<= 1; return g; }
 
+#ifdef __CUDACC__
+// ---- entries of dW / dP from the centre and the current Jones (wbstat.cu, wbgroup.cu) -----------------------------
+// dW[a][c] (a = 2i+j, c = 2k+l) = D_p[i,k] conj(J0_q[j,l]) + J_p[i,k] conj(D_q[j,l])
+__device__ __forceinline__ cplx dW_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
+                                         int q, int a, int c) {
+    const int i = a >> 1, j = a & 1, k = c >> 1, l = c & 1;
+    const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
+    const sagecal_c128 jq0 = J0[4 * q + 2 * j + l], jq = J[4 * q + 2 * j + l];
+    const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
+    return cfmac(mk(jp.re, jp.im), Dq, cmulc(Dp, mk(jq0.re, jq0.im)));
+}
+// dP[a] (a = 2i+j) = (D_p J0_q^H + J_p D_q^H)[i,j]
+__device__ __forceinline__ cplx dP_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
+                                         int q, int a) {
+    const int i = a >> 1, j = a & 1;
+    cplx acc = mk(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < 2; k++) {
+        const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
+        const sagecal_c128 jq0 = J0[4 * q + 2 * j + k], jq = J[4 * q + 2 * j + k];
+        const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
+        acc = cfmac(mk(jp.re, jp.im), Dq, cfmac(Dp, mk(jq0.re, jq0.im), acc));
+    }
+    return acc;
+}
+
+#endif
+
 // ---- M-step kernel tiling (mstep.cu): tile = PB row stations p x 32 column stations q ---------------------------
 constexpr int MS_THREADS = 256, MS_WARPS = 8, MS_TQ = 32, MS_PB_MAX = 16, MS_NV = 12, MS_MAX_GRID = 2048;
 struct MGeom {
@@ -70,7 +98,32 @@ struct CompressWorkspace {
     MstepCtl* ctl;
     unsigned* bar;    // grid barrier arrive counter (zeroed before every launch)
     sagecal_c128* J0; // [2][N][4] centre Jones of the current / previous statistics
+    // cluster-group path (wbgroup.cu)
+    double* SrcG;     // [GRP][B][nsrc] statistics of the GRP clusters of the current group
+    double* Xg;       // [ngroups*GRP_PAIRS][B][nx] cross grams X_ij = sum_tf c_i c_j^H of the cluster pairs inside a group
+    sagecal_c128* J0G;// [2][GRP][N][4] centre Jones of the clusters of the current / previous group
 };
+// ---- cluster groups (wbgroup.cu; DESIGN.md §5.5 "cluster groups") ---------------------------------------------------
+// The statistics are linear in R, so the write-back of GRP consecutive clusters can be deferred and done in ONE pass
+// over R together with the statistics of the next GRP clusters: Src_j taken of the stale residual is corrected per
+// baseline by Src_j -= dW_i X_ij once cluster i < j of the same group has been solved.
+constexpr int GRP = 4, GRP_PAIRS = GRP * (GRP - 1) / 2;
+constexpr int NX_FULL = 32, NX_SCALAR = 2;
+__host__ __device__ constexpr int nxg(bool scalar) { return scalar ? NX_SCALAR : NX_FULL; }
+__host__ __device__ constexpr int grp_pair(int i, int j) { return i * GRP - i * (i + 1) / 2 + (j - i - 1); }   // i < j
+inline int ngroups(int K) { return (K + GRP - 1) / GRP; }
+
+// R -= sum_{i<gp} dW_i c_{kp0+i}, then Src of the new R against c_{kn0+j}, j < gn, into SrcG[j] (srr into SrcG[0] only)
+int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
+                    int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
+                    double* SrcG, cudaStream_t st);
+// Scc of clusters kn0..kn0+gn-1 (into Scc + k*nscc*B) and the cross grams of their pairs (into Xgroup)
+int enqueue_xgram(int N, int T, int F, int coh_format, const sagecal_c128* coh, size_t cstride, int kn0, int gn,
+                  double* Scc, double* Xgroup, cudaStream_t st);
+// cluster i of the group has been solved (J0_i -> J_i): Src_j -= dW_i X_ij for i < j < gn, srr_{i+1} = cost per
+// baseline after cluster i's update
+int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i, const sagecal_c128* J_i,
+                     const double* Scc_i, const double* Xgroup, double* SrcG, cudaStream_t st);
 size_t compress_workspace_bytes(int N, int K, bool scalar);
 CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws);
 

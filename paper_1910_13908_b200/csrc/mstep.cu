@@ -630,6 +630,9 @@ size_t compress_workspace_bytes(int N, int K, bool scalar) {
     n += 3 * round_up((size_t)N * 64, 256);
     n += 256 + 256;
     n += round_up((size_t)2 * N * 64, 256);
+    n += round_up(sizeof(double) * (size_t)GRP * nsrc(scalar) * g.B, 256);
+    n += round_up(sizeof(double) * (size_t)ngroups(K > 0 ? K : 1) * GRP_PAIRS * nxg(scalar) * g.B, 256);
+    n += round_up((size_t)2 * GRP * N * 64, 256);
     return n;
 }
 
@@ -652,6 +655,9 @@ CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws) {
     w.ctl = (MstepCtl*)take(256);
     w.bar = (unsigned*)take(256);
     w.J0 = (sagecal_c128*)take((size_t)2 * N * 64);
+    w.SrcG = (double*)take(sizeof(double) * (size_t)GRP * nsrc(scalar) * g.B);
+    w.Xg = (double*)take(sizeof(double) * (size_t)ngroups(K > 0 ? K : 1) * GRP_PAIRS * nxg(scalar) * g.B);
+    w.J0G = (sagecal_c128*)take((size_t)2 * GRP * N * 64);
     return w;
 }
 

@@ -20,30 +20,6 @@ __device__ __forceinline__ double group_sum(double v, int FP) {  // butterfly ov
     return v;
 }
 
-// dW[a][c] (a = 2i+j, c = 2k+l) = D_p[i,k] conj(J0_q[j,l]) + J_p[i,k] conj(D_q[j,l])
-__device__ __forceinline__ cplx dW_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
-                                         int q, int a, int c) {
-    const int i = a >> 1, j = a & 1, k = c >> 1, l = c & 1;
-    const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
-    const sagecal_c128 jq0 = J0[4 * q + 2 * j + l], jq = J[4 * q + 2 * j + l];
-    const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
-    return cfmac(mk(jp.re, jp.im), Dq, cmulc(Dp, mk(jq0.re, jq0.im)));
-}
-// dP[a] (a = 2i+j) = (D_p J0_q^H + J_p D_q^H)[i,j]
-__device__ __forceinline__ cplx dP_entry(const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J, int p,
-                                         int q, int a) {
-    const int i = a >> 1, j = a & 1;
-    cplx acc = mk(0.0, 0.0);
-#pragma unroll
-    for (int k = 0; k < 2; k++) {
-        const sagecal_c128 jp0 = J0[4 * p + 2 * i + k], jp = J[4 * p + 2 * i + k];
-        const sagecal_c128 jq0 = J0[4 * q + 2 * j + k], jq = J[4 * q + 2 * j + k];
-        const cplx Dp = mk(jp.re - jp0.re, jp.im - jp0.im), Dq = mk(jq.re - jq0.re, jq.im - jq0.im);
-        acc = cfmac(mk(jp.re, jp.im), Dq, cfmac(Dp, mk(jq0.re, jq0.im), acc));
-    }
-    return acc;
-}
-
 // Scc += c c^H in the packed Hermitian layout of compress.cuh: 4 diagonal entries, then the 6 upper pairs
 __device__ __forceinline__ void gram_add(const m22& c, double* acc) {
 #pragma unroll

@@ -50,6 +50,9 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.sagecal_lm_cost_grad_jtj(4, 1, 1, z, 0, z, z, z, z, z, z, 0, z) == -1      # NULL pointers
     assert lib.sagecal_corrupt_subtract(4, 1, 1, 1, 7, z, z, z, -1.0, z, z, z) == -1      # bad coh_format
     assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, 0, z, z, z, 0, z) == -1
+    # lm_mode GROUPED (3) does not re-centre: n_lm > SAGECAL_LM_RECENTRE is refused; lm_mode 4 does not exist
+    assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 11, 1e-3, 3, z, z, z, 0, z) == -4
+    assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, 4, z, z, z, 0, z) == -1
     fr = (ctypes.c_double * 1)(150e6)
     off = (ctypes.c_int * 2)(0, 1)
     assert lib.sagecal_predict_coherencies(4, 1, 1, fr, 150e6, z, 1, off, z, z, z, z, z, z, z, 0, z, 0, z, 0, z) == -1
@@ -92,10 +95,12 @@ def test_mstep_tiling_covers_every_baseline_once(lib, N):
 
 def test_calibrate_workspace_covers_compressed_statistics(lib):
     """SAGECAL_WS_CALIBRATE holds the per-baseline statistics of the compressed mode: K x 16 doubles (gram of the
-    coherencies) + 33 doubles per baseline, on top of the direct pass's partial sums."""
+    coherencies) + 33 doubles per baseline, on top of the direct pass's partial sums; plus, for the cluster-group
+    path, 4 x 34 doubles of group statistics and 6 cross grams of 32 doubles per group of 4 clusters."""
     from paper_1910_13908_b200 import _binding as b
     N, T, F, K = 512, 20, 8, 50
     B = N * (N - 1) // 2
     ws = b.workspace_bytes(b.WS_CALIBRATE, N, T, F, K)
-    assert ws >= b.workspace_bytes(b.WS_LM_PASS, N, T, F) + 8 * B * (16 * K + 33)
-    assert ws < 1.2e9
+    groups = -(-K // 4)
+    assert ws >= b.workspace_bytes(b.WS_LM_PASS, N, T, F) + 8 * B * (16 * K + 33 + 4 * 34 + groups * 6 * 32)
+    assert ws < 4e9
