@@ -10,48 +10,80 @@
 //              srr_{i+1} = srr_i - Re tr(dW_i^H (Src_i + Sec_i))         (the cost per baseline after i's update)
 //   xgram:     X_ij and Scc_i of a group, once per interval (they depend on the coherencies only)
 //
-// (2 + 2 GRP) x 64 B per sample and group instead of GRP x 256 B: 160 B instead of 256 B per cluster at GRP = 4.
-// Nothing is approximated; the LM trajectory is the same to rounding.
+// (2 + 2 GRP) x 64 B per sample and group instead of GRP x 256 B: 160 B instead of 256 B per cluster at GRP = 4
+// (2x2 coherencies; 64 B instead of 160 B with scalar coherencies).  Nothing is approximated; the LM trajectory is the
+// same to rounding.
 //
-// Thread mapping of the streaming kernels: 4 lanes share one (baseline, channel) sample, lane a owns row a of the
-// 4x4 statistics (r_a conj(c_c), c = 0..3), so a thread carries 8 accumulators per cluster instead of 32 and a group
-// fits in registers.  At fixed t a warp touches 8 consecutive samples (512 B per array); the 4 lanes of a sample
-// read the same 64 B of C (one request) and each its own 16 B of R.  Sums over the channel lanes of a baseline by
-// warp shuffles, fixed order, no atomics.
+// Thread mapping of the streaming kernels.
+//   Scalar coherencies: one thread per (baseline, channel) sample as in wbstat.cu -- 8 accumulators per cluster.
+//   2x2 coherencies: 4 lanes share a sample and lane l owns COLUMN l of the 4x4 statistics (r_a conj(c_l), a = 0..3),
+//   8 accumulators per cluster instead of 32, so a group fits in registers.  Lane l loads only entry l of every
+//   coherency sample and of R (16 B each: a warp reads 512 contiguous bytes per array and time slot, nothing twice --
+//   a row-owning layout, where the 4 lanes of a sample each load the whole 64 B, ran at 92 % L1 throughput and 41 %
+//   of DRAM throughput).  The write-back needs a product over columns: every lane forms its column's contribution to
+//   all four rows and a 2-step reduce-scatter over the quad (12 shuffles) leaves row l in lane l; a 2-step all-gather
+//   (12 shuffles) then gives every lane the whole new r for its column of the statistics.
+// Sums over the channel lanes of a baseline by warp shuffles, fixed order, no atomics.
 #include "compress.cuh"
 
 namespace sgc {
 
-constexpr int WG_THREADS = 128, WG_SAMPLES = WG_THREADS / 4;
+constexpr int WG_THREADS = 128;
 
-// lanes of one baseline in a warp: 4 (rows a) x FP (channels); FP = smallest power of two >= F, at most 8
+// 2x2 coherencies: lanes of one baseline in a warp = 4 (columns) x FP (channels); FP = smallest power of two >= F, <= 8
 static inline int group_fp(int F) { int g = 1; while (g < F && g < 8) g <<= 1; return g; }
 
-__device__ __forceinline__ double chan_sum(double v, int FP) {   // over the FP channel lanes (lane bits 2..)
-    for (int o = FP >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, 4 * o);
-    return v;
-}
 __device__ __forceinline__ cplx ld_c(const sagecal_c128* p) {     // coherent 16 B load (R is written by this kernel)
     cplx r;
     asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(r.re), "=d"(r.im) : "l"(p) : "memory");
     return r;
 }
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 __device__ __forceinline__ void st_c(sagecal_c128* p, cplx v) {
     asm volatile("st.global.v2.f64 [%2], {%0,%1};" ::"d"(v.re), "d"(v.im), "l"(p) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+__device__ __forceinline__ cplx shfl_c(unsigned mask, cplx v, int x) {
+    return mk(__shfl_xor_sync(mask, v.re, x), __shfl_xor_sync(mask, v.im, x));
+}
+__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.re + b.re, a.im + b.im); }
+__device__ __forceinline__ cplx csel(bool s, cplx a, cplx b) { return s ? a : b; }
+// sum over lanes l, l ^ stride, l ^ 2 stride, ... (n lanes, n a power of two)
+__device__ __forceinline__ double lanes_sum(double v, int n, int stride) {
+    for (int o = n >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o * stride);
+    return v;
+}
+// every lane of a quad holds one entry x_l of a 4-vector: afterwards all four lanes hold the whole vector
+__device__ __forceinline__ void quad_gather(unsigned qmask, int lane, cplx mine, cplx out[4]) {
+    const int qb = lane & ~3;
+#pragma unroll
+    for (int a = 0; a < 4; a++) out[a] = mk(__shfl_sync(qmask, mine.re, qb + a), __shfl_sync(qmask, mine.im, qb + a));
+}
+// every lane of a quad holds a 4-vector v: afterwards lane l holds entry l of the sum of the four vectors
+__device__ __forceinline__ cplx quad_reduce_scatter(unsigned qmask, int l, const cplx v[4]) {
+    const bool odd = l & 1, hi = l & 2;
+    const cplx k0 = cadd(csel(hi, v[2], v[0]), shfl_c(qmask, csel(hi, v[0], v[2]), 2));
+    const cplx k1 = cadd(csel(hi, v[3], v[1]), shfl_c(qmask, csel(hi, v[1], v[3]), 2));
+    return cadd(csel(odd, k1, k0), shfl_c(qmask, csel(odd, k0, k1), 1));
+}
 
+// ---- write-back of the previous group + statistics of the next group ------------------------------------------------
 template <bool SCALAR, int GP, int GN>
 __global__ void __launch_bounds__(WG_THREADS, 3)
 wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ coh,
                size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev, const sagecal_c128* __restrict__ jones,
                int kn0, double* __restrict__ SrcG) {
     constexpr int NW = SCALAR ? 4 : 16;                  // entries of dP / dW per baseline and cluster
-    constexpr int NC = SCALAR ? 1 : 4;                   // entries of c a lane multiplies with
-    __shared__ cplx s_dw[GP > 0 ? GP : 1][NW][WG_SAMPLES];   // [cluster][entry][baseline of this CTA]
+    constexpr int LPS = SCALAR ? 1 : 4;                  // lanes per sample
+    constexpr int SPC = WG_THREADS / LPS;                // samples per CTA and time slot
+    constexpr int NSRC = SCALAR ? NSRC_SCALAR : NSRC_FULL;
+    constexpr int GPn = GP > 0 ? GP : 1, GNn = GN > 0 ? GN : 1;
+    // scalar: [cluster][entry][baseline] (a warp's lanes differ in the baseline); 2x2: [cluster][baseline][entry], 17
+    // entries per row (the 4 lanes of a sample read 4 consecutive entries, baselines fall on different banks)
+    constexpr int D1 = SCALAR ? NW : SPC, D2 = SCALAR ? SPC : NW + 1;
+    __shared__ cplx s_dw[GPn][D1][D2];
     const int tid = threadIdx.x;
-    const int a = tid & 3, s = tid >> 2;
-    const int BL = WG_SAMPLES / FP;                      // baselines per CTA
+    const int l = SCALAR ? 0 : (tid & 3), s = tid / LPS;
+    const int BL = SPC / FP;                             // baselines per CTA
     const int g = s / FP, fl = s - g * FP;
     const int64_t b = (int64_t)blockIdx.x * BL + g;
 
@@ -68,87 +100,98 @@ wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sa
                 const sagecal_c128* J = jones + (size_t)(kp0 + i) * N * 4;
                 v = SCALAR ? dP_entry(J0, J, p, q, w) : dW_entry(J0, J, p, q, w >> 2, w & 3);
             }
-            s_dw[i][w][bl] = v;
+            if (SCALAR) s_dw[i][w][bl] = v; else s_dw[i][bl][w] = v;
         }
         __syncthreads();
     }
 
-    cplx S[GN > 0 ? GN : 1][NC];
+    cplx S[GNn][4];                                      // scalar: Sr_j[a]; 2x2: column l of Src_j, S[j][a] = Src_j[a][l]
 #pragma unroll
-    for (int j = 0; j < (GN > 0 ? GN : 1); j++)
+    for (int j = 0; j < GNn; j++)
 #pragma unroll
-        for (int c = 0; c < NC; c++) S[j][c] = mk(0.0, 0.0);
+        for (int a = 0; a < 4; a++) S[j][a] = mk(0.0, 0.0);
     double rr = 0.0;
 
     if (b < B) {
         const sagecal_c128* cprev = coh + (size_t)kp0 * cstride;
         const sagecal_c128* cnext = coh + (size_t)kn0 * cstride;
+        const size_t step = (size_t)B * F;
+        const unsigned qmask = SCALAR ? 0u : (0xFu << ((tid & 31) & ~3));
         for (int f = fl; f < F; f += FP) {
             size_t idx = (size_t)b * F + f;
-            const size_t step = (size_t)B * F;
 #pragma unroll 1
             for (int t = 0; t < T; t++, idx += step) {
-                if (t + 1 < T) {   // next time slot's samples into L2: lane a fetches cluster a of either group
-                    const size_t nx = idx + step;
-                    if (a < GP) prefetch_l2(cprev + (size_t)a * cstride + nx * (SCALAR ? 1 : 4));
-                    if (a < GN) prefetch_l2(cnext + (size_t)a * cstride + nx * (SCALAR ? 1 : 4));
-                    if (a == 3) prefetch_l2(R + nx * 4);
-                }
-                cplx ra = ld_c(R + idx * 4 + a);
+                cplx cp[GPn], cn[GNn];
                 if (SCALAR) {
-                    cplx cp[GP > 0 ? GP : 1], cn[GN > 0 ? GN : 1];
+                    m22 r;
+                    load_m22(R + idx * 4, r);
 #pragma unroll
                     for (int i = 0; i < GP; i++) cp[i] = ldg128_stream(cprev + (size_t)i * cstride + idx);
 #pragma unroll
                     for (int j = 0; j < GN; j++) cn[j] = ldg128_stream(cnext + (size_t)j * cstride + idx);
 #pragma unroll
-                    for (int i = 0; i < GP; i++) ra = cfms(s_dw[i][a][g], cp[i], ra);
-                    if (GP > 0) st_c(R + idx * 4 + a, ra);
+                    for (int i = 0; i < GP; i++)
 #pragma unroll
-                    for (int j = 0; j < GN; j++) S[j][0] = cfmac(ra, cn[j], S[j][0]);
+                        for (int a = 0; a < 4; a++) r.a[a] = cfms(s_dw[i][a][g], cp[i], r.a[a]);
+                    if (GP > 0) store_m22(R + idx * 4, r);
+#pragma unroll
+                    for (int j = 0; j < GN; j++)
+#pragma unroll
+                        for (int a = 0; a < 4; a++) S[j][a] = cfmac(r.a[a], cn[j], S[j][a]);
+                    rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
                 } else {
+                    cplx rl = ld_c(R + idx * 4 + l);                     // r_l
 #pragma unroll
-                    for (int i = 0; i < GP; i++) {
-                        m22 cp;
-                        load_m22_stream(cprev + (size_t)i * cstride + idx * 4, cp);
+                    for (int i = 0; i < GP; i++) cp[i] = ldg128_stream(cprev + (size_t)i * cstride + idx * 4 + l);
 #pragma unroll
-                        for (int c = 0; c < 4; c++) ra = cfms(s_dw[i][4 * a + c][g], cp.a[c], ra);
+                    for (int j = 0; j < GN; j++) cn[j] = ldg128_stream(cnext + (size_t)j * cstride + idx * 4 + l);
+                    if (GP > 0) {
+                        // column l of the write-back: v[a] = sum_i dW_i[a][l] c_i[l]; row l of the total to lane l
+                        cplx v[4];
+#pragma unroll
+                        for (int a = 0; a < 4; a++) v[a] = mk(0.0, 0.0);
+#pragma unroll
+                        for (int i = 0; i < GP; i++)
+#pragma unroll
+                            for (int a = 0; a < 4; a++) v[a] = cfma(s_dw[i][g][4 * a + l], cp[i], v[a]);
+                        const cplx w = quad_reduce_scatter(qmask, l, v);
+                        rl = mk(rl.re - w.re, rl.im - w.im);
+                        st_c(R + idx * 4 + l, rl);
                     }
-                    if (GP > 0) st_c(R + idx * 4 + a, ra);
+                    if (GN > 0) {
+                        cplx r[4];
+                        quad_gather(qmask, tid & 31, rl, r);
 #pragma unroll
-                    for (int j = 0; j < GN; j++) {
-                        m22 cn;
-                        load_m22_stream(cnext + (size_t)j * cstride + idx * 4, cn);
+                        for (int j = 0; j < GN; j++)
 #pragma unroll
-                        for (int c = 0; c < 4; c++) S[j][c] = cfmac(ra, cn.a[c], S[j][c]);
+                            for (int a = 0; a < 4; a++) S[j][a] = cfmac(r[a], cn[j], S[j][a]);
                     }
+                    rr = cabs2(rl, rr);
                 }
-                rr = cabs2(ra, rr);
             }
         }
     }
     if (GN > 0) {
-        constexpr int NSRC = SCALAR ? NSRC_SCALAR : NSRC_FULL;
         const bool writer = fl == 0 && b < B;
+        const size_t bb = b < B ? (size_t)b : 0;
 #pragma unroll
         for (int j = 0; j < GN; j++) {
-            double* rec = SrcG + ((size_t)j * B + (b < B ? b : 0)) * NSRC;
+            double* rec = SrcG + ((size_t)j * B + bb) * NSRC;
 #pragma unroll
-            for (int c = 0; c < NC; c++) {
-                const double re = chan_sum(S[j][c].re, FP), im = chan_sum(S[j][c].im, FP);
+            for (int a = 0; a < 4; a++) {
+                const double re = lanes_sum(S[j][a].re, FP, LPS), im = lanes_sum(S[j][a].im, FP, LPS);
                 if (writer) {
-                    rec[2 * (NC * a + c)] = re;
-                    rec[2 * (NC * a + c) + 1] = im;
+                    const int e = SCALAR ? a : 4 * a + l;
+                    rec[2 * e] = re;
+                    rec[2 * e + 1] = im;
                 }
             }
         }
-        rr = chan_sum(rr, FP);
-        rr += __shfl_xor_sync(0xffffffffu, rr, 1);
-        rr += __shfl_xor_sync(0xffffffffu, rr, 2);
-        if (writer && a == 0) {
+        rr = lanes_sum(rr, FP * LPS, 1);
+        if (writer && l == 0) {
 #pragma unroll
             for (int j = 0; j < GN; j++) {
-                double* rec = SrcG + ((size_t)j * B + b) * NSRC;
+                double* rec = SrcG + ((size_t)j * B + bb) * NSRC;
                 rec[NSRC - 2] = rr;        // meaningful for j = 0; groupfix rewrites it for the later clusters
                 rec[NSRC - 1] = 0.0;
             }
@@ -156,56 +199,49 @@ wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sa
     }
 }
 
-
-// Scc_i and X_ij (i < j) of the GN clusters kn0.. of a group.  Lane a owns row a: X_ij[a][c] = sum c_i[a] conj(c_j[c]).
+// ---- Scc_i and X_ij (i < j) of the GN clusters kn0.. of a group -------------------------------------------------------
+// 2x2: lane l owns column l, X_ij[a][l] = sum c_i[a] conj(c_j[l]); the rows c_i[a] come from the quad by an all-gather.
 template <bool SCALAR, int GN>
-__global__ void __launch_bounds__(WG_THREADS, 2)
+__global__ void __launch_bounds__(WG_THREADS, SCALAR ? 4 : 2)
 xgram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, size_t cstride, int kn0,
              double* __restrict__ Scc, double* __restrict__ Xg) {
-    constexpr int NC = SCALAR ? 1 : 4;
+    constexpr int NR = SCALAR ? 1 : 4;
+    constexpr int LPS = SCALAR ? 1 : 4;
+    constexpr int SPC = WG_THREADS / LPS;
     constexpr int NP = GN * (GN + 1) / 2;                // pairs i <= j
     const int tid = threadIdx.x;
-    const int a = tid & 3, s = tid >> 2;
-    const int BL = WG_SAMPLES / FP;
+    const int l = SCALAR ? 0 : (tid & 3), s = tid / LPS;
+    const int BL = SPC / FP;
     const int g = s / FP, fl = s - g * FP;
     const int64_t b = (int64_t)blockIdx.x * BL + g;
-    cplx X[NP][NC];
+    cplx X[NP][NR];
 #pragma unroll
     for (int n = 0; n < NP; n++)
 #pragma unroll
-        for (int c = 0; c < NC; c++) X[n][c] = mk(0.0, 0.0);
+        for (int a = 0; a < NR; a++) X[n][a] = mk(0.0, 0.0);
 
     if (b < B) {
         const sagecal_c128* cb = coh + (size_t)kn0 * cstride;
+        const size_t step = (size_t)B * F;
+        const unsigned qmask = SCALAR ? 0u : (0xFu << ((tid & 31) & ~3));
         for (int f = fl; f < F; f += FP) {
             size_t idx = (size_t)b * F + f;
-            const size_t step = (size_t)B * F;
 #pragma unroll 1
             for (int t = 0; t < T; t++, idx += step) {
-                if (t + 1 < T && a < GN) prefetch_l2(cb + (size_t)a * cstride + (idx + step) * (SCALAR ? 1 : 4));
-                if (SCALAR) {
-                    cplx c[GN];
+                cplx c[GN];
 #pragma unroll
-                    for (int i = 0; i < GN; i++) c[i] = ldg128_stream(cb + (size_t)i * cstride + idx);
-                    int n = 0;
+                for (int i = 0; i < GN; i++) c[i] = ldg128_stream(cb + (size_t)i * cstride + idx * LPS + l);
+                if (!SCALAR && t + 2 < T && l < GN) prefetch_l2(cb + (size_t)l * cstride + (idx + 2 * step) * 4);
+                int n = 0;
 #pragma unroll
-                    for (int i = 0; i < GN; i++)
+                for (int i = 0; i < GN; i++) {
+                    cplx ci[4];
+                    if (SCALAR) ci[0] = c[i];
+                    else quad_gather(qmask, tid & 31, c[i], ci);
 #pragma unroll
-                        for (int j = i; j < GN; j++, n++) X[n][0] = cfmac(c[i], c[j], X[n][0]);
-                } else {
-                    m22 c[GN];
+                    for (int j = i; j < GN; j++, n++)
 #pragma unroll
-                    for (int i = 0; i < GN; i++) load_m22_stream(cb + (size_t)i * cstride + idx * 4, c[i]);
-                    int n = 0;
-#pragma unroll
-                    for (int i = 0; i < GN; i++) {
-                        // c_i[a] without dynamic register indexing
-                        const cplx ca = a == 0 ? c[i].a[0] : a == 1 ? c[i].a[1] : a == 2 ? c[i].a[2] : c[i].a[3];
-#pragma unroll
-                        for (int j = i; j < GN; j++, n++)
-#pragma unroll
-                            for (int cc = 0; cc < 4; cc++) X[n][cc] = cfmac(ca, c[j].a[cc], X[n][cc]);
-                    }
+                        for (int a = 0; a < NR; a++) X[n][a] = cfmac(ci[a], c[j], X[n][a]);
                 }
             }
         }
@@ -217,31 +253,31 @@ xgram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ c
     for (int i = 0; i < GN; i++) {
 #pragma unroll
         for (int j = i; j < GN; j++, n++) {
-            double re[NC], im[NC];
+            double re[NR], im[NR];
 #pragma unroll
-            for (int c = 0; c < NC; c++) { re[c] = chan_sum(X[n][c].re, FP); im[c] = chan_sum(X[n][c].im, FP); }
+            for (int a = 0; a < NR; a++) { re[a] = lanes_sum(X[n][a].re, FP, LPS); im[a] = lanes_sum(X[n][a].im, FP, LPS); }
             if (!writer) continue;
             if (i == j) {
                 double* o = Scc + ((size_t)(kn0 + i) * B + bb) * (SCALAR ? NSCC_SCALAR : NSCC_FULL);
-                if (SCALAR) { if (a == 0) o[0] = re[0]; }
+                if (SCALAR) o[0] = re[0];
                 else {
-                    // packed Hermitian: diagonal [a], then the upper pairs (a, c > a) in the order of compress.cuh
+                    // packed Hermitian: diagonal [l], then the upper pairs (a < l, l) in the order of compress.cuh
 #pragma unroll
-                    for (int c = 0; c < 4; c++) {
-                        if (c == a) o[a] = re[c];
-                        else if (c > a) {
-                            const int pr = a * 4 - a * (a + 1) / 2 + (c - a - 1);
-                            o[4 + 2 * pr] = re[c];
-                            o[5 + 2 * pr] = im[c];
+                    for (int a = 0; a < NR; a++) {
+                        if (a == l) o[l] = re[a];
+                        else if (a < l) {
+                            const int pr = a * 4 - a * (a + 1) / 2 + (l - a - 1);
+                            o[4 + 2 * pr] = re[a];
+                            o[5 + 2 * pr] = im[a];
                         }
                     }
                 }
             } else {
                 double* o = Xg + ((size_t)grp_pair(i, j) * B + bb) * (SCALAR ? NX_SCALAR : NX_FULL);
-                if (SCALAR) { if (a == 0) { o[0] = re[0]; o[1] = im[0]; } }
+                if (SCALAR) { o[0] = re[0]; o[1] = im[0]; }
                 else {
 #pragma unroll
-                    for (int c = 0; c < 4; c++) { o[2 * (4 * a + c)] = re[c]; o[2 * (4 * a + c) + 1] = im[c]; }
+                    for (int a = 0; a < NR; a++) { o[2 * (4 * a + l)] = re[a]; o[2 * (4 * a + l) + 1] = im[a]; }
                 }
             }
         }
@@ -341,7 +377,7 @@ static int launch_wbgroup(int N, int T, int F, sagecal_c128* R, const sagecal_c1
                           const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn, double* SrcG,
                           cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = group_fp(F), BL = WG_SAMPLES / FP;
+    const int FP = SCALAR ? stat_group(F) : group_fp(F), BL = (SCALAR ? WG_THREADS : WG_THREADS / 4) / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_WBSTAT, st);
 #define SGC_GP(GP_) launch_wbgroup_gn<SCALAR, GP_>(gn, grid, st, N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
@@ -372,7 +408,7 @@ template <bool SCALAR>
 static int launch_xgram(int N, int T, int F, const sagecal_c128* coh, size_t cstride, int kn0, int gn, double* Scc,
                         double* Xg, cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = group_fp(F), BL = WG_SAMPLES / FP;
+    const int FP = SCALAR ? stat_group(F) : group_fp(F), BL = (SCALAR ? WG_THREADS : WG_THREADS / 4) / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_XGRAM, st);
 #define SGC_XG(GN_) xgram_kernel<SCALAR, GN_><<<grid, WG_THREADS, 0, st>>>(T, F, FP, B, coh, cstride, kn0, Scc, Xg)
