@@ -261,3 +261,40 @@ def test_calibrate_compressed_is_bit_reproducible(cuda_device, fmt):
     for r in runs[1:]:
         for k in ("jones", "residual", "cost_per_cluster", "cost_trace"):
             assert np.array_equal(r[k], runs[0][k]), k
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("scalar", [False, True])
+def test_calibrate_degenerate_iteration_counts(cuda_device, mode, scalar):
+    """n_lm = 0 (every M-step is one evaluation, no trial step: Jones stay at the start values, the per-cluster
+    cost is ||R||^2 of the initial residual) and n_em = 0 (initial residual only) in every mode and format; K = 0
+    returns the visibilities as residual."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, host
+    p = make_problem(9, 3, 2, 5, 3, seed=61, sigma=0.05, layout="disc:5000", field_deg=4.0, patch_deg=0.5)
+    fmt = sg.COH_SCALAR if scalar else sg.COH_FULL
+    want, got, V, coh = _run_both_nocheck(p, 2, 0, fmt, mode)
+    assert np.array_equal(got["jones"], p.jones_init())
+    assert rel_l2(got["residual"], want["residual"]) < 1e-12
+    assert np.allclose(got["cost_per_cluster"], want["cost_per_cluster"], rtol=1e-12)
+    assert np.allclose(got["cost_trace"], want["cost_trace"], rtol=1e-12)
+    want0, got0, _, _ = _run_both_nocheck(p, 0, 3, fmt, mode)
+    assert rel_l2(got0["residual"], want0["residual"]) < 1e-12 and np.array_equal(got0["jones"], p.jones_init())
+    # K = 0: nothing to subtract
+    Vd = dev(V)
+    out = sg.sage_calibrate(p.N, p.T, p.F, Vd, torch.empty((0, p.rows, p.F, 4), dtype=torch.complex128, device="cuda:0"),
+                            torch.empty((0, p.N, 2, 2), dtype=torch.complex128, device="cuda:0"), 2, 3, p.tau,
+                            lm_mode=_mode(mode))
+    assert np.array_equal(host(out["residual"]), V)
+
+
+def _run_both_nocheck(p, n_em, n_lm, fmt, mode):
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, host
+    coh = oracle.predict(p)
+    V = oracle.simulate(p, coh)
+    want = oracle.sage(p.N, p.T, p.F, V, coh, p.jones_init(), n_em, n_lm, p.tau)
+    got = sg.sage_calibrate(p.N, p.T, p.F, dev(V), gpu_predict(p, fmt), dev(p.jones_init()), n_em, n_lm, p.tau,
+                            coh_format=fmt, lm_mode=_mode(mode))
+    return want, {k: (None if v is None else host(v)) for k, v in got.items()}, V, coh

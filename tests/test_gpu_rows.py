@@ -160,3 +160,43 @@ def test_fully_flagged_station_keeps_its_start_jones(cuda_device):
     got = _pipeline(prob, rl, vis, 1, 6, sg.LM_COMPRESSED, sg.COH_FULL)
     _compare(want, got)
     assert np.array_equal(got["jones"][0, dead], np.eye(2)) and np.array_equal(want["jones"][0, dead], np.eye(2))
+
+
+def test_rows_front_end_at_the_bench_size(cuda_device):
+    """configs[4]'s shape (2.6 M slots x 8 channels), the row list bench.py --rows times.  The loop oracle is too slow
+    here, so: everything that is index work is checked in full against the generator's own bookkeeping (which slot a
+    row belongs to, whether it was swapped), the sample contents on 4096 sampled rows and on sampled empty slots, and
+    the round trip back to row order bit for bit."""
+    import paper_1910_13908_b200 as sg
+    import torch
+    from tests.gpu_util import dev, host
+    prob = si.make_config(4)
+    rl = si.make_rowlist(prob, seed=prob.seed + 1000, drop_frac=0.05, swap_frac=0.3, flag_frac=0.05)
+    n, F = len(rl.ant1), prob.F
+    vis = rl.noise                                             # any content will do: this is index work
+    can = _to_canonical(prob, rl, vis)
+    swapped = rl.ant1 > rl.ant2
+    assert np.array_equal(host(can["row_map"]), 2 * rl.canonical_row + swapped)
+    st = host(can["status"])
+    assert list(st[:3]) == [0, 0, 0] and st[3] == prob.rows - n
+    fl_c = host(can["flags"])
+    want_fl = np.ones((prob.rows, F), np.uint8)
+    want_fl[rl.canonical_row] = rl.flags
+    assert np.array_equal(fl_c, want_fl)
+    rng = np.random.default_rng(8)
+    pick = np.sort(rng.choice(n, 4096, replace=False))
+    slots = torch.from_numpy(rl.canonical_row[pick]).to("cuda:0")
+    got_v, got_u = host(can["vis"][slots]), host(can["uvw"][slots])
+    want_v = np.where(swapped[pick, None, None], vis[pick][:, :, [0, 2, 1, 3]].conj(), vis[pick])
+    want_v = np.where(rl.flags[pick][:, :, None] != 0, 0.0, want_v)
+    assert np.array_equal(got_v, want_v)
+    assert np.array_equal(got_u, prob.uvw[rl.canonical_row[pick]])        # the swap negated uvw back
+    empty = np.setdiff1d(np.arange(prob.rows), rl.canonical_row)[:2048]
+    e_d = torch.from_numpy(empty).to("cuda:0")
+    assert not host(can["vis"][e_d]).any() and not host(can["uvw"][e_d]).any()
+    back = torch.zeros((n, F, 4), dtype=torch.complex128, device="cuda:0")
+    sg.canonical_to_rows(prob.N, prob.T, F, can["row_map"], can["vis"], back)
+    got_b = host(back[torch.from_numpy(pick).to("cuda:0")])
+    assert np.array_equal(got_b, np.where(rl.flags[pick][:, :, None] != 0, 0.0, vis[pick]))
+    del can, back
+    torch.cuda.empty_cache()
