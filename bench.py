@@ -80,9 +80,9 @@ def passes_per_interval(K: int, n_em: int, n_lm: int) -> int:
 
 
 def uses_groups(lm: str, coh: str, n_lm: int) -> bool:
-    """Which streaming kernel sagecal_sage_calibrate runs (calibrate.cu): cluster groups when forced (lm grouped) or,
-    in compressed mode, for scalar coherencies -- where that is the faster order."""
-    return n_lm <= LM_RECENTRE and (lm == "grouped" or (lm == "compressed" and coh == "scalar"))
+    """Which streaming kernel sagecal_sage_calibrate runs (calibrate.cu): cluster groups in compressed mode whenever an
+    M-step is one chunk; cluster by cluster for lm percluster, fullgn and longer M-steps."""
+    return lm == "compressed" and n_lm <= LM_RECENTRE
 
 
 def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "direct", coh: str = "full") -> int:
@@ -296,7 +296,7 @@ def run_ours(args):
     # ---- inputs: replicas, every rank its own interval (seed offset by rank) ----
     p = make_config(args.config, seed=191013908 + args.config + 1000 * rank)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "grouped": sg.LM_GROUPED}[args.lm]
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "percluster": sg.LM_PERCLUSTER}[args.lm]
     # the dominant kernel of the step, the one `roofline` describes
     top = "lm_pass" if args.lm == "direct" else "wbstat"
     N, T, F, K = p.N, p.T, p.F, p.K
@@ -484,7 +484,7 @@ def run_grid(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
-    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "grouped": sg.LM_GROUPED}[args.lm]
+    lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "percluster": sg.LM_PERCLUSTER}[args.lm]
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
     for N in (64, 128, 256, 384, 512):
@@ -587,7 +587,7 @@ def main(argv=None):
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=4, choices=[0, 1, 2, 3, 4])
     ap.add_argument("--coh", choices=["full", "scalar"], default="full")
-    ap.add_argument("--lm", choices=["compressed", "direct", "fullgn", "grouped"], default="compressed",
+    ap.add_argument("--lm", choices=["compressed", "direct", "fullgn", "percluster"], default="compressed",
                     help="lm_mode of sagecal_sage_calibrate (DESIGN.md §5.5, §5.6); direct = every evaluation streams the "
                          "samples; fullgn = full Gauss-Newton matrix + cuSOLVER Cholesky (a different iteration, NEXT-2)")
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")

@@ -61,7 +61,7 @@ typedef struct { double re, im; } sagecal_c128;
  * Both follow the same LM trajectory and agree to rounding. */
 #define SAGECAL_LM_COMPRESSED 0  /* default: per-baseline time/frequency statistics of the residual, taken once per
                                     (EM iteration, cluster) in the same streaming kernel that writes back the previous
-                                    cluster; the n_lm+1 evaluations and the LM control then run in one cooperative
+                                    clusters; the n_lm+1 evaluations and the LM control then run in one cooperative
                                     kernel that reads 392 B per baseline instead of 128 B per sample */
 #define SAGECAL_LM_DIRECT     1  /* every evaluation streams the cluster's T*F samples (sagecal_lm_cost_grad_jtj) */
 #define SAGECAL_LM_FULLGN     2  /* the other reading of "per-station-block J^H J ... small dense per-cluster solve"
@@ -69,12 +69,13 @@ typedef struct { double re, im; } sagecal_c128;
                                     block per baseline, damped Cholesky with cuSOLVER, on the compressed statistics.
                                     A different iteration (it converges in a handful of steps), not the hot path;
                                     needs the SAGECAL_WS_CALIBRATE_FULLGN workspace (3 x (8N)^2 doubles more). */
-#define SAGECAL_LM_GROUPED    3  /* SAGECAL_LM_COMPRESSED with the streaming kernel working on groups of 4 consecutive
-                                    clusters (one read and one write of R per group; statistics corrected inside a
-                                    group through cross grams of the coherencies; DESIGN.md §5.5 "cluster groups").
-                                    Same trajectory to rounding.  SAGECAL_LM_COMPRESSED already takes this route where
-                                    it is the faster one (scalar coherencies, n_lm <= SAGECAL_LM_RECENTRE); the value
-                                    forces it for either format.  n_lm > SAGECAL_LM_RECENTRE: SAGECAL_EUNSUPPORTED. */
+#define SAGECAL_LM_PERCLUSTER 3  /* SAGECAL_LM_COMPRESSED with the cluster-by-cluster streaming kernel forced on (one
+                                    read and one write of R per cluster, wbstat.cu).  SAGECAL_LM_COMPRESSED itself works
+                                    on groups of 4 consecutive clusters whenever an M-step is a single chunk
+                                    (n_lm <= SAGECAL_LM_RECENTRE): one read and one write of R per group, statistics
+                                    corrected inside a group through cross grams of the coherencies, on the FP64 tensor
+                                    cores for 2x2 coherencies (DESIGN.md §5.5 "cluster groups"); longer M-steps take the
+                                    cluster-by-cluster route.  Same trajectory to rounding either way. */
 /* compressed mode re-takes the statistics at the accepted Jones every this many trial steps of one M-step */
 #define SAGECAL_LM_RECENTRE  10
 
@@ -190,7 +191,7 @@ int sagecal_lm_cost_grad_jtj(
  * jones   : dev [K][N][4], in = start values, out = solution.
  * residual: dev out [rows][F][4]; must not alias vis.
  * tau     : initial damping factor (1e-3 in all configs).
- * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT, SAGECAL_LM_FULLGN or SAGECAL_LM_GROUPED (above).
+ * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT, SAGECAL_LM_FULLGN or SAGECAL_LM_PERCLUSTER (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.
  * cost_trace       : dev out [n_em*K + 1] f64 or NULL: ||R||^2 at the start and after every M-step.
  * workspace: dev scratch >= sagecal_workspace_bytes(SAGECAL_WS_CALIBRATE or ..._FULLGN, N, T, F, K).

@@ -11,7 +11,7 @@ from ._binding import (  # noqa: F401
     LM_COMPRESSED,
     LM_DIRECT,
     LM_FULLGN,
-    LM_GROUPED,
+    LM_PERCLUSTER,
     SagecalError,
     apply_flags,
     canonical_to_rows,
@@ -32,7 +32,7 @@ from ._binding import (  # noqa: F401
 )
 
 __all__ = [
-    "COH_FULL", "COH_SCALAR", "LM_COMPRESSED", "LM_DIRECT", "LM_FULLGN", "LM_GROUPED", "SagecalError", "apply_flags", "canonical_to_rows", "rows_to_canonical", "calibrate_interval_host", "corrupt_subtract", "kernel_kinds",
+    "COH_FULL", "COH_SCALAR", "LM_COMPRESSED", "LM_DIRECT", "LM_FULLGN", "LM_PERCLUSTER", "SagecalError", "apply_flags", "canonical_to_rows", "rows_to_canonical", "calibrate_interval_host", "corrupt_subtract", "kernel_kinds",
     "launch_count", "lib_path", "lm_cost_grad_jtj", "load_library", "predict_coherencies", "profile_enable",
     "profile_read", "sage_calibrate", "version", "workspace_bytes",
 ]

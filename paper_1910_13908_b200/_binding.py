@@ -13,7 +13,7 @@ COH_SCALAR = 1
 LM_COMPRESSED = 0
 LM_DIRECT = 1
 LM_FULLGN = 2
-LM_GROUPED = 3
+LM_PERCLUSTER = 3
 WS_LM_PASS = 1
 WS_CALIBRATE_FULLGN = 3
 WS_CALIBRATE = 2

@@ -250,8 +250,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                                       void* workspace, size_t workspace_bytes, void* stream) {
     if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
-    if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT && lm_mode != SAGECAL_LM_FULLGN && lm_mode != SAGECAL_LM_GROUPED) return SAGECAL_EINVAL;
-    if (lm_mode == SAGECAL_LM_GROUPED && n_lm > SAGECAL_LM_RECENTRE) return SAGECAL_EUNSUPPORTED;
+    if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT && lm_mode != SAGECAL_LM_FULLGN && lm_mode != SAGECAL_LM_PERCLUSTER) return SAGECAL_EINVAL;
     if (!vis || !residual || vis == residual || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
     if (K > 0 && (!coh || !jones || !cost_per_cluster)) return SAGECAL_EINVAL;
     if (K > 0 && (!aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32) || !aligned(jones, 16))) return SAGECAL_EINVAL;
@@ -318,10 +317,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     // gram Scc_k of the coherencies, kept for the later ones), then ONE cooperative kernel runs
     // the n_lm+1 evaluations and the LM control on the per-baseline statistics.  Statistics are re-centred every
     // SAGECAL_LM_RECENTRE trial steps.
-    // SAGECAL_LM_COMPRESSED picks the faster of the two arithmetic orders: cluster groups for scalar coherencies
-    // (0.129 against 0.151 s per cfg4 interval), cluster by cluster for 2x2 coherencies, where the group kernel is
-    // bound by load-return bandwidth rather than by HBM (0.295 against 0.223 s)
-    if (lm_mode == SAGECAL_LM_GROUPED || (lm_mode == SAGECAL_LM_COMPRESSED && scalar && n_lm <= SAGECAL_LM_RECENTRE)) {
+    if (lm_mode == SAGECAL_LM_COMPRESSED && n_lm <= SAGECAL_LM_RECENTRE) {
         // cluster groups (wbgroup.cu): the write-back of GRP consecutive clusters is deferred and done in one pass
         // over R together with the statistics of the next GRP clusters; inside a group the statistics taken of the
         // stale residual are corrected per baseline through the cross grams X_ij of the coherencies.  An M-step is one
@@ -357,6 +353,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
         return enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, 0, 0, w.cw.SrcG, st);
     }
 
+    // cluster by cluster: SAGECAL_LM_PERCLUSTER, SAGECAL_LM_FULLGN, and compressed M-steps longer than one chunk
     const sagecal_c128* Cprev = nullptr;      // cluster whose write-back is pending
     const sagecal_c128* Jprev = nullptr;
     const int64_t B = g.B;

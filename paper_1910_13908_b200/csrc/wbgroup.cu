@@ -14,98 +14,51 @@
 // (2x2 coherencies; 64 B instead of 160 B with scalar coherencies).  Nothing is approximated; the LM trajectory is the
 // same to rounding.
 //
-// Thread mapping of the streaming kernels.
-//   Scalar coherencies: one thread per (baseline, channel) sample as in wbstat.cu -- 8 accumulators per cluster.
-//   2x2 coherencies: 4 lanes share a sample and lane l owns COLUMN l of the 4x4 statistics (r_a conj(c_l), a = 0..3),
-//   8 accumulators per cluster instead of 32, so a group fits in registers.  Lane l loads only entry l of every
-//   coherency sample and of R (16 B each: a warp reads 512 contiguous bytes per array and time slot, nothing twice --
-//   a row-owning layout, where the 4 lanes of a sample each load the whole 64 B, ran at 92 % L1 throughput and 41 %
-//   of DRAM throughput).  The write-back needs a product over columns: every lane forms its column's contribution to
-//   all four rows and a 2-step reduce-scatter over the quad (12 shuffles) leaves row l in lane l; a 2-step all-gather
-//   (12 shuffles) then gives every lane the whole new r for its column of the statistics.
-// Sums over the channel lanes of a baseline by warp shuffles, fixed order, no atomics.
+// Scalar coherencies: plain FP64 FMAs, one thread per (baseline, channel) sample as in wbstat.cu (8 accumulators per
+// cluster); sums over the channel lanes of a baseline by warp shuffles.  2x2 coherencies: the FP64 tensor cores, one
+// warp per baseline (below).  Fixed order, no atomics.
 #include "compress.cuh"
 
 namespace sgc {
 
 constexpr int WG_THREADS = 128;
 
-// 2x2 coherencies: lanes of one baseline in a warp = 4 (columns) x FP (channels); FP = smallest power of two >= F, <= 8
-static inline int group_fp(int F) { int g = 1; while (g < F && g < 8) g <<= 1; return g; }
-
-__device__ __forceinline__ cplx ld_c(const sagecal_c128* p) {     // coherent 16 B load (R is written by this kernel)
-    cplx r;
-    asm volatile("ld.global.v2.f64 {%0,%1}, [%2];" : "=d"(r.re), "=d"(r.im) : "l"(p) : "memory");
-    return r;
-}
-__device__ __forceinline__ void st_c(sagecal_c128* p, cplx v) {
-    asm volatile("st.global.v2.f64 [%2], {%0,%1};" ::"d"(v.re), "d"(v.im), "l"(p) : "memory");
-}
-__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-__device__ __forceinline__ cplx shfl_c(unsigned mask, cplx v, int x) {
-    return mk(__shfl_xor_sync(mask, v.re, x), __shfl_xor_sync(mask, v.im, x));
-}
-__device__ __forceinline__ cplx cadd(cplx a, cplx b) { return mk(a.re + b.re, a.im + b.im); }
-__device__ __forceinline__ cplx csel(bool s, cplx a, cplx b) { return s ? a : b; }
-// sum over lanes l, l ^ stride, l ^ 2 stride, ... (n lanes, n a power of two)
-__device__ __forceinline__ double lanes_sum(double v, int n, int stride) {
-    for (int o = n >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o * stride);
+// sum over n consecutive lanes (n a power of two)
+__device__ __forceinline__ double lanes_sum(double v, int n) {
+    for (int o = n >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
     return v;
 }
-// every lane of a quad holds one entry x_l of a 4-vector: afterwards all four lanes hold the whole vector
-__device__ __forceinline__ void quad_gather(unsigned qmask, int lane, cplx mine, cplx out[4]) {
-    const int qb = lane & ~3;
-#pragma unroll
-    for (int a = 0; a < 4; a++) out[a] = mk(__shfl_sync(qmask, mine.re, qb + a), __shfl_sync(qmask, mine.im, qb + a));
-}
-// every lane of a quad holds a 4-vector v: afterwards lane l holds entry l of the sum of the four vectors
-__device__ __forceinline__ cplx quad_reduce_scatter(unsigned qmask, int l, const cplx v[4]) {
-    const bool odd = l & 1, hi = l & 2;
-    const cplx k0 = cadd(csel(hi, v[2], v[0]), shfl_c(qmask, csel(hi, v[0], v[2]), 2));
-    const cplx k1 = cadd(csel(hi, v[3], v[1]), shfl_c(qmask, csel(hi, v[1], v[3]), 2));
-    return cadd(csel(odd, k1, k0), shfl_c(qmask, csel(odd, k0, k1), 1));
-}
 
-// ---- write-back of the previous group + statistics of the next group ------------------------------------------------
-template <bool SCALAR, int GP, int GN>
+// ---- scalar coherencies: write-back of the previous group + statistics of the next group ------------------------------
+template <int GP, int GN>
 __global__ void __launch_bounds__(WG_THREADS, 3)
-wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ coh,
-               size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev, const sagecal_c128* __restrict__ jones,
-               int kn0, double* __restrict__ SrcG) {
-    constexpr int NW = SCALAR ? 4 : 16;                  // entries of dP / dW per baseline and cluster
-    constexpr int LPS = SCALAR ? 1 : 4;                  // lanes per sample
-    constexpr int SPC = WG_THREADS / LPS;                // samples per CTA and time slot
-    constexpr int NSRC = SCALAR ? NSRC_SCALAR : NSRC_FULL;
+wbgroup_scalar_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ coh,
+                      size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev,
+                      const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG) {
     constexpr int GPn = GP > 0 ? GP : 1, GNn = GN > 0 ? GN : 1;
-    // scalar: [cluster][entry][baseline] (a warp's lanes differ in the baseline); 2x2: [cluster][baseline][entry], 17
-    // entries per row (the 4 lanes of a sample read 4 consecutive entries, baselines fall on different banks)
-    constexpr int D1 = SCALAR ? NW : SPC, D2 = SCALAR ? SPC : NW + 1;
-    __shared__ cplx s_dw[GPn][D1][D2];
+    __shared__ cplx s_dp[GPn][4][WG_THREADS];            // dP_i[a] per [cluster][entry][baseline of this CTA]
     const int tid = threadIdx.x;
-    const int l = SCALAR ? 0 : (tid & 3), s = tid / LPS;
-    const int BL = SPC / FP;                             // baselines per CTA
-    const int g = s / FP, fl = s - g * FP;
+    const int BL = WG_THREADS / FP;                      // baselines per CTA
+    const int g = tid / FP, fl = tid - g * FP;
     const int64_t b = (int64_t)blockIdx.x * BL + g;
 
     if (GP > 0) {
-        for (int e = tid; e < BL * NW * GP; e += WG_THREADS) {
-            const int i = e / (BL * NW), rem = e - i * (BL * NW);
-            const int bl = rem / NW, w = rem - bl * NW;
+        for (int e = tid; e < BL * 4 * GP; e += WG_THREADS) {
+            const int i = e / (BL * 4), rem = e - i * (BL * 4);
+            const int bl = rem >> 2, w = rem & 3;
             const int64_t bb = (int64_t)blockIdx.x * BL + bl;
             cplx v = mk(0.0, 0.0);
             if (bb < B) {
                 int p, q;
                 bl_stations(N, bb, p, q);
-                const sagecal_c128* J0 = J0prev + (size_t)i * N * 4;
-                const sagecal_c128* J = jones + (size_t)(kp0 + i) * N * 4;
-                v = SCALAR ? dP_entry(J0, J, p, q, w) : dW_entry(J0, J, p, q, w >> 2, w & 3);
+                v = dP_entry(J0prev + (size_t)i * N * 4, jones + (size_t)(kp0 + i) * N * 4, p, q, w);
             }
-            if (SCALAR) s_dw[i][w][bl] = v; else s_dw[i][bl][w] = v;
+            s_dp[i][w][bl] = v;
         }
         __syncthreads();
     }
 
-    cplx S[GNn][4];                                      // scalar: Sr_j[a]; 2x2: column l of Src_j, S[j][a] = Src_j[a][l]
+    cplx S[GNn][4];                                      // Sr_j[a]
 #pragma unroll
     for (int j = 0; j < GNn; j++)
 #pragma unroll
@@ -116,58 +69,27 @@ wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sa
         const sagecal_c128* cprev = coh + (size_t)kp0 * cstride;
         const sagecal_c128* cnext = coh + (size_t)kn0 * cstride;
         const size_t step = (size_t)B * F;
-        const unsigned qmask = SCALAR ? 0u : (0xFu << ((tid & 31) & ~3));
         for (int f = fl; f < F; f += FP) {
             size_t idx = (size_t)b * F + f;
 #pragma unroll 1
             for (int t = 0; t < T; t++, idx += step) {
                 cplx cp[GPn], cn[GNn];
-                if (SCALAR) {
-                    m22 r;
-                    load_m22(R + idx * 4, r);
+                m22 r;
+                load_m22(R + idx * 4, r);
 #pragma unroll
-                    for (int i = 0; i < GP; i++) cp[i] = ldg128_stream(cprev + (size_t)i * cstride + idx);
+                for (int i = 0; i < GP; i++) cp[i] = ldg128_stream(cprev + (size_t)i * cstride + idx);
 #pragma unroll
-                    for (int j = 0; j < GN; j++) cn[j] = ldg128_stream(cnext + (size_t)j * cstride + idx);
+                for (int j = 0; j < GN; j++) cn[j] = ldg128_stream(cnext + (size_t)j * cstride + idx);
 #pragma unroll
-                    for (int i = 0; i < GP; i++)
+                for (int i = 0; i < GP; i++)
 #pragma unroll
-                        for (int a = 0; a < 4; a++) r.a[a] = cfms(s_dw[i][a][g], cp[i], r.a[a]);
-                    if (GP > 0) store_m22(R + idx * 4, r);
+                    for (int a = 0; a < 4; a++) r.a[a] = cfms(s_dp[i][a][g], cp[i], r.a[a]);
+                if (GP > 0) store_m22(R + idx * 4, r);
 #pragma unroll
-                    for (int j = 0; j < GN; j++)
+                for (int j = 0; j < GN; j++)
 #pragma unroll
-                        for (int a = 0; a < 4; a++) S[j][a] = cfmac(r.a[a], cn[j], S[j][a]);
-                    rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
-                } else {
-                    cplx rl = ld_c(R + idx * 4 + l);                     // r_l
-#pragma unroll
-                    for (int i = 0; i < GP; i++) cp[i] = ldg128_stream(cprev + (size_t)i * cstride + idx * 4 + l);
-#pragma unroll
-                    for (int j = 0; j < GN; j++) cn[j] = ldg128_stream(cnext + (size_t)j * cstride + idx * 4 + l);
-                    if (GP > 0) {
-                        // column l of the write-back: v[a] = sum_i dW_i[a][l] c_i[l]; row l of the total to lane l
-                        cplx v[4];
-#pragma unroll
-                        for (int a = 0; a < 4; a++) v[a] = mk(0.0, 0.0);
-#pragma unroll
-                        for (int i = 0; i < GP; i++)
-#pragma unroll
-                            for (int a = 0; a < 4; a++) v[a] = cfma(s_dw[i][g][4 * a + l], cp[i], v[a]);
-                        const cplx w = quad_reduce_scatter(qmask, l, v);
-                        rl = mk(rl.re - w.re, rl.im - w.im);
-                        st_c(R + idx * 4 + l, rl);
-                    }
-                    if (GN > 0) {
-                        cplx r[4];
-                        quad_gather(qmask, tid & 31, rl, r);
-#pragma unroll
-                        for (int j = 0; j < GN; j++)
-#pragma unroll
-                            for (int a = 0; a < 4; a++) S[j][a] = cfmac(r[a], cn[j], S[j][a]);
-                    }
-                    rr = cabs2(rl, rr);
-                }
+                    for (int a = 0; a < 4; a++) S[j][a] = cfmac(r.a[a], cn[j], S[j][a]);
+                rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
             }
         }
     }
@@ -176,73 +98,53 @@ wbgroup_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sa
         const size_t bb = b < B ? (size_t)b : 0;
 #pragma unroll
         for (int j = 0; j < GN; j++) {
-            double* rec = SrcG + ((size_t)j * B + bb) * NSRC;
+            double* rec = SrcG + ((size_t)j * B + bb) * NSRC_SCALAR;
 #pragma unroll
             for (int a = 0; a < 4; a++) {
-                const double re = lanes_sum(S[j][a].re, FP, LPS), im = lanes_sum(S[j][a].im, FP, LPS);
-                if (writer) {
-                    const int e = SCALAR ? a : 4 * a + l;
-                    rec[2 * e] = re;
-                    rec[2 * e + 1] = im;
-                }
+                const double re = lanes_sum(S[j][a].re, FP), im = lanes_sum(S[j][a].im, FP);
+                if (writer) { rec[2 * a] = re; rec[2 * a + 1] = im; }
             }
         }
-        rr = lanes_sum(rr, FP * LPS, 1);
-        if (writer && l == 0) {
+        rr = lanes_sum(rr, FP);
+        if (writer) {
 #pragma unroll
             for (int j = 0; j < GN; j++) {
-                double* rec = SrcG + ((size_t)j * B + bb) * NSRC;
-                rec[NSRC - 2] = rr;        // meaningful for j = 0; groupfix rewrites it for the later clusters
-                rec[NSRC - 1] = 0.0;
+                double* rec = SrcG + ((size_t)j * B + bb) * NSRC_SCALAR;
+                rec[NSRC_SCALAR - 2] = rr;        // meaningful for j = 0; groupfix rewrites it for the later clusters
+                rec[NSRC_SCALAR - 1] = 0.0;
             }
         }
     }
 }
 
-// ---- Scc_i and X_ij (i < j) of the GN clusters kn0.. of a group -------------------------------------------------------
-// 2x2: lane l owns column l, X_ij[a][l] = sum c_i[a] conj(c_j[l]); the rows c_i[a] come from the quad by an all-gather.
-template <bool SCALAR, int GN>
-__global__ void __launch_bounds__(WG_THREADS, SCALAR ? 4 : 2)
-xgram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, size_t cstride, int kn0,
-             double* __restrict__ Scc, double* __restrict__ Xg) {
-    constexpr int NR = SCALAR ? 1 : 4;
-    constexpr int LPS = SCALAR ? 1 : 4;
-    constexpr int SPC = WG_THREADS / LPS;
+// ---- scalar coherencies: s2_i = sum |c_i|^2 and x_ij = sum c_i conj(c_j) (i < j) of the GN clusters kn0.. -------------
+template <int GN>
+__global__ void __launch_bounds__(WG_THREADS, 4)
+xgram_scalar_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, size_t cstride, int kn0,
+                    double* __restrict__ Scc, double* __restrict__ Xg) {
     constexpr int NP = GN * (GN + 1) / 2;                // pairs i <= j
     const int tid = threadIdx.x;
-    const int l = SCALAR ? 0 : (tid & 3), s = tid / LPS;
-    const int BL = SPC / FP;
-    const int g = s / FP, fl = s - g * FP;
+    const int BL = WG_THREADS / FP;
+    const int g = tid / FP, fl = tid - g * FP;
     const int64_t b = (int64_t)blockIdx.x * BL + g;
-    cplx X[NP][NR];
+    cplx X[NP];
 #pragma unroll
-    for (int n = 0; n < NP; n++)
-#pragma unroll
-        for (int a = 0; a < NR; a++) X[n][a] = mk(0.0, 0.0);
-
+    for (int n = 0; n < NP; n++) X[n] = mk(0.0, 0.0);
     if (b < B) {
         const sagecal_c128* cb = coh + (size_t)kn0 * cstride;
         const size_t step = (size_t)B * F;
-        const unsigned qmask = SCALAR ? 0u : (0xFu << ((tid & 31) & ~3));
         for (int f = fl; f < F; f += FP) {
             size_t idx = (size_t)b * F + f;
 #pragma unroll 1
             for (int t = 0; t < T; t++, idx += step) {
                 cplx c[GN];
 #pragma unroll
-                for (int i = 0; i < GN; i++) c[i] = ldg128_stream(cb + (size_t)i * cstride + idx * LPS + l);
-                if (!SCALAR && t + 2 < T && l < GN) prefetch_l2(cb + (size_t)l * cstride + (idx + 2 * step) * 4);
+                for (int i = 0; i < GN; i++) c[i] = ldg128_stream(cb + (size_t)i * cstride + idx);
                 int n = 0;
 #pragma unroll
-                for (int i = 0; i < GN; i++) {
-                    cplx ci[4];
-                    if (SCALAR) ci[0] = c[i];
-                    else quad_gather(qmask, tid & 31, c[i], ci);
+                for (int i = 0; i < GN; i++)
 #pragma unroll
-                    for (int j = i; j < GN; j++, n++)
-#pragma unroll
-                        for (int a = 0; a < NR; a++) X[n][a] = cfmac(ci[a], c[j], X[n][a]);
-                }
+                    for (int j = i; j < GN; j++, n++) X[n] = cfmac(c[i], c[j], X[n]);
             }
         }
     }
@@ -250,38 +152,212 @@ xgram_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ c
     const size_t bb = b < B ? (size_t)b : 0;
     int n = 0;
 #pragma unroll
-    for (int i = 0; i < GN; i++) {
+    for (int i = 0; i < GN; i++)
 #pragma unroll
         for (int j = i; j < GN; j++, n++) {
-            double re[NR], im[NR];
-#pragma unroll
-            for (int a = 0; a < NR; a++) { re[a] = lanes_sum(X[n][a].re, FP, LPS); im[a] = lanes_sum(X[n][a].im, FP, LPS); }
+            const double re = lanes_sum(X[n].re, FP), im = lanes_sum(X[n].im, FP);
             if (!writer) continue;
-            if (i == j) {
-                double* o = Scc + ((size_t)(kn0 + i) * B + bb) * (SCALAR ? NSCC_SCALAR : NSCC_FULL);
-                if (SCALAR) o[0] = re[0];
-                else {
-                    // packed Hermitian: diagonal [l], then the upper pairs (a < l, l) in the order of compress.cuh
+            if (i == j) Scc[((size_t)(kn0 + i) * B + bb) * NSCC_SCALAR] = re;
+            else {
+                double* o = Xg + ((size_t)grp_pair(i, j) * B + bb) * NX_SCALAR;
+                o[0] = re;
+                o[1] = im;
+            }
+        }
+}
+
+// ---- 2x2 coherencies on the FP64 tensor cores (DMMA m8n8k4) ----------------------------------------------------------
+// The statistics are the one dense contraction of this path: per baseline Src_j = R^T conj(C_j) is a (4 x TF)(TF x 4)
+// complex product, TF = T*F samples.  In real form a sample is 8 doubles (position g = 2a + ri), and
+//   stats     : D_j[g][n] += sum_k r'[sample k][g] * c_j[sample k][n]          (8 x 8 += (8 x 4)(4 x 8), k = 4 samples)
+//   write-back: r'[g][sample n] = r[g][sample n] + sum_k (-W_i)[g][k] c_i[sample n][k]   (k = 8 positions, two k-steps;
+//               W_i = real 8 x 8 form of dW_i, constant per baseline: 2 registers per lane and cluster)
+// One warp owns one baseline and walks its TF samples 8 at a time.  The fragment layouts line up so that nothing is
+// shuffled: the write-back's D fragment (row g, samples 2j and 2j+1, j = lane & 3) IS the A fragment of the statistics
+// if k-step s takes sample 2j + s, and the B fragments are 8-byte loads straight from global memory (a warp reads the 512
+// contiguous bytes of 8 samples in two instructions).  Per 8 samples and group: 18 loads, 2 stores, 16 DMMA -- against
+// ~370 instructions in the DFMA form; accumulators 2 doubles per lane and cluster.  Src = (rr + ii) + i (ir - ri) is
+// combined once per baseline with the partner lane (lane ^ 4) that holds the other real/imaginary row.
+__device__ __forceinline__ void dmma(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+__device__ __forceinline__ double ldg64_stream(const double* p) {
+    double r;
+    asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(r) : "l"(p));
+    return r;
+}
+__device__ __forceinline__ double ld64(const double* p) {
+    double r;
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(r) : "l"(p) : "memory");
+    return r;
+}
+__device__ __forceinline__ void st64(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
+
+constexpr int MMA_WARPS = 8;
+// index (in samples) of sample m = t*F + f of baseline b, or -1 past the end
+template <bool F8>
+__device__ __forceinline__ int64_t sample_index(int m, int TF, int F, int64_t B, int64_t b) {
+    if (m >= TF) return -1;
+    if (F8) return ((int64_t)(m >> 3) * B + b) * 8 + (m & 7);
+    const int t = m / F;
+    return ((int64_t)t * B + b) * F + (m - t * F);
+}
+
+template <int GP, int GN, bool F8>
+__global__ void __launch_bounds__(32 * MMA_WARPS)
+wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagecal_c128* __restrict__ coh_,
+                   size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev,
+                   const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG) {
+    constexpr int GPn = GP > 0 ? GP : 1, GNn = GN > 0 ? GN : 1;
+    const int lane = threadIdx.x & 31;
+    const int64_t b = (int64_t)blockIdx.x * MMA_WARPS + (threadIdx.x >> 5);
+    if (b >= B) return;                                   // whole warps leave together
+    const int g = lane >> 2, j = lane & 3;
+    double* R = reinterpret_cast<double*>(R_);
+    const double* cprev = reinterpret_cast<const double*>(coh_ + (size_t)kp0 * cstride);
+    const double* cnext = reinterpret_cast<const double*>(coh_ + (size_t)kn0 * cstride);
+    const size_t cs = cstride * 2;                        // doubles per cluster
+
+    double Aw[GPn][2];                                    // A fragments of -W_i: row g, column 4s + j
+    if (GP > 0) {
+        int p, q;
+        bl_stations(N, b, p, q);
+        const int a = g >> 1, ri = g & 1;
 #pragma unroll
-                    for (int a = 0; a < NR; a++) {
-                        if (a == l) o[l] = re[a];
-                        else if (a < l) {
-                            const int pr = a * 4 - a * (a + 1) / 2 + (l - a - 1);
-                            o[4 + 2 * pr] = re[a];
-                            o[5 + 2 * pr] = im[a];
-                        }
-                    }
-                }
-            } else {
-                double* o = Xg + ((size_t)grp_pair(i, j) * B + bb) * (SCALAR ? NX_SCALAR : NX_FULL);
-                if (SCALAR) { o[0] = re[0]; o[1] = im[0]; }
-                else {
+        for (int i = 0; i < GP; i++) {
 #pragma unroll
-                    for (int a = 0; a < NR; a++) { o[2 * (4 * a + l)] = re[a]; o[2 * (4 * a + l) + 1] = im[a]; }
-                }
+            for (int s = 0; s < 2; s++) {
+                const int kk = 4 * s + j, c = kk >> 1, ri2 = kk & 1;
+                const cplx w = dW_entry(J0prev + (size_t)i * N * 4, jones + (size_t)(kp0 + i) * N * 4, p, q, a, c);
+                // (w c).re = w.re c.re - w.im c.im,  (w c).im = w.im c.re + w.re c.im
+                Aw[i][s] = -(ri == ri2 ? w.re : (ri ? w.im : -w.im));
             }
         }
     }
+    double D[GNn][2];
+#pragma unroll
+    for (int jn = 0; jn < GNn; jn++) D[jn][0] = D[jn][1] = 0.0;
+    double rr = 0.0;
+
+    const int TF = T * F;
+#pragma unroll 1
+    for (int m0 = 0; m0 < TF; m0 += 8) {
+        const int64_t in = sample_index<F8>(m0 + g, TF, F, B, b);             // sample n = g (B fragments of the write-back)
+        const int64_t i0 = sample_index<F8>(m0 + 2 * j, TF, F, B, b);         // samples 2j, 2j + 1 (C / D / A fragments)
+        const int64_t i1 = sample_index<F8>(m0 + 2 * j + 1, TF, F, B, b);
+        double c0 = i0 >= 0 ? ld64(R + i0 * 8 + g) : 0.0;
+        double c1 = i1 >= 0 ? ld64(R + i1 * 8 + g) : 0.0;
+        double bp[GPn][2], bn[GNn][2];
+#pragma unroll
+        for (int i = 0; i < GP; i++) {
+            bp[i][0] = in >= 0 ? ldg64_stream(cprev + i * cs + in * 8 + j) : 0.0;
+            bp[i][1] = in >= 0 ? ldg64_stream(cprev + i * cs + in * 8 + 4 + j) : 0.0;
+        }
+#pragma unroll
+        for (int jn = 0; jn < GN; jn++) {
+            bn[jn][0] = i0 >= 0 ? ldg64_stream(cnext + jn * cs + i0 * 8 + g) : 0.0;
+            bn[jn][1] = i1 >= 0 ? ldg64_stream(cnext + jn * cs + i1 * 8 + g) : 0.0;
+        }
+        if (GP > 0) {
+#pragma unroll
+            for (int i = 0; i < GP; i++) {
+                dmma(c0, c1, Aw[i][0], bp[i][0]);
+                dmma(c0, c1, Aw[i][1], bp[i][1]);
+            }
+            if (i0 >= 0) st64(R + i0 * 8 + g, c0);
+            if (i1 >= 0) st64(R + i1 * 8 + g, c1);
+        }
+#pragma unroll
+        for (int jn = 0; jn < GN; jn++) {
+            dmma(D[jn][0], D[jn][1], c0, bn[jn][0]);
+            dmma(D[jn][0], D[jn][1], c1, bn[jn][1]);
+        }
+        rr = fma(c0, c0, fma(c1, c1, rr));
+    }
+    if (GN > 0) {
+        const int a = g >> 1, ri = g & 1;
+#pragma unroll
+        for (int jn = 0; jn < GN; jn++) {
+            const double p0 = __shfl_xor_sync(0xffffffffu, D[jn][0], 4), p1 = __shfl_xor_sync(0xffffffffu, D[jn][1], 4);
+            if (ri == 0) {
+                double* rec = SrcG + ((size_t)jn * B + b) * NSRC_FULL + 2 * (4 * a + j);
+                rec[0] = D[jn][0] + p1;
+                rec[1] = p0 - D[jn][1];
+            }
+        }
+        for (int o = 16; o > 0; o >>= 1) rr += __shfl_xor_sync(0xffffffffu, rr, o);
+        if (lane == 0) {
+#pragma unroll
+            for (int jn = 0; jn < GN; jn++) {
+                double* rec = SrcG + ((size_t)jn * B + b) * NSRC_FULL;
+                rec[NSRC_FULL - 2] = rr;
+                rec[NSRC_FULL - 1] = 0.0;
+            }
+        }
+    }
+}
+
+// X_ij[a][c] = sum c_i[a] conj(c_j[c]) (i < j) and Scc_i: the same contraction with both operands coherencies; one
+// loaded fragment (position lane >> 2 of sample 2 (lane & 3) + s) serves as A for its cluster's rows and as B for its
+// columns.
+template <int GN, bool F8>
+__global__ void __launch_bounds__(32 * MMA_WARPS)
+xgram_mma_kernel(int T, int F, int64_t B, const sagecal_c128* __restrict__ coh_, size_t cstride, int kn0,
+                 double* __restrict__ Scc, double* __restrict__ Xg) {
+    constexpr int NP = GN * (GN + 1) / 2;
+    const int lane = threadIdx.x & 31;
+    const int64_t b = (int64_t)blockIdx.x * MMA_WARPS + (threadIdx.x >> 5);
+    if (b >= B) return;
+    const int g = lane >> 2, j = lane & 3;
+    const double* cb = reinterpret_cast<const double*>(coh_ + (size_t)kn0 * cstride);
+    const size_t cs = cstride * 2;
+    double D[NP][2];
+#pragma unroll
+    for (int n = 0; n < NP; n++) D[n][0] = D[n][1] = 0.0;
+    const int TF = T * F;
+#pragma unroll 1
+    for (int m0 = 0; m0 < TF; m0 += 8) {
+        const int64_t i0 = sample_index<F8>(m0 + 2 * j, TF, F, B, b);
+        const int64_t i1 = sample_index<F8>(m0 + 2 * j + 1, TF, F, B, b);
+        double f[GN][2];
+#pragma unroll
+        for (int i = 0; i < GN; i++) {
+            f[i][0] = i0 >= 0 ? ldg64_stream(cb + i * cs + i0 * 8 + g) : 0.0;
+            f[i][1] = i1 >= 0 ? ldg64_stream(cb + i * cs + i1 * 8 + g) : 0.0;
+        }
+        int n = 0;
+#pragma unroll
+        for (int i = 0; i < GN; i++)
+#pragma unroll
+            for (int jj = i; jj < GN; jj++, n++) {
+                dmma(D[n][0], D[n][1], f[i][0], f[jj][0]);
+                dmma(D[n][0], D[n][1], f[i][1], f[jj][1]);
+            }
+    }
+    const int a = g >> 1, ri = g & 1, c = j;
+    int n = 0;
+#pragma unroll
+    for (int i = 0; i < GN; i++)
+#pragma unroll
+        for (int jj = i; jj < GN; jj++, n++) {
+            const double p0 = __shfl_xor_sync(0xffffffffu, D[n][0], 4), p1 = __shfl_xor_sync(0xffffffffu, D[n][1], 4);
+            if (ri != 0) continue;
+            const double re = D[n][0] + p1, im = p0 - D[n][1];
+            if (i == jj) {
+                double* o = Scc + ((size_t)(kn0 + i) * B + b) * NSCC_FULL;
+                if (c == a) o[a] = re;
+                else if (a < c) {
+                    const int pr = a * 4 - a * (a + 1) / 2 + (c - a - 1);
+                    o[4 + 2 * pr] = re;
+                    o[5 + 2 * pr] = im;
+                }
+            } else {
+                double* o = Xg + ((size_t)grp_pair(i, jj) * B + b) * NX_FULL + 2 * (4 * a + c);
+                o[0] = re;
+                o[1] = im;
+            }
+        }
 }
 
 // 4 lanes per baseline, lane a owns row a of dW_i (dP_i[a] in scalar form).
@@ -345,11 +421,19 @@ groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict_
             if (live) { sj[2 * a] = r.re; sj[2 * a + 1] = r.im; }
         } else {
 #pragma unroll
-            for (int c = 0; c < 4; c++) {
-                cplx r = mk(sj[2 * (4 * a + c)], sj[2 * (4 * a + c) + 1]);
+            // 16-byte accesses: records are 16-byte aligned (272 B and 256 B strides)
+            const double2* x2 = reinterpret_cast<const double2*>(x);
+            double2* sj2 = reinterpret_cast<double2*>(sj);
+            cplx xe[16];
 #pragma unroll
-                for (int e = 0; e < 4; e++) r = cfms(dw[e], mk(x[2 * (4 * e + c)], x[2 * (4 * e + c) + 1]), r);
-                if (live) { sj[2 * (4 * a + c)] = r.re; sj[2 * (4 * a + c) + 1] = r.im; }
+            for (int e = 0; e < 16; e++) { const double2 v = __ldg(x2 + e); xe[e] = mk(v.x, v.y); }
+#pragma unroll
+            for (int c = 0; c < 4; c++) {
+                const double2 v = sj2[4 * a + c];
+                cplx r = mk(v.x, v.y);
+#pragma unroll
+                for (int e = 0; e < 4; e++) r = cfms(dw[e], xe[4 * e + c], r);
+                if (live) sj2[4 * a + c] = make_double2(r.re, r.im);
             }
         }
     }
@@ -361,15 +445,33 @@ template <bool SCALAR, int GP>
 static void launch_wbgroup_gn(int gn, unsigned grid, cudaStream_t st, int N, int T, int F, int FP, int64_t B,
                               sagecal_c128* R, const sagecal_c128* coh, size_t cstride, int kp0,
                               const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, double* SrcG) {
-#define SGC_WG(GN_) wbgroup_kernel<SCALAR, GP, GN_><<<grid, WG_THREADS, 0, st>>>(N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
-    switch (gn) {
-        case 0: if (GP > 0) SGC_WG(0); break;
-        case 1: SGC_WG(1); break;
-        case 2: SGC_WG(2); break;
-        case 3: SGC_WG(3); break;
-        default: SGC_WG(4); break;
-    }
+    if (SCALAR) {
+#define SGC_WG(GN_) wbgroup_scalar_kernel<GP, GN_><<<grid, WG_THREADS, 0, st>>>(N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
+        switch (gn) {
+            case 0: if (GP > 0) SGC_WG(0); break;
+            case 1: SGC_WG(1); break;
+            case 2: SGC_WG(2); break;
+            case 3: SGC_WG(3); break;
+            default: SGC_WG(4); break;
+        }
 #undef SGC_WG
+        return;
+    }
+    // 2x2 coherencies: tensor-core form, one warp per baseline
+    const unsigned mgrid = (unsigned)((B + MMA_WARPS - 1) / MMA_WARPS);
+#define SGC_WM(GN_)                                                                                                          \
+    do {                                                                                                                     \
+        if (F == 8) wbgroup_mma_kernel<GP, GN_, true><<<mgrid, 32 * MMA_WARPS, 0, st>>>(N, T, F, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG); \
+        else wbgroup_mma_kernel<GP, GN_, false><<<mgrid, 32 * MMA_WARPS, 0, st>>>(N, T, F, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG);     \
+    } while (0)
+    switch (gn) {
+        case 0: if (GP > 0) SGC_WM(0); break;
+        case 1: SGC_WM(1); break;
+        case 2: SGC_WM(2); break;
+        case 3: SGC_WM(3); break;
+        default: SGC_WM(4); break;
+    }
+#undef SGC_WM
 }
 
 template <bool SCALAR>
@@ -377,7 +479,7 @@ static int launch_wbgroup(int N, int T, int F, sagecal_c128* R, const sagecal_c1
                           const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn, double* SrcG,
                           cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = SCALAR ? stat_group(F) : group_fp(F), BL = (SCALAR ? WG_THREADS : WG_THREADS / 4) / FP;
+    const int FP = stat_group(F), BL = WG_THREADS / FP;   // scalar form; the tensor-core form sizes its own grid
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_WBSTAT, st);
 #define SGC_GP(GP_) launch_wbgroup_gn<SCALAR, GP_>(gn, grid, st, N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
@@ -408,10 +510,15 @@ template <bool SCALAR>
 static int launch_xgram(int N, int T, int F, const sagecal_c128* coh, size_t cstride, int kn0, int gn, double* Scc,
                         double* Xg, cudaStream_t st) {
     const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = SCALAR ? stat_group(F) : group_fp(F), BL = (SCALAR ? WG_THREADS : WG_THREADS / 4) / FP;
+    const int FP = stat_group(F), BL = WG_THREADS / FP;   // scalar form; the tensor-core form sizes its own grid
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_XGRAM, st);
-#define SGC_XG(GN_) xgram_kernel<SCALAR, GN_><<<grid, WG_THREADS, 0, st>>>(T, F, FP, B, coh, cstride, kn0, Scc, Xg)
+#define SGC_XG(GN_)                                                                                                          \
+    do {                                                                                                                     \
+        if (SCALAR) xgram_scalar_kernel<GN_><<<grid, WG_THREADS, 0, st>>>(T, F, FP, B, coh, cstride, kn0, Scc, Xg);            \
+        else if (F == 8) xgram_mma_kernel<GN_, true><<<(unsigned)((B + MMA_WARPS - 1) / MMA_WARPS), 32 * MMA_WARPS, 0, st>>>(T, F, B, coh, cstride, kn0, Scc, Xg); \
+        else xgram_mma_kernel<GN_, false><<<(unsigned)((B + MMA_WARPS - 1) / MMA_WARPS), 32 * MMA_WARPS, 0, st>>>(T, F, B, coh, cstride, kn0, Scc, Xg);          \
+    } while (0)
     switch (gn) {
         case 1: SGC_XG(1); break;
         case 2: SGC_XG(2); break;

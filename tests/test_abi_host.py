@@ -50,8 +50,7 @@ def test_argument_validation_needs_no_device(lib):
     assert lib.sagecal_lm_cost_grad_jtj(4, 1, 1, z, 0, z, z, z, z, z, z, 0, z) == -1      # NULL pointers
     assert lib.sagecal_corrupt_subtract(4, 1, 1, 1, 7, z, z, z, -1.0, z, z, z) == -1      # bad coh_format
     assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, 0, z, z, z, 0, z) == -1
-    # lm_mode GROUPED (3) does not re-centre: n_lm > SAGECAL_LM_RECENTRE is refused; lm_mode 4 does not exist
-    assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 11, 1e-3, 3, z, z, z, 0, z) == -4
+    # lm_mode 4 does not exist
     assert lib.sagecal_sage_calibrate(4, 1, 1, 1, z, 0, z, z, z, 1, 1, 1e-3, 4, z, z, z, 0, z) == -1
     fr = (ctypes.c_double * 1)(150e6)
     off = (ctypes.c_int * 2)(0, 1)

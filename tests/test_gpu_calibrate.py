@@ -11,12 +11,12 @@ from tests.helpers import rel_l2, rel_max
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-8
-MODES = ["compressed", "direct", "grouped"]      # lm_mode of sagecal_sage_calibrate: all follow the oracle's trajectory
+MODES = ["compressed", "direct", "percluster"]      # lm_mode of sagecal_sage_calibrate: all follow the oracle's trajectory
 
 
 def _mode(name):
     import paper_1910_13908_b200 as sg
-    return {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "grouped": sg.LM_GROUPED}[name]
+    return {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "percluster": sg.LM_PERCLUSTER}[name]
 
 
 def _run_both(p, n_em, n_lm, coh_format=None, polarised=False, mode="compressed"):
@@ -69,7 +69,7 @@ def test_calibrate_polarised_small(cuda_device, mode):
     _compare(want, got)
 
 
-@pytest.mark.parametrize("mode", ["compressed", "grouped"])
+@pytest.mark.parametrize("mode", ["compressed", "percluster"])
 @pytest.mark.parametrize("shape", [(37, 3, 3), (33, 2, 5), (70, 2, 8), (6, 2, 40)])
 def test_calibrate_compressed_ragged_shapes(cuda_device, shape, mode):
     """Compressed mode on shapes that leave ragged tiles everywhere: N not a multiple of the 16 x 32 station tile,
@@ -90,7 +90,7 @@ def test_calibrate_grouped_ragged_groups(cuda_device, K, scalar):
     import paper_1910_13908_b200 as sg
     p = make_problem(12, 3, 3, K, 3, seed=500 + K, sigma=0.05, layout="disc:5000", field_deg=4.0, patch_deg=0.5,
                      polarised=not scalar)
-    want, got, _, _ = _run_both(p, 2, 4, coh_format=sg.COH_SCALAR if scalar else sg.COH_FULL, mode="grouped")
+    want, got, _, _ = _run_both(p, 2, 4, coh_format=sg.COH_SCALAR if scalar else sg.COH_FULL, mode="compressed")
     _compare(want, got)
 
 
@@ -128,7 +128,7 @@ def test_calibrate_modes_agree_to_rounding(cuda_device):
     coh_d = gpu_predict(p)
     V = gpu_simulate(p, coh_d)
     out = [sg.sage_calibrate(p.N, p.T, p.F, V, coh_d, dev(p.jones_init()), 2, 6, p.tau, lm_mode=m)
-           for m in (sg.LM_COMPRESSED, sg.LM_GROUPED, sg.LM_DIRECT)]
+           for m in (sg.LM_COMPRESSED, sg.LM_PERCLUSTER, sg.LM_DIRECT)]
     a, c, b = [{k: host(v) for k, v in o.items()} for o in out]
     for x in (a, c):
         assert np.max(np.abs(x["cost_per_cluster"] - b["cost_per_cluster"]) / b["cost_per_cluster"]) < 1e-11
@@ -136,7 +136,7 @@ def test_calibrate_modes_agree_to_rounding(cuda_device):
         assert rel_l2(x["residual"], b["residual"]) < 1e-11
 
 
-@pytest.mark.parametrize("mode", ["compressed", "direct"])     # grouped does not re-centre: n_lm <= 10 only
+@pytest.mark.parametrize("mode", MODES)
 def test_calibrate_noiseless_recovery_on_gpu(cuda_device, mode):
     """P10 on the CUDA path: noiseless single-cluster data, the cost falls below 1e-20 relative and the true Jones
     are recovered up to a unitary matrix.  60 trial steps of one M-step; compressed mode re-centres its statistics
