@@ -332,8 +332,8 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                 double* Xgrp = w.cw.Xg + (size_t)(k0 / GRP) * xgroup;
                 sagecal_c128* J0cur = w.cw.J0G + (size_t)par * GRP * N * 4;
                 const sagecal_c128* J0prev = w.cw.J0G + (size_t)(par ^ 1) * GRP * N * 4;
-                if (em == 0 && (rc = enqueue_xgram(N, T, F, coh_format, coh, cstride, k0, gn, w.cw.Scc, Xgrp, st))) return rc;
-                if ((rc = enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, k0, gn, w.cw.SrcG, st))) return rc;
+                if ((rc = enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, k0, gn, w.cw.SrcG,
+                                          em == 0 ? w.cw.Scc : nullptr, Xgrp, st))) return rc;
                 for (int j = 0; j < gn; j++, it++) {
                     const int k = k0 + j;
                     sagecal_c128* Jk = jones + (size_t)k * N * 4;
@@ -350,7 +350,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
         }
         // last write-back: the group solved last
         const sagecal_c128* J0prev = w.cw.J0G + (size_t)(par ^ 1) * GRP * N * 4;
-        return enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, 0, 0, w.cw.SrcG, st);
+        return enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, 0, 0, w.cw.SrcG, nullptr, nullptr, st);
     }
 
     // cluster by cluster: SAGECAL_LM_PERCLUSTER, SAGECAL_LM_FULLGN, and compressed M-steps longer than one chunk

@@ -113,13 +113,12 @@ __host__ __device__ constexpr int nxg(bool scalar) { return scalar ? NX_SCALAR :
 __host__ __device__ constexpr int grp_pair(int i, int j) { return i * GRP - i * (i + 1) / 2 + (j - i - 1); }   // i < j
 inline int ngroups(int K) { return (K + GRP - 1) / GRP; }
 
-// R -= sum_{i<gp} dW_i c_{kp0+i}, then Src of the new R against c_{kn0+j}, j < gn, into SrcG[j] (srr into SrcG[0] only)
+// R -= sum_{i<gp} dW_i c_{kp0+i}, then Src of the new R against c_{kn0+j}, j < gn, into SrcG[j] (srr into SrcG[0] only).
+// Scc != NULL (first EM iteration): also Scc of clusters kn0..kn0+gn-1 (into Scc + k*nscc*B) and the cross grams of
+// their pairs (into Xgroup) -- fused into the same kernel for 2x2 coherencies, a kernel of its own for scalar ones.
 int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
                     int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
-                    double* SrcG, cudaStream_t st);
-// Scc of clusters kn0..kn0+gn-1 (into Scc + k*nscc*B) and the cross grams of their pairs (into Xgroup)
-int enqueue_xgram(int N, int T, int F, int coh_format, const sagecal_c128* coh, size_t cstride, int kn0, int gn,
-                  double* Scc, double* Xgroup, cudaStream_t st);
+                    double* SrcG, double* Scc, double* Xgroup, cudaStream_t st);
 // cluster i of the group has been solved (J0_i -> J_i): Src_j -= dW_i X_ij for i < j < gn, srr_{i+1} = cost per
 // baseline after cluster i's update
 int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i, const sagecal_c128* J_i,

@@ -194,7 +194,7 @@ __device__ __forceinline__ double ld64(const double* p) {
 }
 __device__ __forceinline__ void st64(double* p, double v) { asm volatile("st.global.f64 [%0], %1;" ::"l"(p), "d"(v) : "memory"); }
 
-constexpr int MMA_WARPS = 8;
+constexpr int MMA_WARPS = 4;
 // index (in samples) of sample m = t*F + f of baseline b, or -1 past the end
 template <bool F8>
 __device__ __forceinline__ int64_t sample_index(int m, int TF, int F, int64_t B, int64_t b) {
@@ -204,11 +204,16 @@ __device__ __forceinline__ int64_t sample_index(int m, int TF, int F, int64_t B,
     return ((int64_t)t * B + b) * F + (m - t * F);
 }
 
-template <int GP, int GN, bool F8>
-__global__ void __launch_bounds__(32 * MMA_WARPS)
+// GRAM (first EM iteration): also X_ij[a][c] = sum c_i[a] conj(c_j[c]) (i < j) and Scc_i of the next group -- the same
+// contraction with both operands coherencies.  The B fragments of the statistics (position lane >> 2 of sample
+// 2 (lane & 3) + s) serve as A for their cluster's rows and as B for its columns, so the cross grams cost no load at
+// all, only GN (GN + 1) more DMMA per 8 samples.
+template <int GP, int GN, bool F8, bool GRAM>
+__global__ void __launch_bounds__(32 * MMA_WARPS, GRAM ? 4 : 5)
 wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagecal_c128* __restrict__ coh_,
                    size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev,
-                   const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG) {
+                   const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG,
+                   double* __restrict__ Scc, double* __restrict__ Xg) {
     constexpr int GPn = GP > 0 ? GP : 1, GNn = GN > 0 ? GN : 1;
     const int lane = threadIdx.x & 31;
     const int64_t b = (int64_t)blockIdx.x * MMA_WARPS + (threadIdx.x >> 5);
@@ -239,6 +244,10 @@ wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagec
 #pragma unroll
     for (int jn = 0; jn < GNn; jn++) D[jn][0] = D[jn][1] = 0.0;
     double rr = 0.0;
+    constexpr int NP = GRAM ? GNn * (GNn + 1) / 2 : 1;
+    double X[NP][2];
+#pragma unroll
+    for (int n = 0; n < NP; n++) X[n][0] = X[n][1] = 0.0;
 
     const int TF = T * F;
 #pragma unroll 1
@@ -274,6 +283,42 @@ wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagec
             dmma(D[jn][0], D[jn][1], c1, bn[jn][1]);
         }
         rr = fma(c0, c0, fma(c1, c1, rr));
+        if (GRAM) {
+            int n = 0;
+#pragma unroll
+            for (int i = 0; i < GN; i++)
+#pragma unroll
+                for (int jj = i; jj < GN; jj++, n++) {
+                    dmma(X[n][0], X[n][1], bn[i][0], bn[jj][0]);
+                    dmma(X[n][0], X[n][1], bn[i][1], bn[jj][1]);
+                }
+        }
+    }
+    if (GRAM) {
+        const int a = g >> 1, ri = g & 1, c = j;
+        int n = 0;
+#pragma unroll
+        for (int i = 0; i < GN; i++)
+#pragma unroll
+            for (int jj = i; jj < GN; jj++, n++) {
+                const double p0 = __shfl_xor_sync(0xffffffffu, X[n][0], 4), p1 = __shfl_xor_sync(0xffffffffu, X[n][1], 4);
+                if (ri != 0) continue;
+                const double re = X[n][0] + p1, im = p0 - X[n][1];
+                if (i == jj) {
+                    // packed Hermitian Scc: diagonal [a], then the upper pairs (a < c) in the order of compress.cuh
+                    double* o = Scc + ((size_t)(kn0 + i) * B + b) * NSCC_FULL;
+                    if (c == a) o[a] = re;
+                    else if (a < c) {
+                        const int pr = a * 4 - a * (a + 1) / 2 + (c - a - 1);
+                        o[4 + 2 * pr] = re;
+                        o[5 + 2 * pr] = im;
+                    }
+                } else {
+                    double* o = Xg + ((size_t)grp_pair(i, jj) * B + b) * NX_FULL + 2 * (4 * a + c);
+                    o[0] = re;
+                    o[1] = im;
+                }
+            }
     }
     if (GN > 0) {
         const int a = g >> 1, ri = g & 1;
@@ -296,68 +341,6 @@ wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagec
             }
         }
     }
-}
-
-// X_ij[a][c] = sum c_i[a] conj(c_j[c]) (i < j) and Scc_i: the same contraction with both operands coherencies; one
-// loaded fragment (position lane >> 2 of sample 2 (lane & 3) + s) serves as A for its cluster's rows and as B for its
-// columns.
-template <int GN, bool F8>
-__global__ void __launch_bounds__(32 * MMA_WARPS)
-xgram_mma_kernel(int T, int F, int64_t B, const sagecal_c128* __restrict__ coh_, size_t cstride, int kn0,
-                 double* __restrict__ Scc, double* __restrict__ Xg) {
-    constexpr int NP = GN * (GN + 1) / 2;
-    const int lane = threadIdx.x & 31;
-    const int64_t b = (int64_t)blockIdx.x * MMA_WARPS + (threadIdx.x >> 5);
-    if (b >= B) return;
-    const int g = lane >> 2, j = lane & 3;
-    const double* cb = reinterpret_cast<const double*>(coh_ + (size_t)kn0 * cstride);
-    const size_t cs = cstride * 2;
-    double D[NP][2];
-#pragma unroll
-    for (int n = 0; n < NP; n++) D[n][0] = D[n][1] = 0.0;
-    const int TF = T * F;
-#pragma unroll 1
-    for (int m0 = 0; m0 < TF; m0 += 8) {
-        const int64_t i0 = sample_index<F8>(m0 + 2 * j, TF, F, B, b);
-        const int64_t i1 = sample_index<F8>(m0 + 2 * j + 1, TF, F, B, b);
-        double f[GN][2];
-#pragma unroll
-        for (int i = 0; i < GN; i++) {
-            f[i][0] = i0 >= 0 ? ldg64_stream(cb + i * cs + i0 * 8 + g) : 0.0;
-            f[i][1] = i1 >= 0 ? ldg64_stream(cb + i * cs + i1 * 8 + g) : 0.0;
-        }
-        int n = 0;
-#pragma unroll
-        for (int i = 0; i < GN; i++)
-#pragma unroll
-            for (int jj = i; jj < GN; jj++, n++) {
-                dmma(D[n][0], D[n][1], f[i][0], f[jj][0]);
-                dmma(D[n][0], D[n][1], f[i][1], f[jj][1]);
-            }
-    }
-    const int a = g >> 1, ri = g & 1, c = j;
-    int n = 0;
-#pragma unroll
-    for (int i = 0; i < GN; i++)
-#pragma unroll
-        for (int jj = i; jj < GN; jj++, n++) {
-            const double p0 = __shfl_xor_sync(0xffffffffu, D[n][0], 4), p1 = __shfl_xor_sync(0xffffffffu, D[n][1], 4);
-            if (ri != 0) continue;
-            const double re = D[n][0] + p1, im = p0 - D[n][1];
-            if (i == jj) {
-                double* o = Scc + ((size_t)(kn0 + i) * B + b) * NSCC_FULL;
-                if (c == a) o[a] = re;
-                else if (a < c) {
-                    const int pr = a * 4 - a * (a + 1) / 2 + (c - a - 1);
-                    o[4 + 2 * pr] = re;
-                    o[5 + 2 * pr] = im;
-                }
-            } else {
-                double* o = Xg + ((size_t)grp_pair(i, jj) * B + b) * NX_FULL + 2 * (4 * a + c);
-                o[0] = re;
-                o[1] = im;
-            }
-        }
 }
 
 // 4 lanes per baseline, lane a owns row a of dW_i (dP_i[a] in scalar form).
@@ -441,85 +424,69 @@ groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict_
 
 
 // ---- host side ----------------------------------------------------------------------------------------------------
-template <bool SCALAR, int GP>
-static void launch_wbgroup_gn(int gn, unsigned grid, cudaStream_t st, int N, int T, int F, int FP, int64_t B,
-                              sagecal_c128* R, const sagecal_c128* coh, size_t cstride, int kp0,
-                              const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, double* SrcG) {
-    if (SCALAR) {
-#define SGC_WG(GN_) wbgroup_scalar_kernel<GP, GN_><<<grid, WG_THREADS, 0, st>>>(N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
-        switch (gn) {
-            case 0: if (GP > 0) SGC_WG(0); break;
-            case 1: SGC_WG(1); break;
-            case 2: SGC_WG(2); break;
-            case 3: SGC_WG(3); break;
-            default: SGC_WG(4); break;
-        }
-#undef SGC_WG
-        return;
-    }
-    // 2x2 coherencies: tensor-core form, one warp per baseline
-    const unsigned mgrid = (unsigned)((B + MMA_WARPS - 1) / MMA_WARPS);
-#define SGC_WM(GN_)                                                                                                          \
-    do {                                                                                                                     \
-        if (F == 8) wbgroup_mma_kernel<GP, GN_, true><<<mgrid, 32 * MMA_WARPS, 0, st>>>(N, T, F, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG); \
-        else wbgroup_mma_kernel<GP, GN_, false><<<mgrid, 32 * MMA_WARPS, 0, st>>>(N, T, F, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG);     \
-    } while (0)
-    switch (gn) {
-        case 0: if (GP > 0) SGC_WM(0); break;
-        case 1: SGC_WM(1); break;
-        case 2: SGC_WM(2); break;
-        case 3: SGC_WM(3); break;
-        default: SGC_WM(4); break;
-    }
+struct WbgArgs {
+    int N, T, F;
+    sagecal_c128* R;
+    const sagecal_c128* coh;
+    size_t cstride;
+    int kp0, gp;
+    const sagecal_c128 *J0prev, *jones;
+    int kn0, gn;
+    double *SrcG, *Scc, *Xg;
+};
+
+template <int GP, int GN>
+static void launch_wbgroup_scalar(const WbgArgs& a, cudaStream_t st) {
+    const int64_t B = (int64_t)a.N * (a.N - 1) / 2;
+    const int FP = stat_group(a.F), BL = WG_THREADS / FP;
+    const unsigned grid = (unsigned)((B + BL - 1) / BL);
+    wbgroup_scalar_kernel<GP, GN><<<grid, WG_THREADS, 0, st>>>(a.N, a.T, a.F, FP, B, a.R, a.coh, a.cstride, a.kp0, a.J0prev, a.jones, a.kn0, a.SrcG);
+}
+template <int GP, int GN>
+static void launch_wbgroup_mma(const WbgArgs& a, cudaStream_t st) {
+    const int64_t B = (int64_t)a.N * (a.N - 1) / 2;
+    const unsigned grid = (unsigned)((B + MMA_WARPS - 1) / MMA_WARPS);
+    const bool gram = a.Scc != nullptr && GN > 0;
+#define SGC_WM(F8_, GR_) wbgroup_mma_kernel<GP, GN, F8_, GR_><<<grid, 32 * MMA_WARPS, 0, st>>>(a.N, a.T, a.F, B, a.R, a.coh, a.cstride, a.kp0, a.J0prev, a.jones, a.kn0, a.SrcG, a.Scc, a.Xg)
+    if (a.F == 8) { if (gram) SGC_WM(true, true); else SGC_WM(true, false); }
+    else { if (gram) SGC_WM(false, true); else SGC_WM(false, false); }
 #undef SGC_WM
 }
-
-template <bool SCALAR>
-static int launch_wbgroup(int N, int T, int F, sagecal_c128* R, const sagecal_c128* coh, size_t cstride, int kp0, int gp,
-                          const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn, double* SrcG,
-                          cudaStream_t st) {
-    const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = stat_group(F), BL = WG_THREADS / FP;   // scalar form; the tensor-core form sizes its own grid
-    const unsigned grid = (unsigned)((B + BL - 1) / BL);
-    LaunchScope ls(KK_WBSTAT, st);
-#define SGC_GP(GP_) launch_wbgroup_gn<SCALAR, GP_>(gn, grid, st, N, T, F, FP, B, R, coh, cstride, kp0, J0prev, jones, kn0, SrcG)
-    switch (gp) {
-        case 0: SGC_GP(0); break;
-        case 1: SGC_GP(1); break;
-        case 2: SGC_GP(2); break;
-        case 3: SGC_GP(3); break;
-        default: SGC_GP(4); break;
+template <bool SCALAR, int GP, int GN>
+static void launch_wbgroup_one(const WbgArgs& a, cudaStream_t st) {
+    if (GP == 0 && GN == 0) return;
+    if (SCALAR) launch_wbgroup_scalar<GP, GN>(a, st);
+    else launch_wbgroup_mma<GP, GN>(a, st);
+}
+template <bool SCALAR, int GP>
+static void launch_wbgroup_gn(const WbgArgs& a, cudaStream_t st) {
+    switch (a.gn) {
+        case 0: launch_wbgroup_one<SCALAR, GP, 0>(a, st); break;
+        case 1: launch_wbgroup_one<SCALAR, GP, 1>(a, st); break;
+        case 2: launch_wbgroup_one<SCALAR, GP, 2>(a, st); break;
+        case 3: launch_wbgroup_one<SCALAR, GP, 3>(a, st); break;
+        default: launch_wbgroup_one<SCALAR, GP, 4>(a, st); break;
     }
-#undef SGC_GP
-    SGC_LAUNCH_CHECK();
-    return SAGECAL_OK;
 }
-
-int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
-                    int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
-                    double* SrcG, cudaStream_t st) {
-    static_assert(GRP == 4, "the dispatch tables above are written for GRP = 4");
-    if (gp <= 0 && gn <= 0) return SAGECAL_OK;
-    if (gp > GRP || gn > GRP) return SAGECAL_EINVAL;
-    return coh_format == SAGECAL_COH_SCALAR
-               ? launch_wbgroup<true>(N, T, F, R, coh, cstride, kp0, gp < 0 ? 0 : gp, J0prev, jones, kn0, gn < 0 ? 0 : gn, SrcG, st)
-               : launch_wbgroup<false>(N, T, F, R, coh, cstride, kp0, gp < 0 ? 0 : gp, J0prev, jones, kn0, gn < 0 ? 0 : gn, SrcG, st);
-}
-
 template <bool SCALAR>
-static int launch_xgram(int N, int T, int F, const sagecal_c128* coh, size_t cstride, int kn0, int gn, double* Scc,
-                        double* Xg, cudaStream_t st) {
-    const int64_t B = (int64_t)N * (N - 1) / 2;
-    const int FP = stat_group(F), BL = WG_THREADS / FP;   // scalar form; the tensor-core form sizes its own grid
+static void launch_wbgroup_gp(const WbgArgs& a, cudaStream_t st) {
+    switch (a.gp) {
+        case 0: launch_wbgroup_gn<SCALAR, 0>(a, st); break;
+        case 1: launch_wbgroup_gn<SCALAR, 1>(a, st); break;
+        case 2: launch_wbgroup_gn<SCALAR, 2>(a, st); break;
+        case 3: launch_wbgroup_gn<SCALAR, 3>(a, st); break;
+        default: launch_wbgroup_gn<SCALAR, 4>(a, st); break;
+    }
+}
+
+// scalar form: the cross grams are a kernel of their own (2x2 form: the GRAM arm of wbgroup_mma_kernel)
+static int launch_xgram_scalar(const WbgArgs& a, cudaStream_t st) {
+    const int64_t B = (int64_t)a.N * (a.N - 1) / 2;
+    const int FP = stat_group(a.F), BL = WG_THREADS / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
     LaunchScope ls(KK_XGRAM, st);
-#define SGC_XG(GN_)                                                                                                          \
-    do {                                                                                                                     \
-        if (SCALAR) xgram_scalar_kernel<GN_><<<grid, WG_THREADS, 0, st>>>(T, F, FP, B, coh, cstride, kn0, Scc, Xg);            \
-        else if (F == 8) xgram_mma_kernel<GN_, true><<<(unsigned)((B + MMA_WARPS - 1) / MMA_WARPS), 32 * MMA_WARPS, 0, st>>>(T, F, B, coh, cstride, kn0, Scc, Xg); \
-        else xgram_mma_kernel<GN_, false><<<(unsigned)((B + MMA_WARPS - 1) / MMA_WARPS), 32 * MMA_WARPS, 0, st>>>(T, F, B, coh, cstride, kn0, Scc, Xg);          \
-    } while (0)
-    switch (gn) {
+#define SGC_XG(GN_) xgram_scalar_kernel<GN_><<<grid, WG_THREADS, 0, st>>>(a.T, a.F, FP, B, a.coh, a.cstride, a.kn0, a.Scc, a.Xg)
+    switch (a.gn) {
         case 1: SGC_XG(1); break;
         case 2: SGC_XG(2); break;
         case 3: SGC_XG(3); break;
@@ -530,11 +497,25 @@ static int launch_xgram(int N, int T, int F, const sagecal_c128* coh, size_t cst
     return SAGECAL_OK;
 }
 
-int enqueue_xgram(int N, int T, int F, int coh_format, const sagecal_c128* coh, size_t cstride, int kn0, int gn,
-                  double* Scc, double* Xgroup, cudaStream_t st) {
-    if (gn < 1 || gn > GRP) return SAGECAL_EINVAL;
-    return coh_format == SAGECAL_COH_SCALAR ? launch_xgram<true>(N, T, F, coh, cstride, kn0, gn, Scc, Xgroup, st)
-                                            : launch_xgram<false>(N, T, F, coh, cstride, kn0, gn, Scc, Xgroup, st);
+int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
+                    int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
+                    double* SrcG, double* Scc, double* Xgroup, cudaStream_t st) {
+    static_assert(GRP == 4, "the dispatch tables above are written for GRP = 4");
+    if (gp < 0) gp = 0;
+    if (gn < 0) gn = 0;
+    if (gp == 0 && gn == 0) return SAGECAL_OK;
+    if (gp > GRP || gn > GRP) return SAGECAL_EINVAL;
+    const bool scalar = coh_format == SAGECAL_COH_SCALAR;
+    const WbgArgs a = {N, T, F, R, coh, cstride, kp0, gp, J0prev, jones, kn0, gn, SrcG, Scc, Xgroup};
+    if (scalar && Scc && gn > 0) {
+        const int rc = launch_xgram_scalar(a, st);
+        if (rc) return rc;
+    }
+    LaunchScope ls(KK_WBSTAT, st);
+    if (scalar) launch_wbgroup_gp<true>(a, st);
+    else launch_wbgroup_gp<false>(a, st);
+    SGC_LAUNCH_CHECK();
+    return SAGECAL_OK;
 }
 
 int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i, const sagecal_c128* J_i,
