@@ -384,8 +384,10 @@ def run_ours(args):
         pass_bytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
     peak, peak_src = load_peaks()
     achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
-    kname = "wbgroup" if uses_groups(args.lm, args.coh, p.n_lm) else top     # both are timed as kind "wbstat"
-    roofline = {"bound": "hbm", "kernel": kname + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    grouped = uses_groups(args.lm, args.coh, p.n_lm)                         # both are timed as kind "wbstat"
+    kname = "wbgroup" if grouped else top
+    kfull = ("wbgroup_mma" if args.coh == "full" else "wbgroup_scalar") if grouped else top
+    roofline = {"bound": "hbm", "kernel": kfull + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": load_traffic(args.coh, kname), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,
                 "share_of_step": prof[top]["ms"] / max(args.steps, 1) / ms_per_step}
