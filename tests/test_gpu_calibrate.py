@@ -298,3 +298,49 @@ def _run_both_nocheck(p, n_em, n_lm, fmt, mode):
     got = sg.sage_calibrate(p.N, p.T, p.F, dev(V), gpu_predict(p, fmt), dev(p.jones_init()), n_em, n_lm, p.tau,
                             coh_format=fmt, lm_mode=_mode(mode))
     return want, {k: (None if v is None else host(v)) for k, v in got.items()}, V, coh
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("scalar", [False, True])
+def test_calibrate_writes_nothing_outside_its_buffers(cuda_device, mode, scalar):
+    """Every buffer the call may write (residual, Jones, costs, trace, workspace of exactly sagecal_workspace_bytes)
+    sits between guard bands of a known byte pattern; ragged shape (N, T*F and K not multiples of any tile, warp or
+    group size).  The guards must come back untouched, the read-only inputs unchanged, and the result must still be
+    the oracle's."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, host
+    p = make_problem(13, 3, 3, 5, 3, seed=71, sigma=0.05, layout="disc:5000", field_deg=4.0, patch_deg=0.5,
+                     polarised=not scalar)
+    fmt = sg.COH_SCALAR if scalar else sg.COH_FULL
+    coh = oracle.predict(p)
+    V = oracle.simulate(p, coh)
+    want = oracle.sage(p.N, p.T, p.F, V, coh, p.jones_init(), 2, 4, p.tau)
+    G = 4096
+
+    def guarded(nbytes):
+        buf = torch.full((G + ((nbytes + 255) // 256) * 256 + G,), 0xA5, dtype=torch.uint8, device="cuda:0")
+        return buf, buf[G:G + nbytes]
+
+    def carve(arr_shape, dtype):
+        n = int(np.prod(arr_shape)) * torch.empty((), dtype=dtype).element_size()
+        buf, body = guarded(n)
+        return buf, body.view(dtype).view(*arr_shape)
+
+    wsb = sg.workspace_bytes(2, p.N, p.T, p.F, p.K)
+    ws_buf, ws = guarded(wsb)
+    res_buf, res = carve((p.rows, p.F, 4), torch.complex128)
+    j_buf, J = carve((p.K, p.N, 2, 2), torch.complex128)
+    J.copy_(dev(p.jones_init()))
+    coh_d, V_d = gpu_predict(p, fmt), dev(V)
+    coh0, V0 = coh_d.clone(), V_d.clone()
+    got = sg.sage_calibrate(p.N, p.T, p.F, V_d, coh_d, J, 2, 4, p.tau, coh_format=fmt, residual=res, workspace=ws,
+                            lm_mode=_mode(mode))
+    torch.cuda.synchronize()
+    for name, buf, n in (("workspace", ws_buf, wsb), ("residual", res_buf, res.numel() * 16), ("jones", j_buf, J.numel() * 16)):
+        body_end = G + n
+        assert bool((buf[:G] == 0xA5).all()), f"{name}: bytes before the buffer were written"
+        assert bool((buf[G + ((n + 255) // 256) * 256:] == 0xA5).all()), f"{name}: bytes after the buffer were written"
+        assert bool((buf[body_end:G + ((n + 255) // 256) * 256] == 0xA5).all()), f"{name}: padding after the buffer was written"
+    assert torch.equal(coh_d, coh0) and torch.equal(V_d, V0)
+    _compare(want, {k: (None if v is None else host(v)) for k, v in got.items()})
