@@ -344,3 +344,17 @@ def test_calibrate_writes_nothing_outside_its_buffers(cuda_device, mode, scalar)
         assert bool((buf[body_end:G + ((n + 255) // 256) * 256] == 0xA5).all()), f"{name}: padding after the buffer was written"
     assert torch.equal(coh_d, coh0) and torch.equal(V_d, V0)
     _compare(want, {k: (None if v is None else host(v)) for k, v in got.items()})
+
+
+@pytest.mark.parametrize("mode", MODES)
+@pytest.mark.parametrize("scalar", [False, True])
+@pytest.mark.parametrize("shape", [(2, 1, 1, 1), (3, 1, 2, 2), (4, 2, 1, 5), (2, 3, 3, 2)])
+def test_calibrate_smallest_shapes(cuda_device, shape, scalar, mode):
+    """The smallest problems there are: one baseline, one sample (a tensor-core chunk with 7 of 8 sample slots empty,
+    three of a CTA's four warps without a baseline), more clusters than stations."""
+    import paper_1910_13908_b200 as sg
+    N, T, F, K = shape
+    p = make_problem(N, T, F, K, 2, seed=900 + N + T, sigma=0.05, layout="disc:5000", field_deg=4.0,
+                     patch_deg=0.5 if K > 1 else None, polarised=not scalar)
+    want, got, _, _ = _run_both(p, 1, 3, coh_format=sg.COH_SCALAR if scalar else sg.COH_FULL, mode=mode)
+    _compare(want, got)
