@@ -299,6 +299,16 @@ int sagecal_debug_pass_cover(int nstations, int ntime, int nchan, int32_t* cover
  */
 int sagecal_debug_mstep_cover(int nstations, int32_t* cover, int64_t* info);
 
+/*
+ * Test hook, host only: replays the fragment addressing of the tensor-core statistics kernel (DESIGN.md §5.5 "cluster
+ * groups", 2x2 form): one warp per baseline walks its T*F samples 8 at a time; every lane touches one double of two
+ * samples as C/D/A fragment and two doubles of one sample as B fragment of the write-back.
+ * cover_cd, cover_b : host out [T*B*F*8] int32 each, zeroed by the caller: how often each double of each sample is
+ *                     addressed in either role; every entry must come back 1 (nothing missed, nothing twice).
+ * Returns 0, SAGECAL_EINVAL, or a positive bit mask (1/2: an address outside the array in either role).
+ */
+int sagecal_debug_mma_cover(int nstations, int ntime, int nchan, int32_t* cover_cd, int32_t* cover_b);
+
 #ifdef __cplusplus
 }
 #endif

@@ -197,7 +197,7 @@ __device__ __forceinline__ void st64(double* p, double v) { asm volatile("st.glo
 constexpr int MMA_WARPS = 4;
 // index (in samples) of sample m = t*F + f of baseline b, or -1 past the end
 template <bool F8>
-__device__ __forceinline__ int64_t sample_index(int m, int TF, int F, int64_t B, int64_t b) {
+__host__ __device__ __forceinline__ int64_t sample_index(int m, int TF, int F, int64_t B, int64_t b) {
     if (m >= TF) return -1;
     if (F8) return ((int64_t)(m >> 3) * B + b) * 8 + (m & 7);
     const int t = m / F;
@@ -531,3 +531,35 @@ int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i
 }
 
 }  // namespace sgc
+
+using namespace sgc;
+
+// Host-side replay of the tensor-core kernel's fragment addressing (CPU tests, no device needed): for every baseline,
+// 8-sample chunk and lane, the doubles the lane touches as C/D/A fragment (and as B fragment of the next group's
+// coherencies) -- position lane >> 2 of samples 2 (lane & 3) and 2 (lane & 3) + 1 -- and as B fragment of the previous
+// group's coherencies -- positions (lane & 3) and 4 + (lane & 3) of sample lane >> 2.
+extern "C" int sagecal_debug_mma_cover(int N, int T, int F, int32_t* cover_cd, int32_t* cover_b) {
+    if (N < 2 || T < 1 || F < 1 || !cover_cd || !cover_b) return SAGECAL_EINVAL;
+    const int64_t B = (int64_t)N * (N - 1) / 2, nd = (int64_t)T * B * F * 8;
+    const int TF = T * F;
+    int bad = 0;
+    for (int64_t b = 0; b < B; b++)
+        for (int m0 = 0; m0 < TF; m0 += 8)
+            for (int lane = 0; lane < 32; lane++) {
+                const int g = lane >> 2, j = lane & 3;
+                const int64_t in = F == 8 ? sample_index<true>(m0 + g, TF, F, B, b) : sample_index<false>(m0 + g, TF, F, B, b);
+                const int64_t i0 = F == 8 ? sample_index<true>(m0 + 2 * j, TF, F, B, b) : sample_index<false>(m0 + 2 * j, TF, F, B, b);
+                const int64_t i1 = F == 8 ? sample_index<true>(m0 + 2 * j + 1, TF, F, B, b) : sample_index<false>(m0 + 2 * j + 1, TF, F, B, b);
+                for (int64_t i : {i0, i1}) {
+                    if (i < 0) continue;
+                    if (i * 8 + g >= nd) { bad |= 1; continue; }
+                    cover_cd[i * 8 + g]++;
+                }
+                if (in >= 0) {
+                    if (in * 8 + 4 + j >= nd) { bad |= 2; continue; }
+                    cover_b[in * 8 + j]++;
+                    cover_b[in * 8 + 4 + j]++;
+                }
+            }
+    return bad;
+}

@@ -92,6 +92,18 @@ def test_mstep_tiling_covers_every_baseline_once(lib, N):
         assert PB == 16 and ntiles == 272
 
 
+@pytest.mark.parametrize("N,T,F", [(2, 1, 1), (3, 1, 8), (5, 3, 3), (9, 2, 5), (6, 20, 8), (7, 2, 40), (12, 7, 1), (4, 3, 16)])
+def test_tensor_core_fragment_addressing_touches_every_double_once(lib, N, T, F):
+    """wbgroup_mma_kernel: over a baseline's 8-sample chunks the 32 lanes address every double of every sample exactly
+    once as C/D/A fragment and exactly once as B fragment of the write-back (F = 8 takes the shift/mask fast path)."""
+    lib.sagecal_debug_mma_cover.restype = ctypes.c_int
+    lib.sagecal_debug_mma_cover.argtypes = [ctypes.c_int] * 3 + [ctypes.c_void_p] * 2
+    nd = T * (N * (N - 1) // 2) * F * 8
+    cd, cb = np.zeros(nd, np.int32), np.zeros(nd, np.int32)
+    assert lib.sagecal_debug_mma_cover(N, T, F, cd.ctypes.data, cb.ctypes.data) == 0
+    assert np.all(cd == 1) and np.all(cb == 1)
+
+
 def test_calibrate_workspace_covers_compressed_statistics(lib):
     """SAGECAL_WS_CALIBRATE holds the per-baseline statistics of the compressed mode: K x 16 doubles (gram of the
     coherencies) + 33 doubles per baseline, on top of the direct pass's partial sums; plus, for the cluster-group
