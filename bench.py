@@ -95,12 +95,11 @@ def expected_launches(K: int, n_em: int, n_lm: int, trace: bool, lm: str = "dire
         return head + n_em * K * (2 + 3 * (n_lm + 1))
     chunks = max(1, -(-n_lm // LM_RECENTRE))
     if uses_groups(lm, coh, n_lm):
-        # cluster groups: per group one write-back+statistics kernel per EM iteration (for scalar coherencies one
-        # cross-gram kernel per group in the first EM iteration as well; for 2x2 ones the cross grams are taken by the
-        # statistics kernel itself), per cluster one M-step kernel, per cluster but the last of its group one
-        # correction kernel; one final write-back
+        # cluster groups: per group one write-back+statistics kernel per EM iteration (in the first one it also takes
+        # the cross grams of the group's coherencies), per cluster one M-step kernel, per cluster but the last of its
+        # group one correction kernel; one final write-back
         gs = group_sizes(K)
-        return head + (len(gs) if coh == "scalar" else 0) + n_em * (len(gs) + K + sum(g - 1 for g in gs)) + 1
+        return head + n_em * (len(gs) + K + sum(g - 1 for g in gs)) + 1
     if lm == "fullgn":
         # per chunk: statistics kernel, evaluation (3 kernels) + control + commit, then per trial step
         # damping/rhs, step, evaluation (3), control, commit (cuSOLVER's own kernels are not counted)

@@ -22,7 +22,7 @@ inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 int num_sms();  // SM count of the current device (cached)
 
 // ---- launch accounting and optional per-kernel CUDA-event timing (profile.cu; sagecal_profile_* in the ABI) ----
-enum KernelKind { KK_PREP = 0, KK_PREDICT, KK_CORRUPT, KK_PASS, KK_REDUCE, KK_LMSTEP, KK_NORM, KK_WBSTAT, KK_MSTEP, KK_FULLGN, KK_ROWS, KK_XGRAM, KK_GFIX, KK_COUNT };
+enum KernelKind { KK_PREP = 0, KK_PREDICT, KK_CORRUPT, KK_PASS, KK_REDUCE, KK_LMSTEP, KK_NORM, KK_WBSTAT, KK_MSTEP, KK_FULLGN, KK_ROWS, KK_GFIX, KK_COUNT };
 // Brackets one kernel launch: counts it, and when timing of its kind is enabled records an event pair on `st`.
 struct LaunchScope {
     int kind;

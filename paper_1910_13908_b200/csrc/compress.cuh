@@ -115,7 +115,7 @@ inline int ngroups(int K) { return (K + GRP - 1) / GRP; }
 
 // R -= sum_{i<gp} dW_i c_{kp0+i}, then Src of the new R against c_{kn0+j}, j < gn, into SrcG[j] (srr into SrcG[0] only).
 // Scc != NULL (first EM iteration): also Scc of clusters kn0..kn0+gn-1 (into Scc + k*nscc*B) and the cross grams of
-// their pairs (into Xgroup) -- fused into the same kernel for 2x2 coherencies, a kernel of its own for scalar ones.
+// their pairs (into Xgroup), by the GRAM arm of the same kernel.
 int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
                     int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
                     double* SrcG, double* Scc, double* Xgroup, cudaStream_t st);

@@ -49,7 +49,7 @@ extern "C" long long sagecal_launch_count(void) {
 extern "C" int sagecal_kernel_kinds(void) { return KK_COUNT; }
 
 extern "C" const char* sagecal_kernel_kind_name(int kind) {
-    static const char* names[KK_COUNT] = {"predict_prep", "predict", "corrupt", "lm_pass", "lm_reduce", "lm_step", "norm2", "wbstat", "mstep", "fullgn", "rows", "xgram", "groupfix"};
+    static const char* names[KK_COUNT] = {"predict_prep", "predict", "corrupt", "lm_pass", "lm_reduce", "lm_step", "norm2", "wbstat", "mstep", "fullgn", "rows", "groupfix"};
     return kind >= 0 && kind < KK_COUNT ? names[kind] : "?";
 }
 

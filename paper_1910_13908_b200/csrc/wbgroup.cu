@@ -8,14 +8,15 @@
 //   groupfix:  after cluster i of the group is solved, for the later j of the group
 //              Src_j <- Src_j - dW_i X_ij,   X_ij = sum_tf c_i c_j^H   (r' = r - dW_i c_i  =>  r' c_j^H = r c_j^H - dW_i c_i c_j^H)
 //              srr_{i+1} = srr_i - Re tr(dW_i^H (Src_i + Sec_i))         (the cost per baseline after i's update)
-//   xgram:     X_ij and Scc_i of a group, once per interval (they depend on the coherencies only)
+//   cross grams X_ij and Scc_i of a group: once per interval (they depend on the coherencies only), by the GRAM arm of
+//              wbgroup in the first EM iteration
 //
 // (2 + 2 GRP) x 64 B per sample and group instead of GRP x 256 B: 160 B instead of 256 B per cluster at GRP = 4
 // (2x2 coherencies; 64 B instead of 160 B with scalar coherencies).  Nothing is approximated; the LM trajectory is the
 // same to rounding.
 //
 // Scalar coherencies: plain FP64 FMAs, one thread per (baseline, channel) sample as in wbstat.cu (8 accumulators per
-// cluster); sums over the channel lanes of a baseline by warp shuffles.  2x2 coherencies: the FP64 tensor cores, one
+// cluster; the cross grams ride along in the first EM iteration); sums over the channel lanes of a baseline by warp shuffles.  2x2 coherencies: the FP64 tensor cores, one
 // warp per baseline (below).  Fixed order, no atomics.
 #include "compress.cuh"
 
@@ -30,11 +31,14 @@ __device__ __forceinline__ double lanes_sum(double v, int n) {
 }
 
 // ---- scalar coherencies: write-back of the previous group + statistics of the next group ------------------------------
-template <int GP, int GN>
+// GRAM (first EM iteration): also s2_i = sum |c_i|^2 and x_ij = sum c_i conj(c_j) (i < j) of the next group, from the
+// coherency samples the statistics load anyway.
+template <int GP, int GN, bool GRAM>
 __global__ void __launch_bounds__(WG_THREADS, 3)
 wbgroup_scalar_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, const sagecal_c128* __restrict__ coh,
                       size_t cstride, int kp0, const sagecal_c128* __restrict__ J0prev,
-                      const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG) {
+                      const sagecal_c128* __restrict__ jones, int kn0, double* __restrict__ SrcG,
+                      double* __restrict__ Scc, double* __restrict__ Xg) {
     constexpr int GPn = GP > 0 ? GP : 1, GNn = GN > 0 ? GN : 1;
     __shared__ cplx s_dp[GPn][4][WG_THREADS];            // dP_i[a] per [cluster][entry][baseline of this CTA]
     const int tid = threadIdx.x;
@@ -64,6 +68,10 @@ wbgroup_scalar_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, c
 #pragma unroll
         for (int a = 0; a < 4; a++) S[j][a] = mk(0.0, 0.0);
     double rr = 0.0;
+    constexpr int NP = GRAM ? GNn * (GNn + 1) / 2 : 1;
+    cplx X[NP];
+#pragma unroll
+    for (int n = 0; n < NP; n++) X[n] = mk(0.0, 0.0);
 
     if (b < B) {
         const sagecal_c128* cprev = coh + (size_t)kp0 * cstride;
@@ -90,8 +98,33 @@ wbgroup_scalar_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, c
 #pragma unroll
                     for (int a = 0; a < 4; a++) S[j][a] = cfmac(r.a[a], cn[j], S[j][a]);
                 rr = cabs2(r.a[3], cabs2(r.a[2], cabs2(r.a[1], cabs2(r.a[0], rr))));
+                if (GRAM) {
+                    int n = 0;
+#pragma unroll
+                    for (int i = 0; i < GN; i++)
+#pragma unroll
+                        for (int j = i; j < GN; j++, n++) X[n] = cfmac(cn[i], cn[j], X[n]);
+                }
             }
         }
+    }
+    if (GRAM) {
+        const bool writer = fl == 0 && b < B;
+        const size_t bb = b < B ? (size_t)b : 0;
+        int n = 0;
+#pragma unroll
+        for (int i = 0; i < GN; i++)
+#pragma unroll
+            for (int j = i; j < GN; j++, n++) {
+                const double re = lanes_sum(X[n].re, FP), im = lanes_sum(X[n].im, FP);
+                if (!writer) continue;
+                if (i == j) Scc[((size_t)(kn0 + i) * B + bb) * NSCC_SCALAR] = re;
+                else {
+                    double* o = Xg + ((size_t)grp_pair(i, j) * B + bb) * NX_SCALAR;
+                    o[0] = re;
+                    o[1] = im;
+                }
+            }
     }
     if (GN > 0) {
         const bool writer = fl == 0 && b < B;
@@ -115,55 +148,6 @@ wbgroup_scalar_kernel(int N, int T, int F, int FP, int64_t B, sagecal_c128* R, c
             }
         }
     }
-}
-
-// ---- scalar coherencies: s2_i = sum |c_i|^2 and x_ij = sum c_i conj(c_j) (i < j) of the GN clusters kn0.. -------------
-template <int GN>
-__global__ void __launch_bounds__(WG_THREADS, 4)
-xgram_scalar_kernel(int T, int F, int FP, int64_t B, const sagecal_c128* __restrict__ coh, size_t cstride, int kn0,
-                    double* __restrict__ Scc, double* __restrict__ Xg) {
-    constexpr int NP = GN * (GN + 1) / 2;                // pairs i <= j
-    const int tid = threadIdx.x;
-    const int BL = WG_THREADS / FP;
-    const int g = tid / FP, fl = tid - g * FP;
-    const int64_t b = (int64_t)blockIdx.x * BL + g;
-    cplx X[NP];
-#pragma unroll
-    for (int n = 0; n < NP; n++) X[n] = mk(0.0, 0.0);
-    if (b < B) {
-        const sagecal_c128* cb = coh + (size_t)kn0 * cstride;
-        const size_t step = (size_t)B * F;
-        for (int f = fl; f < F; f += FP) {
-            size_t idx = (size_t)b * F + f;
-#pragma unroll 1
-            for (int t = 0; t < T; t++, idx += step) {
-                cplx c[GN];
-#pragma unroll
-                for (int i = 0; i < GN; i++) c[i] = ldg128_stream(cb + (size_t)i * cstride + idx);
-                int n = 0;
-#pragma unroll
-                for (int i = 0; i < GN; i++)
-#pragma unroll
-                    for (int j = i; j < GN; j++, n++) X[n] = cfmac(c[i], c[j], X[n]);
-            }
-        }
-    }
-    const bool writer = fl == 0 && b < B;
-    const size_t bb = b < B ? (size_t)b : 0;
-    int n = 0;
-#pragma unroll
-    for (int i = 0; i < GN; i++)
-#pragma unroll
-        for (int j = i; j < GN; j++, n++) {
-            const double re = lanes_sum(X[n].re, FP), im = lanes_sum(X[n].im, FP);
-            if (!writer) continue;
-            if (i == j) Scc[((size_t)(kn0 + i) * B + bb) * NSCC_SCALAR] = re;
-            else {
-                double* o = Xg + ((size_t)grp_pair(i, j) * B + bb) * NX_SCALAR;
-                o[0] = re;
-                o[1] = im;
-            }
-        }
 }
 
 // ---- 2x2 coherencies on the FP64 tensor cores (DMMA m8n8k4) ----------------------------------------------------------
@@ -440,7 +424,10 @@ static void launch_wbgroup_scalar(const WbgArgs& a, cudaStream_t st) {
     const int64_t B = (int64_t)a.N * (a.N - 1) / 2;
     const int FP = stat_group(a.F), BL = WG_THREADS / FP;
     const unsigned grid = (unsigned)((B + BL - 1) / BL);
-    wbgroup_scalar_kernel<GP, GN><<<grid, WG_THREADS, 0, st>>>(a.N, a.T, a.F, FP, B, a.R, a.coh, a.cstride, a.kp0, a.J0prev, a.jones, a.kn0, a.SrcG);
+    if (a.Scc != nullptr && GN > 0)
+        wbgroup_scalar_kernel<GP, GN, true><<<grid, WG_THREADS, 0, st>>>(a.N, a.T, a.F, FP, B, a.R, a.coh, a.cstride, a.kp0, a.J0prev, a.jones, a.kn0, a.SrcG, a.Scc, a.Xg);
+    else
+        wbgroup_scalar_kernel<GP, GN, false><<<grid, WG_THREADS, 0, st>>>(a.N, a.T, a.F, FP, B, a.R, a.coh, a.cstride, a.kp0, a.J0prev, a.jones, a.kn0, a.SrcG, a.Scc, a.Xg);
 }
 template <int GP, int GN>
 static void launch_wbgroup_mma(const WbgArgs& a, cudaStream_t st) {
@@ -479,24 +466,6 @@ static void launch_wbgroup_gp(const WbgArgs& a, cudaStream_t st) {
     }
 }
 
-// scalar form: the cross grams are a kernel of their own (2x2 form: the GRAM arm of wbgroup_mma_kernel)
-static int launch_xgram_scalar(const WbgArgs& a, cudaStream_t st) {
-    const int64_t B = (int64_t)a.N * (a.N - 1) / 2;
-    const int FP = stat_group(a.F), BL = WG_THREADS / FP;
-    const unsigned grid = (unsigned)((B + BL - 1) / BL);
-    LaunchScope ls(KK_XGRAM, st);
-#define SGC_XG(GN_) xgram_scalar_kernel<GN_><<<grid, WG_THREADS, 0, st>>>(a.T, a.F, FP, B, a.coh, a.cstride, a.kn0, a.Scc, a.Xg)
-    switch (a.gn) {
-        case 1: SGC_XG(1); break;
-        case 2: SGC_XG(2); break;
-        case 3: SGC_XG(3); break;
-        default: SGC_XG(4); break;
-    }
-#undef SGC_XG
-    SGC_LAUNCH_CHECK();
-    return SAGECAL_OK;
-}
-
 int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
                     int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
                     double* SrcG, double* Scc, double* Xgroup, cudaStream_t st) {
@@ -507,10 +476,6 @@ int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const 
     if (gp > GRP || gn > GRP) return SAGECAL_EINVAL;
     const bool scalar = coh_format == SAGECAL_COH_SCALAR;
     const WbgArgs a = {N, T, F, R, coh, cstride, kp0, gp, J0prev, jones, kn0, gn, SrcG, Scc, Xgroup};
-    if (scalar && Scc && gn > 0) {
-        const int rc = launch_xgram_scalar(a, st);
-        if (rc) return rc;
-    }
     LaunchScope ls(KK_WBSTAT, st);
     if (scalar) launch_wbgroup_gp<true>(a, st);
     else launch_wbgroup_gp<false>(a, st);

@@ -22,9 +22,9 @@ def test_pass_and_launch_counts():
     # cluster by cluster: per (em,k) one write-back/statistics kernel + one cooperative M-step kernel, + last write-back
     assert bench.expected_launches(50, 3, 10, True, "percluster") == 5 + 150 * 2 + 1
     # compressed, cluster groups of 4 (13 groups at K=50, the last of 2): per EM iteration 13 write-back/statistics
-    # kernels + 50 M-step kernels + (12*3 + 1) correction kernels, + last write-back; scalar coherencies: + 13 cross-gram
-    # kernels (2x2: taken by the statistics kernel of the first EM iteration)
-    assert bench.expected_launches(50, 3, 10, True, "compressed", "scalar") == 5 + 13 + 3 * (13 + 50 + 37) + 1
+    # kernels (which take the cross grams as well in the first one) + 50 M-step kernels + (12*3 + 1) correction kernels,
+    # + last write-back
+    assert bench.expected_launches(50, 3, 10, True, "compressed", "scalar") == 5 + 3 * (13 + 50 + 37) + 1
     assert bench.expected_launches(50, 3, 10, True, "compressed", "full") == 5 + 3 * (13 + 50 + 37) + 1
     per = bench.wbgroup_bytes_per_sample(50, 3, "full")
     assert len(per) == 40 and per[0] == 64 + 4 * 64 and per[1] == 128 + 8 * 64 and per[-1] == 128 + 2 * 64
