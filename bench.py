@@ -385,7 +385,12 @@ def run_ours(args):
     achieved = pass_bytes / (pass_ms * 1e-3) / 1e9 if pass_ms > 0 else 0.0
     grouped = uses_groups(args.lm, args.coh, p.n_lm)                         # both are timed as kind "wbstat"
     kname = "wbgroup" if grouped else top
-    kfull = ("wbgroup_mma" if args.coh == "full" else "wbgroup_scalar") if grouped else top
+    if grouped:
+        kfull = "wbgroup_mma" if args.coh == "full" else "wbgroup_scalar"
+    elif top == "lm_pass":
+        kfull = "lm_pass_mma" if args.coh == "full" else "lm_pass_scalar"
+    else:
+        kfull = top
     roofline = {"bound": "hbm", "kernel": kfull + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": load_traffic(args.coh, kname), "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,

@@ -17,7 +17,7 @@ ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libsagecal_b200.so")
-SOURCES = ["predict.cu", "corrupt.cu", "lm_pass.cu", "calibrate.cu", "profile.cu", "wbstat.cu", "mstep.cu", "fullgn.cu", "rows.cu", "wbgroup.cu"]
+SOURCES = ["predict.cu", "corrupt.cu", "lm_pass.cu", "calibrate.cu", "profile.cu", "wbstat.cu", "mstep.cu", "fullgn.cu", "rows.cu", "wbgroup.cu", "lm_pass_mma.cu"]
 ARCH = ["-gencode", "arch=compute_100a,code=sm_100a"]
 
 

@@ -39,6 +39,8 @@ size_t pass_workspace_bytes(const PassGeom& g) {
     n += round_up(sizeof(double) * (size_t)g.U * PASS_WARPS * PASS_NV, 256);
     n += round_up(sizeof(double) * (size_t)g.U * PASS_WARPS, 256);
     n += round_up(sizeof(double) * (size_t)(g.nslots + g.ncols) * g.TQ * PASS_NV, 256);
+    n += round_up(sizeof(double) * (size_t)g.B * PASS_BREC, 256);
+    n += round_up(sizeof(double) * (size_t)g.N, 256) + 256;
     return n;
 }
 
@@ -47,7 +49,10 @@ PassWorkspace carve_pass_workspace(const PassGeom& g, void* ws) {
     char* p = (char*)ws;
     w.Ppart = (double*)p; p += round_up(sizeof(double) * (size_t)g.U * PASS_WARPS * PASS_NV, 256);
     w.Pcost = (double*)p; p += round_up(sizeof(double) * (size_t)g.U * PASS_WARPS, 256);
-    w.Qpart = (double*)p;
+    w.Qpart = (double*)p; p += round_up(sizeof(double) * (size_t)(g.nslots + g.ncols) * g.TQ * PASS_NV, 256);
+    w.Brec = (double*)p; p += round_up(sizeof(double) * (size_t)g.B * PASS_BREC, 256);
+    w.cost_st = (double*)p; p += round_up(sizeof(double) * (size_t)g.N, 256);
+    w.counter = (unsigned*)p;
     return w;
 }
 
@@ -75,38 +80,6 @@ __device__ __forceinline__ double warp_sum(double v) {
     return v;
 }
 
-// general 2x2 coherency: everything per sample (200 FP64 instructions)
-__device__ __forceinline__ void sample_full(const m22& X, const m22& C, const m22& Jp, const m22& Jq, Side& sp,
-                                            Side& sq, double& cost) {
-    m22 T1, A, E;
-    mm(Jp, C, T1);   // T1 = J_p C
-    mmh(C, Jq, A);   // A  = C J_q^H
-    // E = x - J_p A
-    E.a[0] = cfms(Jp.a[1], A.a[2], cfms(Jp.a[0], A.a[0], X.a[0]));
-    E.a[1] = cfms(Jp.a[1], A.a[3], cfms(Jp.a[0], A.a[1], X.a[1]));
-    E.a[2] = cfms(Jp.a[3], A.a[2], cfms(Jp.a[2], A.a[0], X.a[2]));
-    E.a[3] = cfms(Jp.a[3], A.a[3], cfms(Jp.a[2], A.a[1], X.a[3]));
-    cost = cabs2(E.a[3], cabs2(E.a[2], cabs2(E.a[1], cabs2(E.a[0], cost))));
-    // G_p += E A^H
-    sp.G[0] = cfmac(E.a[1], A.a[1], cfmac(E.a[0], A.a[0], sp.G[0]));
-    sp.G[1] = cfmac(E.a[1], A.a[3], cfmac(E.a[0], A.a[2], sp.G[1]));
-    sp.G[2] = cfmac(E.a[3], A.a[1], cfmac(E.a[2], A.a[0], sp.G[2]));
-    sp.G[3] = cfmac(E.a[3], A.a[3], cfmac(E.a[2], A.a[2], sp.G[3]));
-    // G_q += E^H T1
-    sq.G[0] = cfmaca(E.a[2], T1.a[2], cfmaca(E.a[0], T1.a[0], sq.G[0]));
-    sq.G[1] = cfmaca(E.a[2], T1.a[3], cfmaca(E.a[0], T1.a[1], sq.G[1]));
-    sq.G[2] = cfmaca(E.a[3], T1.a[2], cfmaca(E.a[1], T1.a[0], sq.G[2]));
-    sq.G[3] = cfmaca(E.a[3], T1.a[3], cfmaca(E.a[1], T1.a[1], sq.G[3]));
-    // M_p += A A^H (Hermitian)
-    sp.M00 = cabs2(A.a[1], cabs2(A.a[0], sp.M00));
-    sp.M11 = cabs2(A.a[3], cabs2(A.a[2], sp.M11));
-    sp.M01 = cfmac(A.a[1], A.a[3], cfmac(A.a[0], A.a[2], sp.M01));
-    // M_q += T1^H T1
-    sq.M00 = cabs2(T1.a[2], cabs2(T1.a[0], sq.M00));
-    sq.M11 = cabs2(T1.a[3], cabs2(T1.a[1], sq.M11));
-    sq.M01 = cfmaca(T1.a[2], T1.a[3], cfmaca(T1.a[0], T1.a[1], sq.M01));
-}
-
 // H = J^H J as (H00, H11, H01)
 __device__ __forceinline__ void gram(const m22& J, double& h00, double& h11, cplx& h01) {
     h00 = cabs2(J.a[2], cabs2(J.a[0], 0.0));
@@ -114,9 +87,9 @@ __device__ __forceinline__ void gram(const m22& J, double& h00, double& h11, cpl
     h01 = cfmaca(J.a[2], J.a[3], cfmaca(J.a[0], J.a[1], mk(0.0, 0.0)));
 }
 
-template <bool SCALAR>
+// Scalar coherencies (C = c I2).  General 2x2 coherencies take the tensor-core form in lm_pass_mma.cu.
 __global__ void __launch_bounds__(PASS_THREADS, 3)
-lm_pass_kernel(PassGeom g, const sagecal_c128* __restrict__ x, const sagecal_c128* __restrict__ coh,
+lm_pass_scalar_kernel(PassGeom g, const sagecal_c128* __restrict__ x, const sagecal_c128* __restrict__ coh,
                const sagecal_c128* __restrict__ jones, double* __restrict__ Ppart, double* __restrict__ Pcost,
                double* __restrict__ Qpart) {
     __shared__ double s_red[PASS_NV][PASS_THREADS];
@@ -161,12 +134,12 @@ lm_pass_kernel(PassGeom g, const sagecal_c128* __restrict__ x, const sagecal_c12
             sq.zero();
             q = TQ * c + ql;
             load_jones(jones + (size_t)min(q, N - 1) * 4, Jq);
-            if (SCALAR) gram(Jq, hq00, hq11, hq01);
+            gram(Jq, hq00, hq11, hq01);
         }
         if (p != cur_p) {
             cur_p = p;
             load_jones(jones + (size_t)p * 4, Jp);
-            if (SCALAR) gram(Jp, hp00, hp11, hp01);
+            gram(Jp, hp00, hp11, hp01);
         }
         const bool valid = thread_used && q > p && q < N;
         const int t0 = tc * g.tlen, t1 = min(g.T, t0 + g.tlen);
@@ -175,19 +148,7 @@ lm_pass_kernel(PassGeom g, const sagecal_c128* __restrict__ x, const sagecal_c12
         double cost = 0.0;
         if (valid) {
             const int64_t b = bl_index(N, p, q);
-            if (!SCALAR) {
-                for (int j = 0; j < g.nchunk; j++) {
-                    const int f = g.nchunk > 1 ? tid + j * PASS_THREADS : tid - ql * F;
-                    if (f >= F) break;
-                    for (int t = t0; t < t1; t++) {
-                        const size_t idx = ((size_t)t * g.B + b) * F + f;
-                        m22 X, C;
-                        load_m22_stream(x + idx * 4, X);
-                        load_m22_stream(coh + idx * 4, C);
-                        sample_full(X, C, Jp, Jq, sp, sq, cost);
-                    }
-                }
-            } else {
+            {
                 // C = c*I2: model = c (J_p J_q^H); S = sum conj(c) E; s2 = sum |c|^2
                 m22 P;
                 mmh(Jp, Jq, P);
@@ -308,12 +269,11 @@ lm_reduce_kernel(PassGeom g, const double* __restrict__ Ppart, const double* __r
 int enqueue_pass(const PassGeom& g, const PassWorkspace& w, const sagecal_c128* x, int coh_format,
                  const sagecal_c128* coh_k, const sagecal_c128* jones, double* cost, sagecal_c128* grad,
                  sagecal_c128* jtj, cudaStream_t st) {
+    // 2x2 coherencies: the tensor-core form (lm_pass_mma.cu); the kernel below then serves the scalar form
+    if (coh_format != SAGECAL_COH_SCALAR) return enqueue_pass_mma(g, w, x, coh_k, jones, cost, grad, jtj, st);
     {
         LaunchScope ls(KK_PASS, st);
-        if (coh_format == SAGECAL_COH_SCALAR)
-            lm_pass_kernel<true><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
-        else
-            lm_pass_kernel<false><<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
+        lm_pass_scalar_kernel<<<g.nslots, PASS_THREADS, 0, st>>>(g, x, coh_k, jones, w.Ppart, w.Pcost, w.Qpart);
         SGC_LAUNCH_CHECK();
     }
     {

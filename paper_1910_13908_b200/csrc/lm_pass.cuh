@@ -8,6 +8,7 @@ namespace sgc {
 constexpr int PASS_THREADS = 128;            // one thread per sample slot of a tile segment
 constexpr int PASS_WARPS = PASS_THREADS / 32;
 constexpr int PASS_NV = 12;                  // doubles per station side: G (4 complex) + M (M00, M11, Re M01, Im M01)
+constexpr int PASS_BREC = 26;                // tensor-core form: doubles per baseline record: G_p (8), G_q (8), M_p (4), M_q (4), cost, pad
 
 // The upper triangle of the N x N station grid is cut into column tiles of TQ stations (q) and single rows (p).
 // A "unit" is (column c, row p, time chunk tc): TQ*F samples per time slot, contiguous in memory at fixed t.
@@ -55,10 +56,14 @@ struct PassGeom {
 //   Ppart [U][PASS_WARPS][12]   per-unit, per-warp p-side sums (row station p)
 //   Pcost [U][PASS_WARPS]       per-unit, per-warp cost
 //   Qpart [nslots+ncols][TQ][12] per-(slot,column) q-side sums; record index = slot + column
+//   Brec  [B][PASS_BREC]        tensor-core form (2x2 coherencies, lm_pass_mma.cu): one record per baseline
 struct PassWorkspace {
     double* Ppart;
     double* Pcost;
     double* Qpart;
+    double* Brec;
+    double* cost_st;    // [N] tensor-core form: cost of each station's row-role records
+    unsigned* counter;  // ticket counter of the reduction's last-block step
 };
 
 PassGeom make_pass_geom(int N, int T, int F);
@@ -69,5 +74,9 @@ PassWorkspace carve_pass_workspace(const PassGeom& g, void* ws);
 int enqueue_pass(const PassGeom& g, const PassWorkspace& w, const sagecal_c128* x, int coh_format,
                  const sagecal_c128* coh_k, const sagecal_c128* jones, double* cost, sagecal_c128* grad,
                  sagecal_c128* jtj, cudaStream_t st);
+
+// 2x2 coherencies: the same sums on the FP64 tensor cores, one warp per baseline (lm_pass_mma.cu)
+int enqueue_pass_mma(const PassGeom& g, const PassWorkspace& w, const sagecal_c128* x, const sagecal_c128* coh_k,
+                     const sagecal_c128* jones, double* cost, sagecal_c128* grad, sagecal_c128* jtj, cudaStream_t st);
 
 }  // namespace sgc

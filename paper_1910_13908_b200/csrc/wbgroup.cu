@@ -387,7 +387,6 @@ groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict_
             const cplx r = cfms(dw[0], mk(x[0], x[1]), mk(sj[2 * a], sj[2 * a + 1]));
             if (live) { sj[2 * a] = r.re; sj[2 * a + 1] = r.im; }
         } else {
-#pragma unroll
             // 16-byte accesses: records are 16-byte aligned (272 B and 256 B strides)
             const double2* x2 = reinterpret_cast<const double2*>(x);
             double2* sj2 = reinterpret_cast<double2*>(sj);
