@@ -339,11 +339,12 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                     sagecal_c128* Jk = jones + (size_t)k * N * 4;
                     sagecal_c128* J0 = J0cur + (size_t)j * N * 4;
                     const double* Scc_k = w.cw.Scc + (size_t)k * nscc(scalar) * B;
+                    if (j > 0 && (rc = enqueue_groupfix(N, scalar, j, J0cur, jones + (size_t)k0 * N * 4,
+                                                         w.cw.Scc + (size_t)(k - 1) * nscc(scalar) * B, Xgrp, w.cw.SrcG, st))) return rc;
                     CompressWorkspace cwj = w.cw;
                     cwj.Src = w.cw.SrcG + (size_t)j * srec;
                     if ((rc = enqueue_mstep(N, scalar, cwj, Scc_k, J0, Jk, n_lm, true, tau, cost_per_cluster + k,
                                             cost_trace ? cost_trace + it : nullptr, st))) return rc;
-                    if ((rc = enqueue_groupfix(N, scalar, j, gn, J0, Jk, Scc_k, Xgrp, w.cw.SrcG, st))) return rc;
                 }
                 kp0 = k0; gp = gn; par ^= 1;
             }

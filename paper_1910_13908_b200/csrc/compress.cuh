@@ -119,10 +119,11 @@ inline int ngroups(int K) { return (K + GRP - 1) / GRP; }
 int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const sagecal_c128* coh, size_t cstride,
                     int kp0, int gp, const sagecal_c128* J0prev, const sagecal_c128* jones, int kn0, int gn,
                     double* SrcG, double* Scc, double* Xgroup, cudaStream_t st);
-// cluster i of the group has been solved (J0_i -> J_i): Src_j -= dW_i X_ij for i < j < gn, srr_{i+1} = cost per
-// baseline after cluster i's update
-int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i, const sagecal_c128* J_i,
-                     const double* Scc_i, const double* Xgroup, double* SrcG, cudaStream_t st);
+// right before cluster j >= 1 of the group is solved: Src_j -= sum_{i<j} dW_i X_ij and srr_j = cost per baseline after
+// cluster j-1's update.  J0g / Jg: centre and solved Jones of the group's clusters ([GRP][N][4], [>= j][N][4]);
+// Scc_prev: Scc of cluster j-1
+int enqueue_groupfix(int N, bool scalar, int j, const sagecal_c128* J0g, const sagecal_c128* Jg, const double* Scc_prev,
+                     const double* Xgroup, double* SrcG, cudaStream_t st);
 size_t compress_workspace_bytes(int N, int K, bool scalar);
 CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws);
 

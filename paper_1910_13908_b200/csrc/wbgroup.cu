@@ -5,9 +5,9 @@
 //
 //   wbgroup:   R <- R - sum_{i in previous group} dW_i c_i          (ONE read and ONE write of R per group)
 //              Src_j = sum_tf r c_j^H for every j in the next group, srr = sum_tf |r|^2
-//   groupfix:  after cluster i of the group is solved, for the later j of the group
-//              Src_j <- Src_j - dW_i X_ij,   X_ij = sum_tf c_i c_j^H   (r' = r - dW_i c_i  =>  r' c_j^H = r c_j^H - dW_i c_i c_j^H)
-//              srr_{i+1} = srr_i - Re tr(dW_i^H (Src_i + Sec_i))         (the cost per baseline after i's update)
+//   groupfix:  right before cluster j of the group is solved, with the clusters i < j of the group solved so far
+//              Src_j <- Src_j - sum_i dW_i X_ij,  X_ij = sum_tf c_i c_j^H  (r' = r - dW_i c_i  =>  r' c_j^H = r c_j^H - dW_i c_i c_j^H)
+//              srr_j = srr_{j-1} - Re tr(dW_{j-1}^H (Src_{j-1} + Sec_{j-1}))   (the cost per baseline after j-1's update)
 //   cross grams X_ij and Scc_i of a group: once per interval (they depend on the coherencies only), by the GRAM arm of
 //              wbgroup in the first EM iteration
 //
@@ -327,11 +327,14 @@ wbgroup_mma_kernel(int N, int T, int F, int64_t B, sagecal_c128* R_, const sagec
     }
 }
 
-// 4 lanes per baseline, lane a owns row a of dW_i (dP_i[a] in scalar form).
+// Right before cluster j >= 1 of a group is solved: Src_j -= sum_{i<j} dW_i X_ij (the clusters of the group solved so
+// far, each Src record read and written once) and srr_j = srr_{j-1} - Re tr(dW_{j-1}^H (Src_{j-1} + Sec_{j-1})), the
+// cost per baseline after cluster j-1's update.  4 lanes per baseline, lane a owns row a of dW_i (dP_i[a] in scalar
+// form).  J0g / Jg: centre and solved Jones of the group's clusters, [GRP][N][4] each.
 template <bool SCALAR>
 __global__ void __launch_bounds__(128)
-groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict__ J0, const sagecal_c128* __restrict__ J,
-                const double* __restrict__ Scc_i, const double* __restrict__ Xg, double* __restrict__ SrcG) {
+groupfix_kernel(int N, int64_t B, int j, const sagecal_c128* __restrict__ J0g, const sagecal_c128* __restrict__ Jg,
+                const double* __restrict__ Scc_prev, const double* __restrict__ Xg, double* __restrict__ SrcG) {
     constexpr int NSRC = SCALAR ? NSRC_SCALAR : NSRC_FULL;
     constexpr int NC = SCALAR ? 1 : 4;
     const int64_t gid = (int64_t)blockIdx.x * 128 + threadIdx.x;
@@ -341,20 +344,48 @@ groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict_
     const size_t bb = live ? (size_t)b : 0;
     int p, q;
     bl_stations(N, (int64_t)bb, p, q);
-    cplx dw[NC];
-#pragma unroll
-    for (int c = 0; c < NC; c++) dw[c] = SCALAR ? dP_entry(J0, J, p, q, a) : dW_entry(J0, J, p, q, a, c);
 
-    // srr after cluster i's update: srr - Re tr(dW^H (Src_i + Sec_i)), Sec_i = Src_i - dW Scc_i
-    const double* si = SrcG + ((size_t)i * B + bb) * NSRC;
+    double* sj = SrcG + ((size_t)j * B + bb) * NSRC;
+    cplx r[NC];                                          // row a of Src_j (Sr_j[a] in scalar form)
+    if (SCALAR) r[0] = mk(sj[2 * a], sj[2 * a + 1]);
+    else {
+#pragma unroll
+        for (int c = 0; c < 4; c++) { const double2 v = reinterpret_cast<const double2*>(sj)[4 * a + c]; r[c] = mk(v.x, v.y); }
+    }
+    cplx dw[NC];
+    for (int i = 0; i < j; i++) {
+        const sagecal_c128* J0 = J0g + (size_t)i * N * 4;
+        const sagecal_c128* J = Jg + (size_t)i * N * 4;
+#pragma unroll
+        for (int c = 0; c < NC; c++) dw[c] = SCALAR ? dP_entry(J0, J, p, q, a) : dW_entry(J0, J, p, q, a, c);
+        const double* x = Xg + ((size_t)grp_pair(i, j) * B + bb) * (SCALAR ? NX_SCALAR : NX_FULL);
+        if (SCALAR) r[0] = cfms(dw[0], mk(x[0], x[1]), r[0]);
+        else {
+            const double2* x2 = reinterpret_cast<const double2*>(x);      // records are 16-byte aligned
+#pragma unroll
+            for (int e = 0; e < 4; e++)
+#pragma unroll
+                for (int c = 0; c < 4; c++) { const double2 v = __ldg(x2 + 4 * e + c); r[c] = cfms(dw[e], mk(v.x, v.y), r[c]); }
+        }
+    }
+    if (live) {
+        if (SCALAR) { sj[2 * a] = r[0].re; sj[2 * a + 1] = r[0].im; }
+        else {
+#pragma unroll
+            for (int c = 0; c < 4; c++) reinterpret_cast<double2*>(sj)[4 * a + c] = make_double2(r[c].re, r[c].im);
+        }
+    }
+
+    // dw now holds row a of dW_{j-1}: srr_j = srr_{j-1} - Re tr(dW^H (Src + Sec)), Sec = Src - dW Scc, of cluster j-1
+    const double* si = SrcG + ((size_t)(j - 1) * B + bb) * NSRC;
     double d = 0.0;
     if (SCALAR) {
-        const double s2 = Scc_i[bb];
+        const double s2 = Scc_prev[bb];
         const cplx sr = mk(si[2 * a], si[2 * a + 1]);
         const cplx v = mk(2.0 * sr.re - s2 * dw[0].re, 2.0 * sr.im - s2 * dw[0].im);
         d = dw[0].re * v.re + dw[0].im * v.im;
     } else {
-        const double* sc = Scc_i + bb * NSCC_FULL;
+        const double* sc = Scc_prev + bb * NSCC_FULL;
 #pragma unroll
         for (int c = 0; c < 4; c++) {
             // (dW Scc)[a][c] = sum_e dW[a][e] Scc[e][c], Scc Hermitian from its packed form
@@ -377,32 +408,7 @@ groupfix_kernel(int N, int64_t B, int i, int gn, const sagecal_c128* __restrict_
     }
     d += __shfl_xor_sync(0xffffffffu, d, 1);
     d += __shfl_xor_sync(0xffffffffu, d, 2);
-    if (live && a == 0 && i + 1 < gn) SrcG[((size_t)(i + 1) * B + bb) * NSRC + NSRC - 2] = si[NSRC - 2] - d;
-
-    // Src_j -= dW_i X_ij for the later clusters of the group
-    for (int j = i + 1; j < gn; j++) {
-        const double* x = Xg + ((size_t)grp_pair(i, j) * B + bb) * (SCALAR ? NX_SCALAR : NX_FULL);
-        double* sj = SrcG + ((size_t)j * B + bb) * NSRC;
-        if (SCALAR) {
-            const cplx r = cfms(dw[0], mk(x[0], x[1]), mk(sj[2 * a], sj[2 * a + 1]));
-            if (live) { sj[2 * a] = r.re; sj[2 * a + 1] = r.im; }
-        } else {
-            // 16-byte accesses: records are 16-byte aligned (272 B and 256 B strides)
-            const double2* x2 = reinterpret_cast<const double2*>(x);
-            double2* sj2 = reinterpret_cast<double2*>(sj);
-            cplx xe[16];
-#pragma unroll
-            for (int e = 0; e < 16; e++) { const double2 v = __ldg(x2 + e); xe[e] = mk(v.x, v.y); }
-#pragma unroll
-            for (int c = 0; c < 4; c++) {
-                const double2 v = sj2[4 * a + c];
-                cplx r = mk(v.x, v.y);
-#pragma unroll
-                for (int e = 0; e < 4; e++) r = cfms(dw[e], xe[4 * e + c], r);
-                if (live) sj2[4 * a + c] = make_double2(r.re, r.im);
-            }
-        }
-    }
+    if (live && a == 0) sj[NSRC - 2] = si[NSRC - 2] - d;
 }
 
 
@@ -482,14 +488,14 @@ int enqueue_wbgroup(int N, int T, int F, int coh_format, sagecal_c128* R, const 
     return SAGECAL_OK;
 }
 
-int enqueue_groupfix(int N, bool scalar, int i, int gn, const sagecal_c128* J0_i, const sagecal_c128* J_i,
-                     const double* Scc_i, const double* Xgroup, double* SrcG, cudaStream_t st) {
-    if (i + 1 >= gn) return SAGECAL_OK;
+int enqueue_groupfix(int N, bool scalar, int j, const sagecal_c128* J0g, const sagecal_c128* Jg, const double* Scc_prev,
+                     const double* Xgroup, double* SrcG, cudaStream_t st) {
+    if (j < 1 || j >= GRP) return SAGECAL_OK;
     const int64_t B = (int64_t)N * (N - 1) / 2;
     const unsigned grid = (unsigned)((4 * B + 127) / 128);
     LaunchScope ls(KK_GFIX, st);
-    if (scalar) groupfix_kernel<true><<<grid, 128, 0, st>>>(N, B, i, gn, J0_i, J_i, Scc_i, Xgroup, SrcG);
-    else groupfix_kernel<false><<<grid, 128, 0, st>>>(N, B, i, gn, J0_i, J_i, Scc_i, Xgroup, SrcG);
+    if (scalar) groupfix_kernel<true><<<grid, 128, 0, st>>>(N, B, j, J0g, Jg, Scc_prev, Xgroup, SrcG);
+    else groupfix_kernel<false><<<grid, 128, 0, st>>>(N, B, j, J0g, Jg, Scc_prev, Xgroup, SrcG);
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
 }
