@@ -80,7 +80,7 @@ typedef struct { double re, im; } sagecal_c128;
 #define SAGECAL_LM_RECENTRE  10
 
 /* `what` of sagecal_workspace_bytes */
-#define SAGECAL_WS_LM_PASS   1          /* sagecal_lm_cost_grad_jtj: per-unit partial sums */
+#define SAGECAL_WS_LM_PASS   1          /* sagecal_lm_cost_grad_jtj: per-unit partial sums and per-baseline records */
 #define SAGECAL_WS_CALIBRATE 2          /* sagecal_sage_calibrate, lm_mode COMPRESSED or DIRECT, either coherency format:
                                            the above + per baseline K x 16 + 5 x 34 doubles of statistics and 6 x 32 doubles of
                                            cross grams per group of 4 clusters (3.7 GB at N=512, K=50) */
@@ -166,7 +166,9 @@ int sagecal_corrupt_subtract(
  * coh_k  : dev, this cluster's coherencies ([rows][F][4] or [rows][F]).
  * jones_k: dev [N][4].
  * cost   : dev out [1] f64.   grad, jtj : dev out [N][4] c128.
- * Sums are formed without global atomics in a fixed order: results are bit-reproducible run to run.
+ * Sums are formed without global atomics in a fixed order: results are bit-reproducible run to run.  (2x2 coherencies:
+ * on the FP64 tensor cores, one warp per baseline; an integer ticket counter decides which block adds the per-station
+ * cost partials last -- control flow only, the order of every floating-point sum is fixed.)
  */
 int sagecal_lm_cost_grad_jtj(
     int nstations, int ntime, int nchan,
