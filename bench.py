@@ -1,19 +1,23 @@
 #!/usr/bin/env python
 """bench.py -- one calibration interval per step on one B200 (replicas on N GPUs).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--coh full|scalar] [--impl ours|reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--coh full|scalar]
+                    [--lm compressed|percluster|direct|fullgn] [--impl ours|reference] [--grid | --rows]
 
 A step is one pass of the whole hot path over one synthetic interval:
-sagecal_predict_coherencies for all K clusters, then sagecal_sage_calibrate (initial residual, n_em x K x
-[add-back, (n_lm+1) fused cost/gradient/J^H J passes with the device-side LM control, write-back]).
+sagecal_predict_coherencies for all K clusters, then sagecal_sage_calibrate (initial residual, n_em x K M-steps of
+n_lm+1 cost/gradient/J^H J evaluations with the device-side LM control; in the default lm_mode the evaluations run on
+per-baseline statistics that one streaming kernel per group of four clusters takes together with the write-back of
+the previous group, in --lm direct every evaluation streams the cluster's samples).
 Workload: BASELINE.json configs[4] (N=512, T=20, F=8, K=50 x 40 sources, 3 EM x 10 LM), the configuration
 north_star's target is quoted on; it fits one GPU (67 GB of 2x2 coherencies).  Inputs are seeded and synthetic
 (sagecal_inputs, recipe in DESIGN.md §4); the visibilities are built on the device by the CUDA path itself.
 
 Prints ONE JSON line (rank 0).  `value` = seconds per interval with inputs resident in HBM; `e2e` = the same through
-sagecal_calibrate_interval_host with pinned HOST buffers (copies inside the timed region); `roofline` = the fused LM
-pass kernel (the dominant kernel: 1650 launches per step) against the measured HBM copy rate, its launch durations
-taken live with CUDA events on the launching stream inside the timed region; `cpu_baseline` = the oracle, as it
+sagecal_calibrate_interval_host with pinned HOST buffers (copies inside the timed region); `roofline` = the dominant
+streaming kernel of the mode (default: wbgroup_mma_kernel, 40 launches per step; --lm direct: the fused LM pass, 1650
+launches) against the measured HBM copy rate, its launch durations taken live with CUDA events on the launching stream
+inside the timed region; `cpu_baseline` = the oracle, as it
 stands, on a bounded sample of the same workload on the host cores.
 
 --impl reference times the oracle (the only other place bench.py executes oracle/) and prints the same line shape.
