@@ -129,3 +129,51 @@ def test_pass_errors(cuda_device):
                                     z.data_ptr(), z.data_ptr(), 1 << 20, None)
     assert rc == -1
     assert b.workspace_bytes(b.WS_LM_PASS, 512, 20, 8) > 0
+
+
+def test_lm_pass_full_size_tensor_core_form(cuda_device):
+    """sagecal_lm_cost_grad_jtj at configs[4]'s shape (N=512, T=20, F=8) with general 2x2 (polarised) coherencies: the
+    launch configuration of bench.py --lm direct, tensor-core form with the F = 8 fast path.  The oracle cannot run
+    130 816 baselines inside a test, so: gradient and J^H J of sampled stations against the definition evaluated by
+    the oracle's coherencies and plain numpy on those stations' 511 baselines (1e-10), and the cost against
+    ||x - J_p C J_q^H||^2 of the residual the corrupt kernel leaves (an independent kernel)."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from sagecal_inputs import baseline_index, make_config
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+
+    p = make_config(4, K=1, polarised=True)
+    N, T, F, B = p.N, p.T, p.F, p.B
+    coh_d = gpu_predict(p)
+    V = gpu_simulate(p, coh_d)
+    rng = np.random.default_rng(5)
+    J = (np.eye(2) + 0.2 * (rng.standard_normal((N, 2, 2)) + 1j * rng.standard_normal((N, 2, 2)))).astype(np.complex128)
+    Jd = dev(J)
+    cost, grad, jtj = sg.lm_cost_grad_jtj(N, T, F, V, coh_d[0], Jd)
+    res = sg.corrupt_subtract(N, T, F, coh_d, Jd.reshape(1, N, 2, 2), V, sign=-1.0)
+    r2 = float((res.abs() ** 2).sum())
+    assert abs(float(cost[0]) - r2) <= 1e-11 * r2
+    for s in (0, 255, 511):
+        others = [o for o in range(N) if o != s]
+        bl = np.array([baseline_index(N, min(s, o), max(s, o)) for o in others])
+        rows = (np.arange(T)[:, None] * B + bl[None, :]).reshape(-1)
+        C = oracle.predict(p, rows=rows)[0].reshape(T, N - 1, F, 2, 2)            # the oracle's coherencies
+        X = host(V[torch.from_numpy(rows).to(V.device)]).reshape(T, N - 1, F, 2, 2)
+        G = np.zeros((2, 2), complex)
+        M = np.zeros((2, 2), complex)
+        for j, o in enumerate(others):
+            Cm, Xm = C[:, j].reshape(-1, 2, 2), X[:, j].reshape(-1, 2, 2)
+            if s < o:   # s is the row station p: E = x - J_s C J_o^H, G += E A^H, M += A A^H, A = C J_o^H
+                A = Cm @ J[o].conj().T[None]
+                E = Xm - J[s][None] @ A
+                G += np.einsum("nij,nkj->ik", E, A.conj())
+                M += np.einsum("nij,nkj->ik", A, A.conj())
+            else:       # s is the column station q: E = x - J_o C J_s^H, G += E^H T1, M += T1^H T1, T1 = J_o C
+                T1 = J[o][None] @ Cm
+                E = Xm - T1 @ J[s].conj().T[None]
+                G += np.einsum("nji,njk->ik", E.conj(), T1)
+                M += np.einsum("nji,njk->ik", T1.conj(), T1)
+        assert rel_l2(host(grad[s]), G) < 1e-10, s
+        assert rel_l2(host(jtj[s]), M) < 1e-10, s
+    del coh_d, V, res
+    torch.cuda.empty_cache()
