@@ -293,13 +293,15 @@ int sagecal_profile_read(double* ms_host, long long* timed_host, long long* laun
 int sagecal_debug_pass_cover(int nstations, int ntime, int nchan, int32_t* cover, int64_t* info);
 
 /*
- * Test hook, host only: replays the tiling and lane mapping of the compressed M-step kernel and the
- * record lists of its station reduction.  cover : host out [B] int32, zeroed by the caller; every entry must come
- * back 1.  info : host out [6] int64 = {q tiles, p blocks, tiles decoded, B, rows per tile, tiles}.  Returns 0,
- * SAGECAL_EINVAL, or a positive bit mask (1/4: a row/column record is read but never written; 2/8: a record that
- * carries a baseline is never read; 16/32: a tile or record index out of range).
+ * Test hook, host only: replays the work decomposition of the compressed M-step kernel (one thread per
+ * baseline, a warp per chunk of rows of one 32-column segment) and the record lists of its station reduction, for a
+ * device with `sms` SMs, through the same geometry routines the launch uses.  cover : host out [B] int32, zeroed by the
+ * caller; every entry must come back 1.  info : host out [8] int64 = {column segments, rows per chunk, chunks, B, units,
+ * units visited, grid, shared-memory slots per warp}.  Returns 0, SAGECAL_EINVAL, or a positive bit mask (1/4: a
+ * row/column record is read but never written; 2/8: a record that carries a baseline is never read; 16/32: a chunk or
+ * record index out of range; 64: a unit visited twice).
  */
-int sagecal_debug_mstep_cover(int nstations, int32_t* cover, int64_t* info);
+int sagecal_debug_mstep_cover(int nstations, int sms, int32_t* cover, int64_t* info);
 
 /*
  * Test hook, host only: replays the fragment addressing of the tensor-core statistics kernel (DESIGN.md §5.5 "cluster

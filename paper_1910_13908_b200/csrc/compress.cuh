@@ -62,22 +62,40 @@ __device__ __forceinline__ cplx dP_entry(const sagecal_c128* __restrict__ J0, co
 
 #endif
 
-// ---- M-step kernel tiling (mstep.cu): tile = PB row stations p x 32 column stations q ---------------------------
-constexpr int MS_THREADS = 256, MS_WARPS = 8, MS_TQ = 32, MS_PB_MAX = 16, MS_NV = 12, MS_MAX_GRID = 2048;
+// ---- M-step kernel work decomposition (mstep.cu) -------------------------------------------------------------------
+// One THREAD per baseline.  A unit is (column segment qt, row station p): the up to 32 baselines (p, q), q in
+// [32 qt, 32 qt + 32), q > p, one per lane.  Segment qt has rows p = 0 .. nrows(qt)-1; units are numbered segment by
+// segment, u = ubase(qt) + p.  A chunk is m consecutive rows of one segment and belongs to one warp for the whole
+// launch (the lane's column station never changes, so its Jones and its column sums live in registers); chunks are
+// numbered segment by segment too.  m is the smallest chunk length for which all chunks fit the co-resident warps.
+constexpr int MS_THREADS = 256, MS_WARPS = 8, MS_TQ = 32, MS_NV = 12, MS_MAX_GRID = 160;
+constexpr int MS_MAX_WARPS = MS_MAX_GRID * MS_WARPS;
 struct MGeom {
-    int N, PB, nqt, npb, ntiles;
+    int N, nqt, m, nchunks, U;
     int64_t B;
-    // largest q of column tile qt
-    __host__ __device__ int qmax(int qt) const { int h = MS_TQ * (qt + 1); return (h < N ? h : N) - 1; }
-    // live row blocks of column tile qt: blocks pb with PB*pb < qmax(qt)
-    __host__ __device__ int nlive(int qt) const { return (qmax(qt) + PB - 1) / PB; }
+    __host__ __device__ int nrows(int qt) const { int h = MS_TQ * (qt + 1); return (h < N ? h : N) - 1; }
+    __host__ __device__ int chunks_in(int qt) const { return (nrows(qt) + m - 1) / m; }
+    // units before segment qt (every earlier segment is full: 32 (t+1) - 1 rows)
+    __host__ __device__ int ubase(int qt) const { return 16 * qt * (qt + 1) - qt; }
+    // chunks before segment qt
+    __host__ __device__ int cbase(int qt) const { int c = 0; for (int t = 0; t < qt; t++) c += chunks_in(t); return c; }
+    // chunk c -> its segment, first row and number of rows
+    __host__ __device__ void decode(int c, int& qt, int& p0, int& cnt) const {
+        qt = 0;
+        for (;;) { const int nc = chunks_in(qt); if (c < nc || qt == nqt - 1) break; c -= nc; qt++; }
+        p0 = c * m;
+        const int left = nrows(qt) - p0;
+        cnt = left < m ? (left > 0 ? left : 0) : m;
+    }
 };
-inline MGeom make_mgeom(int N, int PB) {
+inline MGeom make_mgeom(int N, int max_warps) {
     MGeom g;
-    g.N = N; g.PB = PB; g.nqt = (N + MS_TQ - 1) / MS_TQ; g.npb = (N - 1 + PB - 1) / PB;
-    g.B = (int64_t)N * (N - 1) / 2;
-    g.ntiles = 0;
-    for (int qt = 0; qt < g.nqt; qt++) g.ntiles += g.nlive(qt);
+    g.N = N; g.nqt = (N + MS_TQ - 1) / MS_TQ; g.B = (int64_t)N * (N - 1) / 2;
+    g.U = g.ubase(g.nqt - 1) + (N - 1);
+    for (g.m = 1;; g.m++) {
+        g.nchunks = g.cbase(g.nqt);
+        if (g.nchunks <= max_warps) break;
+    }
     return g;
 }
 
@@ -87,13 +105,12 @@ struct MstepCtl { double phi, mu, nu, pad; };
 struct CompressWorkspace {
     double* Scc;      // [K][B][nscc]
     double* Src;      // [B][nsrc]
-    double* Ppart;    // [nqt][N][12]  row-station partial sums, one record per (column tile, row)
-    double* Qpart;    // [npb(PB=2)][N][12]  column-station partial sums, one record per (row block, column)
+    double* Ppart;    // [U][12]  row-station partial sums, one record per unit
+    double* Qpart;    // [MS_MAX_WARPS][32][12]  column-station partial sums, one record per (chunk, column)
     double* cost_cta; // [MS_MAX_GRID] cost summed per CTA
-    double* pred_st;  // [2][N] predicted reduction per station, halves alternate by evaluation (readers of one
-                      //        evaluation must not see the next one's values)
-    double* mm_st;    // [N] max(M00, M11) per station (damping initialisation)
-    double* Htry;     // [N][4] J_try^H J_try as (h00, h11, Re h01, Im h01)
+    double* pred_cta; // [2][MS_MAX_GRID] predicted reduction summed per CTA, halves alternate by evaluation (readers
+                      //        of one evaluation must not see the next one's values)
+    double* mm_cta;   // [MS_MAX_GRID] max over the CTA's stations of max(M00, M11) (damping initialisation)
     sagecal_c128 *G, *M, *J_try;   // [N][4] accepted gradient / J^H J, trial Jones
     MstepCtl* ctl;
     unsigned* bar;    // grid barrier arrive counter (zeroed before every launch)

@@ -74,22 +74,30 @@ def test_pass_geometry_covers_every_baseline_once(lib, N, T, F):
     assert TC * tlen >= T > (TC - 1) * tlen
 
 
+@pytest.mark.parametrize("sms", [148, 16, 1])
 @pytest.mark.parametrize("N", [2, 3, 8, 16, 17, 31, 32, 33, 34, 47, 48, 49, 64, 65, 100, 129, 256, 257, 384, 512, 700])
-def test_mstep_tiling_covers_every_baseline_once(lib, N):
-    """mstep_kernel's tiles (PB rows x 32 columns, 4 lanes per baseline) visit every baseline exactly once, and its
-    station reduction reads exactly the records that were written and carry a contribution."""
+def test_mstep_decomposition_covers_every_baseline_once(lib, N, sms):
+    """mstep_kernel's units (one row station x one 32-column segment, a thread per baseline) are spread over the warps
+    in chunks of m rows: every baseline is visited exactly once, every unit once, and the station reduction reads exactly
+    the records that were written and carry a contribution -- for a full B200, a 16-SM and a 1-SM device."""
     lib.sagecal_debug_mstep_cover.restype = ctypes.c_int
-    lib.sagecal_debug_mstep_cover.argtypes = [ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    lib.sagecal_debug_mstep_cover.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
     B = N * (N - 1) // 2
     cover = np.zeros(B, np.int32)
-    info = np.zeros(6, np.int64)
-    rc = lib.sagecal_debug_mstep_cover(N, cover.ctypes.data, info.ctypes.data)
+    info = np.zeros(8, np.int64)
+    rc = lib.sagecal_debug_mstep_cover(N, sms, cover.ctypes.data, info.ctypes.data)
     assert rc == 0, f"record bookkeeping violated: mask {rc}, info {info}"
     assert np.all(cover == 1)
-    nqt, npb, seen, B_, PB, ntiles = info
-    assert nqt == -(-N // 32) and PB in (2, 4, 8, 16) and npb == -(-(N - 1) // PB) and B_ == B and seen == ntiles
-    if N == 512:
-        assert PB == 16 and ntiles == 272
+    nqt, m, nchunks, B_, U, units, grid, slots = info
+    nrows = [min(32 * (t + 1), N) - 1 for t in range(nqt)]
+    assert nqt == -(-N // 32) and B_ == B and U == sum(nrows) and units == U
+    assert nchunks == sum(-(-r // m) for r in nrows) and nchunks <= 8 * grid and grid <= max(sms, -(-nqt // 8))
+    assert m == 1 or sum(-(-r // (m - 1)) for r in nrows) > 8 * max(sms, -(-nqt // 8))     # m is the smallest that fits
+    assert slots == m or slots == 2
+    if N == 512 and sms == 148:
+        assert m == 4 and nchunks == 1088 and grid == 148 and slots == 2
+    if N == 256 and sms == 148:
+        assert m == 1 and slots == 1
 
 
 @pytest.mark.parametrize("N,T,F", [(2, 1, 1), (3, 1, 8), (5, 3, 3), (9, 2, 5), (6, 20, 8), (7, 2, 40), (12, 7, 1), (4, 3, 16)])
