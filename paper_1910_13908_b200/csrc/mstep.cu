@@ -60,26 +60,28 @@ __device__ __forceinline__ cplx lds_c(const double* p) {
     return mk(v.x, v.y);
 }
 
-// every lane of every warp gets the same sum / maximum of n <= MS_MAX_GRID values other CTAs wrote
-__device__ __forceinline__ double strided_sum(const double* p, int n, int lane) {
-    double t[MS_MAX_GRID / 32];
+// every lane of every warp gets the same sum / maximum of n <= MS_MAX_GRID values other CTAs wrote; the loads are a
+// separate step so that several sums' loads can be in flight together
+struct Strided { double t[MS_MAX_GRID / 32]; };
+__device__ __forceinline__ Strided strided_load(const double* p, int n, int lane) {
+    Strided r;
 #pragma unroll
     for (int u = 0; u < MS_MAX_GRID / 32; u++) {
         const int i = 32 * u + lane;
-        t[u] = i < n ? __ldcg(p + i) : 0.0;
+        r.t[u] = i < n ? __ldcg(p + i) : 0.0;
     }
+    return r;
+}
+__device__ __forceinline__ double strided_sum(const Strided& r) {
     double v = 0.0;
 #pragma unroll
-    for (int u = 0; u < MS_MAX_GRID / 32; u++) v += t[u];
+    for (int u = 0; u < MS_MAX_GRID / 32; u++) v += r.t[u];
     return wsum(v);
 }
-__device__ __forceinline__ double strided_max(const double* p, int n, int lane) {
+__device__ __forceinline__ double strided_max(const Strided& r) {
     double v = 0.0;
 #pragma unroll
-    for (int u = 0; u < MS_MAX_GRID / 32; u++) {
-        const int i = 32 * u + lane;
-        v = fmax(v, i < n ? __ldcg(p + i) : 0.0);
-    }
+    for (int u = 0; u < MS_MAX_GRID / 32; u++) v = fmax(v, r.t[u]);
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
     return v;
@@ -149,22 +151,38 @@ __device__ __forceinline__ void issue_unit(const MstepArgs& A, unsigned char* sl
     const int qlo = max(q0, p + 1), qhi = min(q0 + MS_TQ, N), cnt = qhi - qlo, l0 = qlo - q0;
     if (cnt <= 0) return;
     const int64_t b0 = bl_index(N, p, qlo);
-    {
-        const unsigned char* g = reinterpret_cast<const unsigned char*>(A.Src) + (size_t)b0 * S::SRC_B;
-        unsigned char* d = slot + l0 * S::SRC_B;
-        const int nchunk = cnt * (S::SRC_B / 16);
-        for (int c = lane; c < nchunk; c += 32) cp_async16(d + 16 * c, g + 16 * c);
+    const unsigned char* gs = reinterpret_cast<const unsigned char*>(A.Src) + (size_t)b0 * S::SRC_B;
+    const unsigned char* gc = reinterpret_cast<const unsigned char*>(A.Scc) + (size_t)b0 * S::SCC_B;
+    unsigned char* dc = slot + S::SCC_OFF;
+    if (cnt == MS_TQ) {
+        // a full row (every unit above the diagonal block): fixed trip counts, offsets are immediates
+        constexpr int NCH = MS_TQ * S::SRC_B / 16;                  // 16-byte chunks of the 32 Src records
+#pragma unroll
+        for (int k = 0; k < NCH / 32; k++) cp_async16(slot + 16 * lane + 512 * k, gs + 16 * lane + 512 * k);
+        if (NCH % 32 && lane < NCH % 32) cp_async16(slot + 16 * lane + 512 * (NCH / 32), gs + 16 * lane + 512 * (NCH / 32));
+        if (SCALAR) {
+            cp_async8(dc + 8 * lane, gc + 8 * lane);
+        } else {
+            // chunk c = lane + 32 k: record (lane >> 3) + 4 k, part lane & 7, rotated by the record index
+            const int rec = lane >> 3, rot0 = ((lane & 7) + rec) & 7;
+            unsigned char* d0 = dc + rec * 128 + rot0 * 16;
+            unsigned char* d1 = dc + rec * 128 + ((rot0 + 4) & 7) * 16;
+#pragma unroll
+            for (int k = 0; k < 8; k++) cp_async16(((k & 1) ? d1 : d0) + 512 * k, gc + 16 * lane + 512 * k);
+        }
+        return;
     }
     {
-        const unsigned char* g = reinterpret_cast<const unsigned char*>(A.Scc) + (size_t)b0 * S::SCC_B;
-        unsigned char* d = slot + S::SCC_OFF;
-        if (SCALAR) {
-            if (lane < cnt) cp_async8(d + 8 * (l0 + lane), g + 8 * lane);
-        } else {
-            for (int c = lane; c < cnt * 8; c += 32) {
-                const int l = l0 + (c >> 3);
-                cp_async16(d + l * 128 + (((c & 7) + l) & 7) * 16, g + 16 * c);
-            }
+        unsigned char* d = slot + l0 * S::SRC_B;
+        const int nchunk = cnt * (S::SRC_B / 16);
+        for (int c = lane; c < nchunk; c += 32) cp_async16(d + 16 * c, gs + 16 * c);
+    }
+    if (SCALAR) {
+        if (lane < cnt) cp_async8(dc + 8 * (l0 + lane), gc + 8 * lane);
+    } else {
+        for (int c = lane; c < cnt * 8; c += 32) {
+            const int l = l0 + (c >> 3);
+            cp_async16(dc + l * 128 + (((c & 7) + l) & 7) * 16, gc + 16 * c);
         }
     }
 }
@@ -400,26 +418,38 @@ __device__ __forceinline__ void phase_baselines(const MstepArgs& A, const Smem& 
 // ---- phase B helpers ----------------------------------------------------------------------------------------------
 struct StAcc { cplx g[4]; cplx m[4]; };
 
-// adds station s's records: lanes over records, butterfly; every lane returns the sums
+// adds station s's records: lanes over records (the loads of up to five records per lane are issued before the first
+// addition), butterfly; every lane returns the sums
+__device__ __forceinline__ void rec_load(const double* base, bool on, double2* t) {
+    const double2* rec = reinterpret_cast<const double2*>(base);
+#pragma unroll
+    for (int x = 0; x < MS_NV / 2; x++) t[x] = on ? __ldcg(rec + x) : make_double2(0.0, 0.0);
+}
 __device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, int s, int lane) {
     const MGeom& g = A.g;
     double acc[MS_NV];
 #pragma unroll
     for (int x = 0; x < MS_NV; x++) acc[x] = 0.0;
-    if (s <= g.N - 2) {      // as row station: one record per column segment that holds a q > s
-        for (int qt = (s + 1) / MS_TQ + lane; qt < g.nqt; qt += 32) {
-            const double2* rec = reinterpret_cast<const double2*>(A.Ppart + (size_t)(g.ubase(qt) + s) * MS_NV);
+    // as row station: one record per column segment that holds a q > s; as column station: the chunks of its
+    // segment that hold a row p < s
+    const int qt0 = (s + 1) / MS_TQ, nrow = s <= g.N - 2 ? g.nqt - qt0 : 0;
+    const int qts = s / MS_TQ, c0 = g.cbase(qts);
+    const int nr = min(s, g.nrows(qts)), nc = (nr + g.m - 1) / g.m;
+    const double* colbase = A.Qpart + ((size_t)c0 * MS_TQ + (s - MS_TQ * qts)) * MS_NV;
+    for (int i = 0; i < nrow || 4 * i < nc; i += 32) {
+        double2 tr[MS_NV / 2], tc[4][MS_NV / 2];
+        const int qt = qt0 + i + lane;
+        rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + s) * MS_NV, i + lane < nrow, tr);
 #pragma unroll
-            for (int x = 0; x < MS_NV / 2; x++) { const double2 t = __ldcg(rec + x); acc[2 * x] += t.x; acc[2 * x + 1] += t.y; }
+        for (int u = 0; u < 4; u++) {
+            const int c = 4 * i + 32 * u + lane;
+            rec_load(colbase + (size_t)(c < nc ? c : 0) * MS_TQ * MS_NV, c < nc, tc[u]);
         }
-    }
-    if (s >= 1) {            // as column station: the chunks of its segment that hold a row p < s
-        const int qt = s / MS_TQ, c0 = g.cbase(qt);
-        const int nr = min(s, g.nrows(qt)), nc = (nr + g.m - 1) / g.m;
-        for (int c = lane; c < nc; c += 32) {
-            const double2* rec = reinterpret_cast<const double2*>(A.Qpart + ((size_t)(c0 + c) * MS_TQ + (s - MS_TQ * qt)) * MS_NV);
 #pragma unroll
-            for (int x = 0; x < MS_NV / 2; x++) { const double2 t = __ldcg(rec + x); acc[2 * x] += t.x; acc[2 * x + 1] += t.y; }
+        for (int x = 0; x < MS_NV / 2; x++) {
+            acc[2 * x] += tr[x].x; acc[2 * x + 1] += tr[x].y;
+#pragma unroll
+            for (int u = 0; u < 4; u++) { acc[2 * x] += tc[u][x].x; acc[2 * x + 1] += tc[u][x].y; }
         }
     }
 #pragma unroll
@@ -438,7 +468,8 @@ __device__ __forceinline__ double trial_step(const MstepArgs& A, int s, int lane
     const double a = m[0].re + mu, d = m[3].re + mu;
     const cplx b = m[1];
     const double det = a * d - (b.re * b.re + b.im * b.im);
-    const cplx inv[4] = {mk(d / det, 0.0), mk(-b.re / det, -b.im / det), mk(-b.re / det, b.im / det), mk(a / det, 0.0)};
+    const double rdet = 1.0 / det;
+    const cplx inv[4] = {mk(d * rdet, 0.0), mk(-b.re * rdet, -b.im * rdet), mk(-b.re * rdet, b.im * rdet), mk(a * rdet, 0.0)};
     cplx dj[4];
     dj[0] = cfma(g[1], inv[2], cmul(g[0], inv[0]));
     dj[1] = cfma(g[1], inv[3], cmul(g[0], inv[1]));
@@ -529,12 +560,12 @@ mstep_kernel(const MstepArgs A) {
                 }
                 mm = fmax(mm, fmax(r.m[0].re, r.m[3].re));
             }
-            phi = strided_sum(A.cost_cta, (int)gridDim.x, lane);
+            phi = strided_sum(strided_load(A.cost_cta, (int)gridDim.x, lane));
             if (lane == 0) sm.s_red[2 * MS_WARPS + warp] = mm;
             __syncthreads();
             if (threadIdx.x == 0) publish(sm.s_red + 2 * MS_WARPS, A.mm_cta, true);
             grid_barrier<CLUSTER>(A.bar, ++gen);
-            mu = A.tau * strided_max(A.mm_cta, (int)gridDim.x, lane);
+            mu = A.tau * strided_max(strided_load(A.mm_cta, (int)gridDim.x, lane));
             nu = 2.0;
             if (!(mu >= 1e-300)) mu = 1e-300;
             if (mu > 1e300) mu = 1e300;
@@ -555,19 +586,21 @@ mstep_kernel(const MstepArgs A) {
                 const sagecal_c128* src = which < 4 ? A.G : which < 8 ? A.M : which < 12 ? A.Jk : A.J_try;
                 return ldcg_c(src + 4 * s + (which & 3));
             };
+            const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
+            const Strided pred_l = strided_load(A.pred_cta + (size_t)((e + 1) & 1) * MS_MAX_GRID, e > 0 ? (int)gridDim.x : 0, lane);
             cplx mine = mk(0.0, 0.0);
             StAcc r0;
             if (s0 < N) {
                 mine = old_elem(s0);
                 r0 = station_reduce(A, s0, lane);
             }
-            const double fresh = strided_sum(A.cost_cta, (int)gridDim.x, lane);
+            const double fresh = strided_sum(cost_l);
             bool accept = false;
             if (e == 0) {
                 phi = fresh;                  // re-centre: fresh (phi, G, M) at the accepted Jones, mu and nu continue
             } else {
                 // summed per CTA in the previous evaluation; this evaluation's go to the other half
-                const double pred = strided_sum(A.pred_cta + (size_t)((e - 1) & 1) * MS_MAX_GRID, (int)gridDim.x, lane);
+                const double pred = strided_sum(pred_l);
                 const double rho = (phi - fresh) / pred;
                 accept = isfinite(fresh) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
                 if (accept) {
@@ -670,9 +703,11 @@ CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws) {
 }
 
 // Launch plan of the M-step kernel for N stations on a device with `sms` SMs (one CTA per SM): work decomposition,
-// slots per warp, grid.  Device independent but for `sms`, so that the host replay below sees what the kernel does.
+// slots per warp, grid.  Device independent but for `sms` and `cluster_cap` (the largest thread-block cluster the
+// device schedules, 0 = none), so that the host replay below sees what the kernel does.
+constexpr int MS_CLUSTER_MAX = 16;
 struct MstepPlan { MGeom g; int slots, grid; bool cluster; };
-static MstepPlan make_plan(int N, bool scalar, int sms) {
+static MstepPlan make_plan(int N, bool scalar, int sms, int cluster_cap) {
     MstepPlan pl;
     int cap = sms < MS_MAX_GRID ? sms : MS_MAX_GRID;
     if (cap < 1) cap = 1;
@@ -685,37 +720,59 @@ static MstepPlan make_plan(int N, bool scalar, int sms) {
     pl.grid = want < cap ? want : cap;
     if (pl.grid * MS_WARPS < pl.g.nchunks) pl.grid = (pl.g.nchunks + MS_WARPS - 1) / MS_WARPS;
     if (pl.grid < 1) pl.grid = 1;
-    pl.cluster = false;
+    // the smallest arrays run as ONE thread-block cluster: its hardware barrier replaces the arrive counter
+    pl.cluster = pl.g.nchunks <= cluster_cap * MS_WARPS;
+    if (pl.cluster) {
+        if (pl.grid > cluster_cap) pl.grid = cluster_cap;
+        if (pl.grid * MS_WARPS < pl.g.nchunks) pl.grid = (pl.g.nchunks + MS_WARPS - 1) / MS_WARPS;
+    }
     return pl;
 }
 
+struct MstepDevice { bool ready; int sms, cluster_cap; };
 template <bool SCALAR>
-static int mstep_prepare(int* sms_out) {
+static int mstep_prepare(MstepDevice* out) {
     // per device: the opt-in to large dynamic shared memory is a per-device function attribute
-    static bool ready[64] = {};
-    static int sms[64] = {};
+    static MstepDevice devs[64] = {};
     int dev = 0;
     SGC_CUDA(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
-    if (!ready[dev]) {
+    MstepDevice& d = devs[dev];
+    if (!d.ready) {
         const int smem = (int)mstep_smem_bytes<SCALAR>(max_slots<SCALAR>());
         SGC_CUDA(cudaFuncSetAttribute(mstep_kernel<SCALAR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        int n = 0;
-        SGC_CUDA(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
-        sms[dev] = n;
-        ready[dev] = true;
+        SGC_CUDA(cudaFuncSetAttribute(mstep_kernel<SCALAR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SGC_CUDA(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev));
+        // the largest cluster (16 needs the non-portable opt-in, 8 is portable) that can be resident with the
+        // shared memory of a small array (its rows are resident: one slot per warp)
+        d.cluster_cap = 0;
+        const bool np = cudaFuncSetAttribute(mstep_kernel<SCALAR, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+        for (int csz = np ? MS_CLUSTER_MAX : 8; csz >= 2 && !d.cluster_cap; csz >>= 1) {
+            cudaLaunchConfig_t cfg = {};
+            cfg.gridDim = dim3((unsigned)csz); cfg.blockDim = dim3(MS_THREADS);
+            cfg.dynamicSmemBytes = mstep_smem_bytes<SCALAR>(1);
+            cudaLaunchAttribute at;
+            at.id = cudaLaunchAttributeClusterDimension;
+            at.val.clusterDim.x = (unsigned)csz; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+            cfg.attrs = &at; cfg.numAttrs = 1;
+            int ncl = 0;
+            if (cudaOccupancyMaxActiveClusters(&ncl, mstep_kernel<SCALAR, true>, &cfg) == cudaSuccess && ncl >= 1) d.cluster_cap = csz;
+        }
+        (void)cudaGetLastError();
+        d.ready = true;
     }
-    *sms_out = sms[dev];
+    *out = d;
     return SAGECAL_OK;
 }
 
 int enqueue_mstep(int N, bool scalar, const CompressWorkspace& w, const double* Scc_k, sagecal_c128* J0,
                   sagecal_c128* Jk, int n_trial, bool init, double tau, double* cost_out, double* trace_out,
                   cudaStream_t st) {
-    int sms = 0, rc;
-    if ((rc = scalar ? mstep_prepare<true>(&sms) : mstep_prepare<false>(&sms))) return rc;
-    const MstepPlan pl = make_plan(N, scalar, sms);
-    if (pl.grid > sms || pl.grid > MS_MAX_GRID) return SAGECAL_EUNSUPPORTED;     // more column segments than warps
+    MstepDevice dv;
+    int rc;
+    if ((rc = scalar ? mstep_prepare<true>(&dv) : mstep_prepare<false>(&dv))) return rc;
+    const MstepPlan pl = make_plan(N, scalar, dv.sms, dv.cluster_cap);
+    if (pl.grid > dv.sms || pl.grid > MS_MAX_GRID) return SAGECAL_EUNSUPPORTED;     // more column segments than warps
     MstepArgs A;
     A.g = pl.g;
     A.slots = pl.slots;
@@ -724,9 +781,22 @@ int enqueue_mstep(int N, bool scalar, const CompressWorkspace& w, const double* 
     A.G = w.G; A.M = w.M; A.J_try = w.J_try; A.J0 = J0; A.Jk = Jk;
     A.ctl = w.ctl; A.bar = w.bar; A.n_trial = n_trial; A.init = init ? 1 : 0; A.tau = tau;
     A.cost_out = cost_out; A.trace_out = trace_out;
+    const size_t smem = scalar ? mstep_smem_bytes<true>(pl.slots) : mstep_smem_bytes<false>(pl.slots);
+    if (pl.cluster) {
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = dim3((unsigned)pl.grid); cfg.blockDim = dim3(MS_THREADS);
+        cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cudaLaunchAttribute at;
+        at.id = cudaLaunchAttributeClusterDimension;
+        at.val.clusterDim.x = (unsigned)pl.grid; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
+        cfg.attrs = &at; cfg.numAttrs = 1;
+        LaunchScope ls(KK_MSTEP, st);
+        if (scalar) SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_kernel<true, true>, A));
+        else SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_kernel<false, true>, A));
+        return SAGECAL_OK;
+    }
     SGC_CUDA(cudaMemsetAsync(w.bar, 0, 256, st));
     void* args[] = {(void*)&A};
-    const size_t smem = scalar ? mstep_smem_bytes<true>(pl.slots) : mstep_smem_bytes<false>(pl.slots);
     LaunchScope ls(KK_MSTEP, st);
     SGC_CUDA(cudaLaunchCooperativeKernel(scalar ? (const void*)mstep_kernel<true, false> : (const void*)mstep_kernel<false, false>,
                                          dim3((unsigned)pl.grid), dim3(MS_THREADS), args, smem, st));
@@ -741,7 +811,7 @@ using namespace sgc;
 // MGeom / make_plan the launch uses, for a device with `sms` SMs.
 extern "C" int sagecal_debug_mstep_cover(int N, int sms, int32_t* cover, int64_t* info) {
     if (N < 2 || sms < 1 || !cover || !info) return SAGECAL_EINVAL;
-    const MstepPlan pl = make_plan(N, false, sms);
+    const MstepPlan pl = make_plan(N, false, sms, sms >= MS_CLUSTER_MAX ? MS_CLUSTER_MAX : 0);
     const MGeom& g = pl.g;
     const size_t nP = (size_t)g.U, nQ = (size_t)g.nchunks * MS_TQ;
     // bit 0: written, bit 1: carries a baseline, bit 2: read by the station reduction
