@@ -72,11 +72,11 @@ __device__ __forceinline__ Strided strided_load(const double* p, int n, int lane
     }
     return r;
 }
-__device__ __forceinline__ double strided_sum(const Strided& r) {
+__device__ __forceinline__ double strided_partial(const Strided& r) {     // this lane's share, fixed order
     double v = 0.0;
 #pragma unroll
     for (int u = 0; u < MS_MAX_GRID / 32; u++) v += r.t[u];
-    return wsum(v);
+    return v;
 }
 __device__ __forceinline__ double strided_max(const Strided& r) {
     double v = 0.0;
@@ -190,7 +190,7 @@ __device__ __forceinline__ void issue_unit(const MstepArgs& A, unsigned char* sl
 // ---- one baseline -------------------------------------------------------------------------------------------------
 // The lane's column station q, constant over the rows of its chunk.
 struct QSide {
-    cplx j[4], j0[4], d[4];     // J_q (trial), J0_q, D_q = J_q - J0_q
+    cplx j[4], d[4];            // J_q (trial), D_q = J_q - J0_q
     double h00, h11; cplx h01;  // J_q^H J_q
 };
 __device__ __forceinline__ void gram22(const cplx* j, double& h00, double& h11, cplx& h01) {
@@ -218,13 +218,14 @@ __device__ __forceinline__ void baseline_task(const double* src, const unsigned 
         for (int a = 0; a < 4; a++) {
             const int i = a >> 1, j = a & 1;
             const cplx jp[2] = {lds_c(pj + 4 * i), lds_c(pj + 4 * i + 2)};
+            const cplx jp0[2] = {lds_c(pj + 8 + 4 * i), lds_c(pj + 8 + 4 * i + 2)};
             const cplx dp[2] = {lds_c(pj + 16 + 4 * i), lds_c(pj + 16 + 4 * i + 2)};
             const cplx sr = lds_c(src + 2 * a);
-            // dP[(i,j)] = sum_k D_p[i,k] conj(J0_q[j,k]) + J_p[i,k] conj(D_q[j,k])
-            cplx dP = cmulc(dp[0], Q.j0[2 * j]);
-            dP = cfmac(dp[1], Q.j0[2 * j + 1], dP);
-            dP = cfmac(jp[0], Q.d[2 * j], dP);
-            dP = cfmac(jp[1], Q.d[2 * j + 1], dP);
+            // dP[(i,j)] = sum_k D_p[i,k] conj(J_q[j,k]) + J0_p[i,k] conj(D_q[j,k])   (= D_p J0_q^H + J_p D_q^H)
+            cplx dP = cmulc(dp[0], Q.j[2 * j]);
+            dP = cfmac(dp[1], Q.j[2 * j + 1], dP);
+            dP = cfmac(jp0[0], Q.d[2 * j], dP);
+            dP = cfmac(jp0[1], Q.d[2 * j + 1], dP);
             const cplx se = mk(fma(-s2, dP.re, sr.re), fma(-s2, dP.im, sr.im));
             acc = fma(dP.re, sr.re + se.re, fma(dP.im, sr.im + se.im, acc));
             gp[2 * i] = cfma(se, Q.j[2 * j], gp[2 * i]);              // G_p[i,k] += Se[(i,j)] J_q[j,k]
@@ -256,13 +257,15 @@ __device__ __forceinline__ void baseline_task(const double* src, const unsigned 
         for (int a = 0; a < 4; a++) {
             const int i = a >> 1, j = a & 1;
             const cplx jp[2] = {lds_c(pj + 4 * i), lds_c(pj + 4 * i + 2)};
-            // row a of dW: dW[(k,l)] = D_p[i,k] conj(J0_q[j,l]) + J_p[i,k] conj(D_q[j,l])
+            // row a of dW: dW[(k,l)] = D_p[i,k] conj(J_q[j,l]) + J0_p[i,k] conj(D_q[j,l])
+            // (= D_p (x) conj(J0_q) + J_p (x) conj(D_q), with J0_q = J_q - D_q substituted: no centre Jones per lane)
             cplx dW[4];
             {
                 const cplx dp[2] = {lds_c(pj + 16 + 4 * i), lds_c(pj + 16 + 4 * i + 2)};
+                const cplx jp0[2] = {lds_c(pj + 8 + 4 * i), lds_c(pj + 8 + 4 * i + 2)};
 #pragma unroll
                 for (int c = 0; c < 4; c++)
-                    dW[c] = cfmac(jp[c >> 1], Q.d[2 * j + (c & 1)], cmulc(dp[c >> 1], Q.j0[2 * j + (c & 1)]));
+                    dW[c] = cfmac(jp0[c >> 1], Q.d[2 * j + (c & 1)], cmulc(dp[c >> 1], Q.j[2 * j + (c & 1)]));
             }
             // row a of Src (64 B), Sec = Src - dW Scc (the diagonal of Scc is real), cost
             cplx sec[4];
@@ -369,9 +372,8 @@ __device__ __forceinline__ void phase_baselines(const MstepArgs& A, const Smem& 
         QSide Q;
 #pragma unroll
         for (int x = 0; x < 4; x++) {
-            Q.j0[x] = j0q[x];
             Q.j[x] = e == 0 ? j0q[x] : (qlive ? ldcg_c(A.J_try + 4 * q + x) : mk(0.0, 0.0));
-            Q.d[x] = csub(Q.j[x], Q.j0[x]);
+            Q.d[x] = csub(Q.j[x], j0q[x]);
         }
         gram22(Q.j, Q.h00, Q.h11, Q.h01);
         cplx gq[4] = {mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0)};
@@ -416,34 +418,47 @@ __device__ __forceinline__ void phase_baselines(const MstepArgs& A, const Smem& 
 }
 
 // ---- phase B helpers ----------------------------------------------------------------------------------------------
-struct StAcc { cplx g[4]; cplx m[4]; };
+struct StAcc { cplx g[4]; cplx m[4]; double x0, x1; };
 
-// adds station s's records: lanes over records (the loads of up to five records per lane are issued before the first
-// addition), butterfly; every lane returns the sums
+// Where station s finds its records: as row station one record per column segment that holds a q > s, as column
+// station the chunks of its segment that hold a row p < s.  Constant over the launch, computed once per warp for its
+// first station (the integer divisions behind cbase() would otherwise sit on the critical path of every evaluation).
+struct StationPlan { int s, qt0, nrow, nc; const double* colbase; };
+__device__ __forceinline__ StationPlan make_station_plan(const MstepArgs& A, int s) {
+    const MGeom& g = A.g;
+    StationPlan sp;
+    sp.s = s;
+    sp.qt0 = (s + 1) / MS_TQ;
+    sp.nrow = s <= g.N - 2 ? g.nqt - sp.qt0 : 0;
+    const int qts = s / MS_TQ, c0 = g.cbase(qts);
+    const int nr = min(s, g.nrows(qts));
+    sp.nc = (nr + g.m - 1) / g.m;
+    sp.colbase = A.Qpart + ((size_t)c0 * MS_TQ + (s - MS_TQ * qts)) * MS_NV;
+    return sp;
+}
+
+// Adds the station's records, lanes over records (the loads of up to five records per lane are issued before the first
+// addition), then ONE halving exchange sums the 12 station values together with two more lane-partial values x0, x1
+// (the CTA costs and predicted reductions: the same numbers in the same lanes of every warp, so every warp of the grid
+// gets bit-identical totals) and 14 shuffles hand every lane every total.
 __device__ __forceinline__ void rec_load(const double* base, bool on, double2* t) {
     const double2* rec = reinterpret_cast<const double2*>(base);
 #pragma unroll
     for (int x = 0; x < MS_NV / 2; x++) t[x] = on ? __ldcg(rec + x) : make_double2(0.0, 0.0);
 }
-__device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, int s, int lane) {
+__device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, const StationPlan& sp, int lane, double x0, double x1) {
     const MGeom& g = A.g;
-    double acc[MS_NV];
+    double acc[16];
 #pragma unroll
-    for (int x = 0; x < MS_NV; x++) acc[x] = 0.0;
-    // as row station: one record per column segment that holds a q > s; as column station: the chunks of its
-    // segment that hold a row p < s
-    const int qt0 = (s + 1) / MS_TQ, nrow = s <= g.N - 2 ? g.nqt - qt0 : 0;
-    const int qts = s / MS_TQ, c0 = g.cbase(qts);
-    const int nr = min(s, g.nrows(qts)), nc = (nr + g.m - 1) / g.m;
-    const double* colbase = A.Qpart + ((size_t)c0 * MS_TQ + (s - MS_TQ * qts)) * MS_NV;
-    for (int i = 0; i < nrow || 4 * i < nc; i += 32) {
+    for (int x = 0; x < 16; x++) acc[x] = 0.0;
+    for (int i = 0; i < sp.nrow || 4 * i < sp.nc; i += 32) {
         double2 tr[MS_NV / 2], tc[4][MS_NV / 2];
-        const int qt = qt0 + i + lane;
-        rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + s) * MS_NV, i + lane < nrow, tr);
+        const int qt = sp.qt0 + i + lane;
+        rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + sp.s) * MS_NV, i + lane < sp.nrow, tr);
 #pragma unroll
         for (int u = 0; u < 4; u++) {
             const int c = 4 * i + 32 * u + lane;
-            rec_load(colbase + (size_t)(c < nc ? c : 0) * MS_TQ * MS_NV, c < nc, tc[u]);
+            rec_load(sp.colbase + (size_t)(c < sp.nc ? c : 0) * MS_TQ * MS_NV, c < sp.nc, tc[u]);
         }
 #pragma unroll
         for (int x = 0; x < MS_NV / 2; x++) {
@@ -452,12 +467,16 @@ __device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, int s, int l
             for (int u = 0; u < 4; u++) { acc[2 * x] += tc[u][x].x; acc[2 * x + 1] += tc[u][x].y; }
         }
     }
+    acc[12] = x0; acc[13] = x1;
+    halve_sum16(acc, lane);
+    double t[14];
 #pragma unroll
-    for (int x = 0; x < MS_NV; x++) acc[x] = wsum(acc[x]);
+    for (int x = 0; x < 14; x++) t[x] = __shfl_sync(0xffffffffu, acc[0], 2 * x);     // lane 2x holds index x
     StAcc r;
 #pragma unroll
-    for (int x = 0; x < 4; x++) r.g[x] = mk(acc[2 * x], acc[2 * x + 1]);
-    r.m[0] = mk(acc[8], 0.0); r.m[1] = mk(acc[10], acc[11]); r.m[2] = mk(acc[10], -acc[11]); r.m[3] = mk(acc[9], 0.0);
+    for (int x = 0; x < 4; x++) r.g[x] = mk(t[2 * x], t[2 * x + 1]);
+    r.m[0] = mk(t[8], 0.0); r.m[1] = mk(t[10], t[11]); r.m[2] = mk(t[10], -t[11]); r.m[3] = mk(t[9], 0.0);
+    r.x0 = t[12]; r.x1 = t[13];
     return r;
 }
 
@@ -534,7 +553,12 @@ mstep_kernel(const MstepArgs A) {
         }
     }
 
-    // LM state, identical in every thread of the grid
+    // this warp's stations: gw, gw + nw, ...; the plan of the first (for almost every shape the only one)
+    StationPlan sp0;
+    sp0.s = gw; sp0.qt0 = 0; sp0.nrow = 0; sp0.nc = 0; sp0.colbase = A.Qpart;
+    if (gw < N) sp0 = make_station_plan(A, gw);
+
+    // LM state, identical in every thread that owns a station
     double phi = 0.0, mu = A.init ? 0.0 : A.ctl->mu, nu = A.init ? 2.0 : A.ctl->nu;
 
     // the centre of this chunk's statistics = the current Jones of the cluster (read by the later write-back)
@@ -548,59 +572,60 @@ mstep_kernel(const MstepArgs A) {
         if (threadIdx.x == 0) publish(sm.s_red, A.cost_cta, false);
         grid_barrier<CLUSTER>(A.bar, ++gen);
 
+        // Warps without a station have nothing to decide; they only keep the barriers company.
         double pred_w = 0.0;
         if (e == 0 && A.init) {
             // (phi, G, M) at the centre are the accepted state; mu = tau * max_p max(M_p00, M_p11)
             double mm = 0.0;
-            for (int s = gw; s < N; s += nw) {
-                const StAcc r = station_reduce(A, s, lane);
-                if (lane == 0) {
+            if (sp0.s < N) {
+                const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
+                for (int s = sp0.s; s < N; s += nw) {
+                    const StAcc r = station_reduce(A, s == sp0.s ? sp0 : make_station_plan(A, s), lane, strided_partial(cost_l), 0.0);
+                    if (lane == 0) {
 #pragma unroll
-                    for (int x = 0; x < 4; x++) { st_c(A.G + 4 * s + x, r.g[x]); st_c(A.M + 4 * s + x, r.m[x]); }
+                        for (int x = 0; x < 4; x++) { st_c(A.G + 4 * s + x, r.g[x]); st_c(A.M + 4 * s + x, r.m[x]); }
+                    }
+                    mm = fmax(mm, fmax(r.m[0].re, r.m[3].re));
+                    phi = r.x0;
                 }
-                mm = fmax(mm, fmax(r.m[0].re, r.m[3].re));
             }
-            phi = strided_sum(strided_load(A.cost_cta, (int)gridDim.x, lane));
             if (lane == 0) sm.s_red[2 * MS_WARPS + warp] = mm;
             __syncthreads();
             if (threadIdx.x == 0) publish(sm.s_red + 2 * MS_WARPS, A.mm_cta, true);
             grid_barrier<CLUSTER>(A.bar, ++gen);
-            mu = A.tau * strided_max(strided_load(A.mm_cta, (int)gridDim.x, lane));
-            nu = 2.0;
-            if (!(mu >= 1e-300)) mu = 1e-300;
-            if (mu > 1e300) mu = 1e300;
-            if (!last) {
-                for (int s = gw; s < N; s += nw) {
-                    cplx g4[4], m4[4], jj[4];
+            if (sp0.s < N) {
+                mu = A.tau * strided_max(strided_load(A.mm_cta, (int)gridDim.x, lane));
+                nu = 2.0;
+                if (!(mu >= 1e-300)) mu = 1e-300;
+                if (mu > 1e300) mu = 1e300;
+                if (!last) {
+                    for (int s = sp0.s; s < N; s += nw) {
+                        cplx g4[4], m4[4], jj[4];
 #pragma unroll
-                    for (int x = 0; x < 4; x++) { g4[x] = ldcg_c(A.G + 4 * s + x); m4[x] = ldcg_c(A.M + 4 * s + x); jj[x] = ldcg_c(A.Jk + 4 * s + x); }
-                    pred_w += trial_step(A, s, lane, g4, m4, jj, mu);
+                        for (int x = 0; x < 4; x++) { g4[x] = ldcg_c(A.G + 4 * s + x); m4[x] = ldcg_c(A.M + 4 * s + x); jj[x] = ldcg_c(A.Jk + 4 * s + x); }
+                        pred_w += trial_step(A, s, lane, g4, m4, jj, mu);
+                    }
                 }
             }
-        } else {
-            // this warp's first station: its loads are issued before the control sums so that both are in flight.
-            // The accepted (G, M, J) and the trial J of a station are 16 complex numbers: lane x & 15 holds one.
-            const int s0 = gw;
+        } else if (sp0.s < N) {
+            // All loads are issued before anything is consumed: the CTA partials, the accepted (G, M, J) and the trial
+            // J of the station (16 complex numbers: lane x & 15 holds one), then its records.
+            const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
+            const Strided pred_l = strided_load(A.pred_cta + (size_t)((e + 1) & 1) * MS_MAX_GRID, e > 0 ? (int)gridDim.x : 0, lane);
             const int which = lane & 15;
             auto old_elem = [&](int s) {
                 const sagecal_c128* src = which < 4 ? A.G : which < 8 ? A.M : which < 12 ? A.Jk : A.J_try;
                 return ldcg_c(src + 4 * s + (which & 3));
             };
-            const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
-            const Strided pred_l = strided_load(A.pred_cta + (size_t)((e + 1) & 1) * MS_MAX_GRID, e > 0 ? (int)gridDim.x : 0, lane);
-            cplx mine = mk(0.0, 0.0);
-            StAcc r0;
-            if (s0 < N) {
-                mine = old_elem(s0);
-                r0 = station_reduce(A, s0, lane);
-            }
-            const double fresh = strided_sum(cost_l);
+            cplx mine = old_elem(sp0.s);
+            StAcc r = station_reduce(A, sp0, lane, strided_partial(cost_l), strided_partial(pred_l));
+            const double fresh = r.x0;
             bool accept = false;
             if (e == 0) {
                 phi = fresh;                  // re-centre: fresh (phi, G, M) at the accepted Jones, mu and nu continue
             } else {
                 // summed per CTA in the previous evaluation; this evaluation's go to the other half
-                const double pred = strided_sum(pred_l);
+                const double pred = r.x1;
                 const double rho = (phi - fresh) / pred;
                 accept = isfinite(fresh) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
                 if (accept) {
@@ -617,13 +642,10 @@ mstep_kernel(const MstepArgs A) {
             if (mu > 1e300) mu = 1e300;
             if (nu > 0x1p60) nu = 0x1p60;
             const bool take = accept || e == 0;
-            for (int s = s0; s < N; s += nw) {
-                StAcc r;
-                if (s == s0) {
-                    r = r0;
-                } else {
+            for (int s = sp0.s; s < N; s += nw) {
+                if (s != sp0.s) {
                     mine = old_elem(s);
-                    r = station_reduce(A, s, lane);
+                    r = station_reduce(A, make_station_plan(A, s), lane, 0.0, 0.0);
                 }
                 cplx g4[4], m4[4], jj[4];
 #pragma unroll
