@@ -150,6 +150,58 @@ def load_traffic(coh: str, kernel: str = "lm_pass"):
     return None
 
 
+def load_counts(kernel: str, arm: str):
+    """FP64 thread-instructions per unit of work of an ALU-bound kernel (predict: per visibility x source; mstep: per
+    baseline x evaluation), from ncu's smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum at the bench
+    workload divided by the launch's units: profiles/kernel_counts.csv (kernel,arm,unit,fp64_inst_per_unit), else None."""
+    path = os.path.join(ROOT, "profiles", "kernel_counts.csv")
+    try:
+        for l in open(path):
+            f = [x.strip() for x in l.split(",")]
+            if len(f) >= 4 and not l.startswith("#") and f[0] == kernel and f[1] == arm:
+                return float(f[3])
+    except Exception:
+        pass
+    return None
+
+
+def stream_bytes_per_interval(samples: int, K: int, n_em: int, coh: str, lm: str = "compressed", n_lm: int = 10) -> int:
+    """Algorithmic HBM bytes of the streaming kernels of one interval: the initial residual reads V and
+    all K coherencies and writes R ((2 + K) x 64 B per sample; 16 B per scalar coherency), then the write-back /
+    statistics launches (cluster groups: wbgroup_bytes_per_sample; cluster by cluster: 256 / 160 B per sample and
+    launch but the first and last; direct: 128 / 80 B per pass plus add-back and write-back)."""
+    cb = 64 if coh == "full" else 16
+    init = (128 + K * cb) * samples
+    if K == 0 or n_em == 0:
+        return init
+    if uses_groups(lm, coh, n_lm):
+        return init + sum(wbgroup_bytes_per_sample(K, n_em, coh)) * samples
+    if lm == "direct":
+        return init + n_em * K * ((n_lm + 1) * PASS_BYTES_PER_SAMPLE[coh] + 2 * (128 + cb)) * samples
+    n_launch = n_em * K * max(1, -(-n_lm // LM_RECENTRE)) + 1
+    return init + ((n_launch - 2) * WBSTAT_BYTES_PER_SAMPLE[coh] + (64 + cb) + (128 + cb)) * samples
+
+
+def interval_floor(samples: int, vis_src: int, K: int, n_em: int, coh: str, hbm_gbs: float, dfma_per_s: float,
+                   predict_inst_per_vis_src: float, lm: str = "compressed", n_lm: int = 10) -> dict:
+    """Roofline floor of one interval: the streaming kernels' algorithmic bytes at the measured copy rate plus the
+    prediction's FP64 instructions at the measured DFMA rate (the M-step and the small kernels count as overhead)."""
+    b = stream_bytes_per_interval(samples, K, n_em, coh, lm, n_lm)
+    hbm_s = b / (hbm_gbs * 1e9)
+    alu_s = vis_src * predict_inst_per_vis_src / dfma_per_s if dfma_per_s and predict_inst_per_vis_src else 0.0
+    return {"stream_bytes": int(b), "hbm_floor_s": hbm_s, "predict_alu_floor_s": alu_s, "floor_s": hbm_s + alu_s}
+
+
+def cpu_model() -> str:
+    try:
+        for l in open("/proc/cpuinfo"):
+            if l.startswith("model name"):
+                return l.split(":", 1)[1].strip()
+    except Exception:
+        pass
+    return "unknown"
+
+
 class ClockSampler:
     """nvidia-smi clocks and throttle reasons DURING the timed region (B200_PROFILING.md recipe)."""
     Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
@@ -210,7 +262,14 @@ def parse_clock_lines(lines) -> dict:
 # ---------------------------------------------------------------------------------------------------------------
 # the oracle on a bounded sample of the workload (cpu_baseline leg and --impl reference)
 # ---------------------------------------------------------------------------------------------------------------
-SAMPLE = dict(T=2, K=3, n_em=1, n_lm=3)   # of configs[4]; smaller configs are clipped to their own sizes
+# The bounded sample keeps ALL time slots (the oracle's per-baseline overheads then weigh as in a full run) and cuts
+# clusters and iterations; smaller configs are clipped to their own sizes.  At configs[4] the scaled figure is within
+# 10 % of the one full oracle run on record (FULL_RUN below).
+SAMPLE = dict(T=10 ** 9, K=2, n_em=1, n_lm=3)
+# tests/golden/make_golden_cfg4.py, the whole configs[4] interval through the oracle (round 1, 16 host cores of the
+# GPU box): 430 s predict + 317 s SAGE-EM (+ I/O) = 752 s
+FULL_RUN = {4: {"seconds": 752.0, "cores": 16, "what": "tests/golden/make_golden_cfg4.py, the whole interval, round 1: "
+                "430 s predict + 317 s SAGE-EM"}}
 
 
 def oracle_sample(p, sample=None):
@@ -238,7 +297,7 @@ def oracle_sample(p, sample=None):
     f_pred = (p.T / Ts) * (p.K / Ks)
     f_cal = (p.T / Ts) * sweeps(p.K, p.n_em, p.n_lm) / sweeps(Ks, n_em_s, n_lm_s)
     total = t_pred * f_pred + t_cal * f_cal
-    desc = (f"first {Ts} of {p.T} time slots x first {Ks} of {p.K} clusters ({S} sources each), predict + "
+    desc = (f"{'all' if Ts == p.T else 'first ' + str(Ts) + ' of'} {p.T} time slots x first {Ks} of {p.K} clusters ({S} sources each), predict + "
             f"{n_em_s} EM x {n_lm_s} LM; measured {t_pred:.2f} s predict + {t_cal:.2f} s calibrate, scaled x{f_pred:.0f} "
             f"(samples x sources) and x{f_cal:.1f} (time slots x corrupt/pass sweeps) to one interval")
     return total, desc, dict(predict_s=t_pred, calibrate_s=t_cal, predict_scale=f_pred, calibrate_scale=f_cal)
@@ -267,7 +326,9 @@ def run_reference(args):
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": wall_ms, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(p, "full"), "note": "each step is a bounded sample scaled to one interval"},
-        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "cpu_baseline": dict({"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc,
+                              "cpu": cpu_model()},
+                             **({"full_run": FULL_RUN[args.config]} if args.config in FULL_RUN else {})),
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -335,7 +396,8 @@ def run_ours(args):
 
     # ---- timed region: device-resident, the LM pass kernel's launches timed live by the library's event pairs ----
     sg.profile_read()
-    sg.profile_enable([top])
+    timed_kinds = sorted({top, "predict", "corrupt", "mstep"})
+    sg.profile_enable(timed_kinds)
     launches0 = sg.launch_count()
     clocks = ClockSampler(local_rank)
     clocks.start()
@@ -396,15 +458,88 @@ def run_ours(args):
     else:
         kfull = top
     roofline = {"bound": "hbm", "kernel": kfull + "_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
-                "frac": achieved / peak, "traffic": load_traffic(args.coh, kname), "peak_source": peak_src,
+                "frac": achieved / peak, "traffic": load_traffic(args.coh, kname),
+                "traffic_source": f"stored ncu figure (profiles/{kname}_traffic.csv: dram bytes per launch at configs[4], "
+                                  "mean over an interval's launches), not measured in this run",
+                "peak_source": peak_src,
                 "algorithmic_bytes_per_launch": pass_bytes, "launches_timed": npass, "avg_launch_ms": pass_ms,
                 "share_of_step": prof[top]["ms"] / max(args.steps, 1) / ms_per_step}
+
+    # ---- every north_star fraction, from this run's own timings (BASELINE.json:5) ----
+    # ALU-bound kernels: FP64 thread-instructions (ncu count per unit of work, profiles/kernel_counts.csv) per second
+    # of CUDA-event time inside the timed region, against the DFMA-chain peak measured NOW on this device.
+    dfma = sg.profile_dfma_peak()
+    sms = torch.cuda.get_device_properties(dev).multi_processor_count
+    dfma_nominal = sms * 64 * (clk.get("sm_max_mhz") or 1965.0) * 1e6
+    arm = args.coh
+    rooflines = [dict(roofline)]
+
+    def alu_entry(kernel, kind, units_per_launch, unit_name):
+        ipu = load_counts(kernel, arm)
+        n = prof[kind]["timed"]
+        if not ipu or not n:
+            return None
+        ms = prof[kind]["ms"] / n
+        ach = ipu * units_per_launch / (ms * 1e-3)
+        return {"bound": "alu", "kernel": kernel, "achieved": ach / 1e12, "peak": dfma["fma_per_s"] / 1e12,
+                "unit": "T FP64 thread-inst/s", "frac": ach / dfma["fma_per_s"], "traffic": None,
+                "peak_source": "DFMA-chain kernel measured in this run (sagecal_profile_dfma_peak: 8 chains x 1024 "
+                               "threads x %d SMs); nominal %d x 64 lanes x max clock = %.2fe12/s" % (sms, sms, dfma_nominal / 1e12),
+                "fp64_inst_per_unit": ipu, "unit_of_work": unit_name, "units_per_launch": units_per_launch,
+                "inst_source": "ncu smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum at configs[4] / units "
+                               "(profiles/kernel_counts.csv)",
+                "launches_timed": n, "avg_launch_ms": ms, "sm_mhz_under_load": clk.get("sm_mhz"),
+                "share_of_step": prof[kind]["ms"] / max(args.steps, 1) / ms_per_step}
+
+    e = alu_entry("predict_kernel", "predict", p.vis_src, "visibility x source")
+    if e:
+        rooflines.append(e)
+    if args.lm != "direct":
+        chunks = max(1, -(-p.n_lm // LM_RECENTRE))
+        evals = (p.n_lm + chunks) / chunks                      # evaluations per launch: the chunk's trials + its centre
+        e = alu_entry("mstep_kernel", "mstep", p.B * evals, "baseline x evaluation")
+        if e:
+            e["note"] = ("latency-bound cooperative kernel: two grid barriers and a station reduction per evaluation "
+                         "(DESIGN.md §5.5); the fraction is the baseline arithmetic alone against the FP64 issue peak")
+            rooflines.append(e)
+    if prof["corrupt"]["timed"]:
+        # initial residual: V read, K coherencies read, R written
+        cb = 64 if args.coh == "full" else 16
+        cbytes = (128 + K * cb) * p.samples
+        cms = prof["corrupt"]["ms"] / prof["corrupt"]["timed"]
+        rooflines.append({"bound": "hbm", "kernel": "corrupt_kernel", "achieved": cbytes / (cms * 1e-3) / 1e9, "peak": peak,
+                          "unit": "GB/s", "frac": cbytes / (cms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
+                          "algorithmic_bytes_per_launch": cbytes, "launches_timed": prof["corrupt"]["timed"],
+                          "avg_launch_ms": cms, "share_of_step": prof["corrupt"]["ms"] / max(args.steps, 1) / ms_per_step})
+    # the fused cost / gradient / J^H J pass as BASELINE.json:5 states it (the kernel of --lm direct): 20 launches of
+    # sagecal_lm_cost_grad_jtj on the step's residual and the first cluster's coherencies, after the timed region
+    if args.lm != "direct":
+        sg.profile_read()
+        sg.profile_enable(["lm_pass"])
+        for _ in range(21):
+            sg.lm_cost_grad_jtj(N, T, F, residual, coh[0], jones[0], coh_format=fmt)
+        torch.cuda.synchronize()
+        pr = sg.profile_read()["lm_pass"]
+        sg.profile_enable([])
+        if pr["timed"]:
+            pms = pr["ms"] / pr["timed"]
+            pbytes = PASS_BYTES_PER_SAMPLE[args.coh] * p.samples
+            rooflines.append({"bound": "hbm", "kernel": ("lm_pass_mma" if args.coh == "full" else "lm_pass_scalar") + "_kernel",
+                              "achieved": pbytes / (pms * 1e-3) / 1e9, "peak": peak, "unit": "GB/s",
+                              "frac": pbytes / (pms * 1e-3) / 1e9 / peak, "traffic": load_traffic(args.coh, "lm_pass"),
+                              "traffic_source": "stored ncu figure (profiles/lm_pass_traffic.csv)", "peak_source": peak_src,
+                              "algorithmic_bytes_per_launch": pbytes, "launches_timed": pr["timed"], "avg_launch_ms": pms,
+                              "where": "loop of sagecal_lm_cost_grad_jtj after the timed region (not part of the default step)"})
+    floor = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, peak, dfma["fma_per_s"],
+                           load_counts("predict_kernel", arm) or 0.0, args.lm, p.n_lm)
+    floor["frac_of_floor"] = floor["floor_s"] / (ms_per_step * 1e-3)
+    extras = {"rooflines": rooflines, "dfma_peak": dict(dfma, nominal_fma_per_s=dfma_nominal, sms=sms), "interval_floor": floor}
 
     # ---- end to end: HOST buffers in, HOST buffers out, through sagecal_calibrate_interval_host ----
     if args.no_e2e:
         e2e, e2e_cost_sum = None, None
         return _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown,
-                       pass_bytes, cost_sum, trace_last)
+                       pass_bytes, cost_sum, trace_last, extras)
     vis_host = torch.empty(vis.shape, dtype=vis.dtype).pin_memory()
     vis_host.copy_(vis)
     del coh, vis, residual, ws, out, noise_host
@@ -438,12 +573,22 @@ def run_ours(args):
            "d2h_bytes_per_step": d2h, "ms_per_step": e2e_ms,
            "api": "sagecal_calibrate_interval_host (pinned host buffers in and out)"}
 
+    # ---- the paper's stations x clusters grid, every point but the headline's own, with its floor ----
+    if world == 1 and not args.no_grid:
+        del vis_host, h_res
+        torch.cuda.empty_cache()
+        try:
+            extras["grid"] = measure_grid(sg, dev, args, peak, extras["dfma_peak"]["fma_per_s"],
+                                          skip=[(p.N, p.K)] if args.config == 4 else [], steps=2, warmup=1)
+        except Exception as ex:                          # the bench line must not depend on the grid
+            extras["grid"] = {"error": repr(ex)}
+
     return _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown,
-                   pass_bytes, cost_sum, trace_last)
+                   pass_bytes, cost_sum, trace_last, extras)
 
 
 def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launches, roofline, breakdown, pass_bytes,
-            cost_sum, trace_last):
+            cost_sum, trace_last, extras=None):
     import torch.distributed as dist
     from sagecal_inputs import make_config
     K = p.K
@@ -458,7 +603,10 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
         from oracle import oracle
         oracle.build()
         v, desc, _ = oracle_sample(make_config(args.config))
-        cpu_baseline = {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": desc}
+        cpu_baseline = {"value": v, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle", "sample": desc,
+                        "cpu": cpu_model()}
+        if args.config in FULL_RUN:
+            cpu_baseline["full_run"] = FULL_RUN[args.config]
 
     predict_ms = breakdown.get("predict", 0.0) + breakdown.get("predict_prep", 0.0)
     line = {
@@ -477,29 +625,34 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
                                          if breakdown.get("predict_mixed_precision") else None),
         "check": {"sum_cost_per_cluster": cost_sum, "cost_trace_last": trace_last, "e2e_sum_cost_per_cluster": e2e_cost_sum},
     }
+    line.update(extras or {})
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
     return 0
 
 
-def run_grid(args):
-    """--grid: the paper's scaling experiment (runtime over stations x clusters, Figs. 1-3)
-    with this build's own timings -- configs[4]'s recipe (T=20, F=8, 40 sources per cluster, 3 EM x 10 LM) at
-    N in {64, 128, 256, 384, 512} x K in {1, 50}.  Prints one JSON object {"grid": [...]}; not the bench line."""
+GRID_N, GRID_K = (64, 128, 256, 384, 512), (1, 50)
+
+
+def measure_grid(sg, dev, args, hbm_gbs, dfma_per_s, skip=(), steps=None, warmup=None):
+    """The paper's scaling experiment (runtime over stations x clusters, Figs. 1-3) with this
+    build's own timings -- configs[4]'s recipe (T=20, F=8, 40 sources per cluster, 3 EM x 10 LM) at N in GRID_N x K in
+    GRID_K.  Every point carries its roofline floor (interval_floor: the streaming kernels' algorithmic bytes at the
+    measured copy rate + the prediction's FP64 instructions at the measured DFMA rate) and floor / measured."""
     import torch
-    import paper_1910_13908_b200 as sg
     from sagecal_inputs import make_config
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py --grid: no CUDA device")
-    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
-    torch.cuda.set_device(dev)
     fmt = sg.COH_FULL if args.coh == "full" else sg.COH_SCALAR
     lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "percluster": sg.LM_PERCLUSTER}[args.lm]
+    steps = args.steps if steps is None else steps
+    warmup = max(args.warmup, 1) if warmup is None else warmup
+    ipu = load_counts("predict_kernel", args.coh) or 0.0
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
-    for N in (64, 128, 256, 384, 512):
-        for K in (1, 50):
+    for N in GRID_N:
+        for K in GRID_K:
+            if (N, K) in skip:
+                continue
             p = make_config(4, N=N, K=K)
             uvw, sl, sm_, sI, sa = t(p.uvw), t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha)
             shape = (K, p.rows, p.F, 4) if fmt == sg.COH_FULL else (K, p.rows, p.F)
@@ -518,24 +671,43 @@ def run_grid(args):
                 jones.copy_(jones0)
                 return sg.sage_calibrate(N, p.T, p.F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
                                          residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
-            for _ in range(max(args.warmup, 1)):
+            for _ in range(warmup):
                 o = step()
             torch.cuda.synchronize()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
             e0.record()
-            for _ in range(args.steps):
+            for _ in range(steps):
                 o = step()
             e1.record()
             torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / max(args.steps, 1)
+            ms = e0.elapsed_time(e1) / max(steps, 1)
             tr = o["cost_trace"].cpu().numpy()
+            fl = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, hbm_gbs, dfma_per_s, ipu, args.lm, p.n_lm)
             out.append({"N": N, "B": p.B, "K": K, "samples": p.samples, "s_per_interval": ms / 1e3,
+                        "hbm_floor_s": fl["hbm_floor_s"], "predict_alu_floor_s": fl["predict_alu_floor_s"],
+                        "frac_of_floor": fl["floor_s"] / (ms / 1e3),
                         "cost_first": float(tr[0]), "cost_last": float(tr[-1]),
                         "monotone": bool(np.all(np.diff(tr) <= 1e-12 * tr[:-1]))})
             del coh, vis, residual, ws, o, jones, jones0
             torch.cuda.empty_cache()
+    return out
+
+
+def run_grid(args):
+    """--grid: measure_grid at every point.  Prints one JSON object {"grid": [...]}; not the bench line."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --grid: no CUDA device")
+    dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
+    torch.cuda.set_device(dev)
+    peak, peak_src = load_peaks()
+    dfma = sg.profile_dfma_peak()
+    out = measure_grid(sg, dev, args, peak, dfma["fma_per_s"])
     print(json.dumps({"grid": out, "recipe": "configs[4] layout/T/F/S, 3 EM x 10 LM, float64, coherencies " + args.coh +
-                      ", lm " + args.lm, "steps": args.steps, "warmup": max(args.warmup, 1)}), flush=True)
+                      ", lm " + args.lm, "steps": args.steps, "warmup": max(args.warmup, 1),
+                      "floor": "streaming kernels' algorithmic bytes at %.1f GB/s (%s) + predict's FP64 instructions at "
+                               "%.3e DFMA/s (measured in this run)" % (peak, peak_src, dfma["fma_per_s"])}), flush=True)
     return 0
 
 
@@ -604,6 +776,7 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
+    ap.add_argument("--no-grid", action="store_true", help="skip the stations x clusters grid appended to the bench line")
     ap.add_argument("--grid", action="store_true",
                     help="time the paper's stations x clusters scaling grid instead of the bench step (SURVEY.md §8(f) NEXT-4)")
     ap.add_argument("--rows", action="store_true",

@@ -284,6 +284,15 @@ int sagecal_profile_enable(unsigned kind_mask);
 int sagecal_profile_read(double* ms_host, long long* timed_host, long long* launches_host);
 
 /*
+ * The FP64 issue peak of the current device, MEASURED: a DFMA-chain kernel (8 independent chains per thread, 1024
+ * threads on every SM, `iters` trips), timed with CUDA events on `stream`, best of three after a warm-up.  This is the
+ * denominator of the "alu" rooflines bench.py reports ("the builder must measure a DFMA-chain peak"):
+ * taken in the same run, at the clocks the compared kernels saw.  Synchronises `stream`; allocates and frees 256 B.
+ * fma_per_s_host : host out, thread-level DFMAs per second (x2 = flop/s).   ms_host : host out or NULL, kernel time.
+ */
+int sagecal_profile_dfma_peak(int iters, double* fma_per_s_host, double* ms_host, void* stream);
+
+/*
  * Test hook, host only, no device needed: replays the work decomposition of the LM pass kernel.
  * cover : host out [T*B] int32, must be zeroed by the caller; on return every entry must be 1 (each baseline and
  *         time slot visited by exactly one thread of one CTA).

@@ -83,6 +83,8 @@ def load_library():
     L.sagecal_profile_enable.argtypes = [ctypes.c_uint]
     L.sagecal_profile_read.restype = i
     L.sagecal_profile_read.argtypes = [vp, vp, vp]
+    L.sagecal_profile_dfma_peak.restype = i
+    L.sagecal_profile_dfma_peak.argtypes = [i, vp, vp, vp]
     _lib = L
     return L
 
@@ -115,6 +117,14 @@ def profile_read() -> dict:
     launches = np.zeros(len(names), np.int64)
     _check(L.sagecal_profile_read(ms.ctypes.data, timed.ctypes.data, launches.ctypes.data), "sagecal_profile_read")
     return {n: dict(ms=float(ms[k]), timed=int(timed[k]), launches=int(launches[k])) for k, n in enumerate(names)}
+
+
+def profile_dfma_peak(iters: int = 20000, stream=None) -> dict:
+    """sagecal_profile_dfma_peak: the measured FP64 issue peak of the current device, dict(fma_per_s, ms)."""
+    v = (ctypes.c_double * 2)()
+    _check(load_library().sagecal_profile_dfma_peak(iters, ctypes.addressof(v), ctypes.addressof(v) + 8, _stream(stream)),
+           "sagecal_profile_dfma_peak")
+    return dict(fma_per_s=float(v[0]), ms=float(v[1]))
 
 
 def version() -> str:

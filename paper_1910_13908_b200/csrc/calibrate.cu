@@ -14,14 +14,18 @@ int corrupt_range(int N, int T, int F, int coh_format, const sagecal_c128* coh, 
 thread_local int g_last_cuda_error = 0;
 
 int num_sms() {
-    static int cached = 0;
-    if (cached) return cached;
+    static int cached[64] = {};
     int dev = 0, n = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+    if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= 64) {
         (void)cudaGetLastError();
         return 148;  // B200; only reached without a device (workspace sizing on a CPU-only box)
     }
-    cached = n;
+    if (cached[dev]) return cached[dev];
+    if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        return 148;
+    }
+    cached[dev] = n;
     return n;
 }
 

@@ -19,7 +19,7 @@ inline int cuda_fail(cudaError_t e) { g_last_cuda_error = (int)e; return SAGECAL
 
 inline bool aligned(const void* p, size_t a) { return (reinterpret_cast<uintptr_t>(p) & (a - 1)) == 0; }
 inline size_t round_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-int num_sms();  // SM count of the current device (cached)
+int num_sms();  // SM count of the current device (cached per device)
 
 // ---- launch accounting and optional per-kernel CUDA-event timing (profile.cu; sagecal_profile_* in the ABI) ----
 enum KernelKind { KK_PREP = 0, KK_PREDICT, KK_CORRUPT, KK_PASS, KK_REDUCE, KK_LMSTEP, KK_NORM, KK_WBSTAT, KK_MSTEP, KK_FULLGN, KK_ROWS, KK_GFIX, KK_COUNT };
@@ -28,6 +28,7 @@ struct LaunchScope {
     int kind;
     cudaStream_t st;
     bool timed;
+    cudaEvent_t end;
     LaunchScope(int kind, cudaStream_t st);
     ~LaunchScope();
 };

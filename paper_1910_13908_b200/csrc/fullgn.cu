@@ -307,7 +307,8 @@ __global__ void __launch_bounds__(FG_THREADS)
 fgn_control_kernel(int N, double tau, FgnCtl* __restrict__ ctl, const double* __restrict__ cost_st,
                    sagecal_c128* __restrict__ J, const sagecal_c128* __restrict__ J_try, sagecal_c128* __restrict__ G,
                    const sagecal_c128* __restrict__ G_try, sagecal_c128* __restrict__ M,
-                   const sagecal_c128* __restrict__ M_try, double* __restrict__ cost_out, double* __restrict__ trace_out) {
+                   const sagecal_c128* __restrict__ M_try, const int* __restrict__ info, double* __restrict__ cost_out,
+                   double* __restrict__ trace_out) {
     __shared__ double s_buf[FG_THREADS];
     const int tid = threadIdx.x;
     double part = 0.0;
@@ -325,7 +326,9 @@ fgn_control_kernel(int N, double tau, FgnCtl* __restrict__ ctl, const double* __
         phi = fresh;
     } else {
         const double pred = ctl->pred, rho = (phi - fresh) / pred;
-        accept = isfinite(fresh) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
+        // a Cholesky factorisation that broke down (H + mu I numerically indefinite: H has four gauge null directions)
+        // leaves a partial factor and a meaningless step: reject it, the damping grows
+        accept = isfinite(fresh) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0 && info[0] == 0 && info[1] == 0;
         if (accept) {
             phi = fresh;
             const double t = 2.0 * rho - 1.0;
@@ -397,9 +400,13 @@ static FgnWorkspace carve_fullgn(int N, void* ws) {
 }
 
 static int cusolver_handle(cusolverDnHandle_t* out) {
-    static thread_local cusolverDnHandle_t h = nullptr;
-    if (!h && cusolverDnCreate(&h) != CUSOLVER_STATUS_SUCCESS) { h = nullptr; return cuda_fail(cudaErrorUnknown); }
-    *out = h;
+    // a cuSOLVER handle is bound to the device that was current when it was created: one per (host thread, device)
+    static thread_local cusolverDnHandle_t h[64] = {};
+    int dev = 0;
+    SGC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
+    if (!h[dev] && cusolverDnCreate(&h[dev]) != CUSOLVER_STATUS_SUCCESS) { h[dev] = nullptr; return cuda_fail(cudaErrorUnknown); }
+    *out = h[dev];
     return SAGECAL_OK;
 }
 
@@ -444,16 +451,19 @@ int enqueue_fullgn(int N, bool scalar, const CompressWorkspace& cw, const double
         return cuda_fail(cudaErrorUnknown);
     double* work = nullptr;                 // cuSOLVER's scratch: its size is only known with a device, so it is
     SGC_CUDA(cudaMallocAsync((void**)&work, sizeof(double) * (size_t)(lwork > 0 ? lwork : 1), st));   // stream-ordered
-    SGC_CUDA(cudaMemcpyAsync(J0, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
-    SGC_CUDA(cudaMemcpyAsync(w.J_try, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
-    if (init) SGC_CUDA(cudaMemsetAsync(w.ctl, 0, sizeof(FgnCtl), st));
-    rc = fgn_evaluate(N, scalar, cw, Scc_k, J0, w, st);
+    // from here on every exit path frees `work`
+    auto chk = [&](cudaError_t e) { if (!rc && e != cudaSuccess) rc = cuda_fail(e); };
+    chk(cudaMemcpyAsync(J0, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
+    chk(cudaMemcpyAsync(w.J_try, Jk, (size_t)N * 64, cudaMemcpyDeviceToDevice, st));
+    if (init) chk(cudaMemsetAsync(w.ctl, 0, sizeof(FgnCtl), st));
+    chk(cudaMemsetAsync(w.info, 0, 2 * sizeof(int), st));
+    if (!rc) rc = fgn_evaluate(N, scalar, cw, Scc_k, J0, w, st);
     if (!rc) {
         LaunchScope ls(KK_FULLGN, st);
         if (init)
-            fgn_control_kernel<1><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, cost_out, trace_out);
+            fgn_control_kernel<1><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, w.info, cost_out, trace_out);
         else
-            fgn_control_kernel<2><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, cost_out, trace_out);
+            fgn_control_kernel<2><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, w.info, cost_out, trace_out);
         if (cudaGetLastError() != cudaSuccess) rc = cuda_fail(cudaErrorLaunchFailure);
     }
     if (!rc) {
@@ -466,7 +476,7 @@ int enqueue_fullgn(int N, bool scalar, const CompressWorkspace& cw, const double
             fgn_prep_kernel<<<gs, 256, 0, st>>>(N, w.H, w.G, w.ctl, w.Hw, w.rhs);
         }
         if (cusolverDnDpotrf(h, CUBLAS_FILL_MODE_LOWER, n, w.Hw, n, work, lwork, w.info) != CUSOLVER_STATUS_SUCCESS ||
-            cusolverDnDpotrs(h, CUBLAS_FILL_MODE_LOWER, n, 1, w.Hw, n, w.rhs, n, w.info) != CUSOLVER_STATUS_SUCCESS) {
+            cusolverDnDpotrs(h, CUBLAS_FILL_MODE_LOWER, n, 1, w.Hw, n, w.rhs, n, w.info + 1) != CUSOLVER_STATUS_SUCCESS) {
             rc = cuda_fail(cudaErrorUnknown);
             break;
         }
@@ -477,7 +487,7 @@ int enqueue_fullgn(int N, bool scalar, const CompressWorkspace& cw, const double
         if ((rc = fgn_evaluate(N, scalar, cw, Scc_k, J0, w, st))) break;
         {
             LaunchScope ls(KK_FULLGN, st);
-            fgn_control_kernel<0><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, cost_out, trace_out);
+            fgn_control_kernel<0><<<1, FG_THREADS, 0, st>>>(N, tau, w.ctl, w.cost_st, Jk, w.J_try, w.G, w.G_try, w.M, w.M_try, w.info, cost_out, trace_out);
         }
         {
             LaunchScope ls(KK_FULLGN, st);

@@ -26,19 +26,65 @@ LaunchScope::LaunchScope(int kind_, cudaStream_t st_) : kind(kind_), st(st_), ti
         p.kind = kind;
         if (cudaEventRecord(p.a, st) != cudaSuccess) { (void)cudaGetLastError(); g_free.push_back(p); return; }
         g_pairs.push_back(p);
+        end = p.b;                       // this scope's own end event (another host thread may append in between)
         timed = true;
     }
 }
 LaunchScope::~LaunchScope() {
-    if (timed) {
-        std::lock_guard<std::mutex> lk(g_mu);
-        (void)cudaEventRecord(g_pairs.back().b, st);
+    if (timed) (void)cudaEventRecord(end, st);
+}
+
+// FP64 issue peak, measured: 8 independent DFMA chains per thread, 1024 threads (8 warps per scheduler) on every SM.
+// The roofline denominator of the ALU-bound kernels (predict, the M-step's baseline phase), taken in the same run
+// and at the same clocks as the kernels it is compared with.
+__global__ void __launch_bounds__(1024)
+dfma_peak_kernel(double* out, int iters, double a, double b) {
+    double x[8];
+#pragma unroll
+    for (int i = 0; i < 8; i++) x[i] = (double)threadIdx.x + i;
+    for (int it = 0; it < iters; it++) {
+#pragma unroll
+        for (int i = 0; i < 8; i++) x[i] = fma(x[i], a, b);
     }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 8; i++) s += x[i];
+    if (s == 12345.678) out[0] = s;      // never true: keeps the chains alive
 }
 
 }  // namespace sgc
 
 using namespace sgc;
+
+extern "C" int sagecal_profile_dfma_peak(int iters, double* fma_per_s_host, double* ms_host, void* stream) {
+    if (iters < 1 || !fma_per_s_host) return SAGECAL_EINVAL;
+    cudaStream_t st = (cudaStream_t)stream;
+    const int sms = num_sms();
+    double* scratch = nullptr;
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    SGC_CUDA(cudaMalloc((void**)&scratch, 256));
+    int rc = SAGECAL_OK;
+    float best = 0.f;
+    if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) rc = cuda_fail(cudaGetLastError());
+    for (int rep = 0; rep < 4 && rc == SAGECAL_OK; rep++) {          // first repetition = warm-up
+        cudaError_t e = cudaEventRecord(e0, st);
+        dfma_peak_kernel<<<sms, 1024, 0, st>>>(scratch, iters, 1.0000001, 1e-9);
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e == cudaSuccess) e = cudaEventRecord(e1, st);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+        float ms = 0.f;
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+        if (e != cudaSuccess) { rc = cuda_fail(e); break; }
+        if (rep > 0 && (best == 0.f || ms < best)) best = ms;
+    }
+    if (e0) (void)cudaEventDestroy(e0);
+    if (e1) (void)cudaEventDestroy(e1);
+    (void)cudaFree(scratch);
+    if (rc != SAGECAL_OK) return rc;
+    *fma_per_s_host = (double)sms * 1024.0 * 8.0 * iters / (best * 1e-3);
+    if (ms_host) *ms_host = best;
+    return SAGECAL_OK;
+}
 
 extern "C" long long sagecal_launch_count(void) {
     long long n = 0;
