@@ -211,9 +211,13 @@ int sagecal_sage_calibrate(
 /*
  * Whole-interval convenience entry with HOST buffers (used for end-to-end timing): copies uvw, the source table,
  * the visibilities and the start Jones to the device, runs predict + calibrate, copies Jones, residual and costs
- * back.  Allocates and frees its own device memory (cudaMallocAsync on `stream`) and synchronises `stream` before
- * returning.  All array pointers are host pointers (pinned memory recommended).  residual_host / cost_trace_host
- * may be NULL (not copied back).
+ * back.  Allocates and frees its own device memory, stream-ordered on `stream`, from a PRIVATE memory pool the library
+ * creates once per (host thread, device) and whose blocks it keeps between calls (the arena, about 70 GB at
+ * configs[4], stays reserved until the process ends; the device's default pool and its attributes are not touched).
+ * The visibilities travel on an internal copy stream while the coherencies are predicted, and the last write-back runs
+ * in ranges of time slots whose copies to the host overlap the next range's kernel.  Synchronises `stream` and the
+ * copy stream before returning.  All array pointers are host pointers (pinned memory recommended: pageable memory
+ * serialises the copies).  residual_host / cost_trace_host may be NULL (not copied back).
  */
 int sagecal_calibrate_interval_host(
     int nstations, int ntime, int nchan,

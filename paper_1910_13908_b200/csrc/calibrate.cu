@@ -248,10 +248,15 @@ extern "C" size_t sagecal_workspace_bytes(int what, int N, int T, int F, int K) 
     }
 }
 
-extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_c128* vis, int coh_format,
-                                      const sagecal_c128* coh, sagecal_c128* jones, sagecal_c128* residual, int n_em,
-                                      int n_lm, double tau, int lm_mode, double* cost_per_cluster, double* cost_trace,
-                                      void* workspace, size_t workspace_bytes, void* stream) {
+// The residual is final time slot by time slot once the last write-back has passed: the host entry asks for that
+// write-back in `final_chunks` ranges of time slots and is told after each (it starts the range's copy to the host on
+// another stream while the next range is written).  The device entry runs it as one launch.
+typedef int (*FinalChunkFn)(void* ctx, int t0, int t1);
+static int sage_calibrate_core(int N, int T, int F, int K, const sagecal_c128* vis, int coh_format,
+                               const sagecal_c128* coh, sagecal_c128* jones, sagecal_c128* residual, int n_em,
+                               int n_lm, double tau, int lm_mode, double* cost_per_cluster, double* cost_trace,
+                               void* workspace, size_t workspace_bytes, void* stream, int final_chunks,
+                               FinalChunkFn after_chunk, void* after_ctx) {
     if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
     if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT && lm_mode != SAGECAL_LM_FULLGN && lm_mode != SAGECAL_LM_PERCLUSTER) return SAGECAL_EINVAL;
@@ -271,6 +276,11 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     const int64_t samples = (int64_t)T * g.B * F;
     const size_t cstride = scalar ? (size_t)samples : (size_t)samples * 4;
     int rc;
+    if (final_chunks < 1) final_chunks = 1;
+    if (final_chunks > T) final_chunks = T;
+    const int tchunk = (T + final_chunks - 1) / final_chunks;
+    const size_t rows_slot = (size_t)g.B * F;                 // samples per time slot
+    auto whole = [&]() { return after_chunk ? after_chunk(after_ctx, 0, T) : SAGECAL_OK; };
 
     // R = V - sum_k J_k C_k J_k^H
     if (K > 0) {
@@ -290,7 +300,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
             SGC_LAUNCH_CHECK();
         }
     }
-    if (K == 0 || n_em == 0) return SAGECAL_OK;
+    if (K == 0 || n_em == 0) return whole();
 
     if (lm_mode == SAGECAL_LM_DIRECT) {
         // every LM evaluation streams the T*F samples of the cluster (rows 8a-3, 8a-4, 8a-6 as written)
@@ -313,7 +323,7 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                 if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, k, k + 1, -1.0, residual, residual, st))) return rc;
             }
         }
-        return SAGECAL_OK;
+        return whole();
     }
 
     // compressed mode: `residual` always holds R; per (em, k) one streaming kernel writes back the
@@ -355,7 +365,14 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
         }
         // last write-back: the group solved last
         const sagecal_c128* J0prev = w.cw.J0G + (size_t)(par ^ 1) * GRP * N * 4;
-        return enqueue_wbgroup(N, T, F, coh_format, residual, coh, cstride, kp0, gp, J0prev, jones, 0, 0, w.cw.SrcG, nullptr, nullptr, st);
+        for (int t0 = 0; t0 < T; t0 += tchunk) {
+            const int t1 = t0 + tchunk < T ? t0 + tchunk : T;
+            const size_t off = (size_t)t0 * rows_slot;
+            if ((rc = enqueue_wbgroup(N, t1 - t0, F, coh_format, residual + off * 4, coh + off * (scalar ? 1 : 4), cstride, kp0, gp,
+                                      J0prev, jones, 0, 0, w.cw.SrcG, nullptr, nullptr, st))) return rc;
+            if (after_chunk && (rc = after_chunk(after_ctx, t0, t1))) return rc;
+        }
+        return SAGECAL_OK;
     }
 
     // cluster by cluster: SAGECAL_LM_PERCLUSTER, SAGECAL_LM_FULLGN, and compressed M-steps longer than one chunk
@@ -390,8 +407,77 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
     // last write-back: R -= dW c of the cluster solved last
     {
         const sagecal_c128* J0prev = w.cw.J0 + (size_t)(par ^ 1) * N * 4;
-        if ((rc = enqueue_wbstat(N, T, F, coh_format, residual, Cprev, J0prev, Jprev, nullptr, w.cw.Src, nullptr, st))) return rc;
+        for (int t0 = 0; t0 < T; t0 += tchunk) {
+            const int t1 = t0 + tchunk < T ? t0 + tchunk : T;
+            const size_t off = (size_t)t0 * rows_slot;
+            if ((rc = enqueue_wbstat(N, t1 - t0, F, coh_format, residual + off * 4, Cprev ? Cprev + off * (scalar ? 1 : 4) : nullptr,
+                                     J0prev, Jprev, nullptr, w.cw.Src, nullptr, st))) return rc;
+            if (after_chunk && (rc = after_chunk(after_ctx, t0, t1))) return rc;
+        }
     }
+    return SAGECAL_OK;
+}
+
+extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_c128* vis, int coh_format,
+                                      const sagecal_c128* coh, sagecal_c128* jones, sagecal_c128* residual, int n_em,
+                                      int n_lm, double tau, int lm_mode, double* cost_per_cluster, double* cost_trace,
+                                      void* workspace, size_t workspace_bytes, void* stream) {
+    return sage_calibrate_core(N, T, F, K, vis, coh_format, coh, jones, residual, n_em, n_lm, tau, lm_mode,
+                               cost_per_cluster, cost_trace, workspace, workspace_bytes, stream, 1, nullptr, nullptr);
+}
+
+// Per (host thread, device) helpers of the host entry, created once: a PRIVATE memory pool that keeps the arena between
+// calls (intervals arrive back to back; the device's default pool and its release threshold are left alone), the copy
+// stream and the events that order it against the caller's stream.
+constexpr int HOST_FINAL_CHUNKS = 7;
+struct HostCtx {
+    bool ready = false;
+    cudaMemPool_t pool = nullptr;
+    cudaStream_t cs = nullptr;
+    cudaEvent_t ev_alloc = nullptr, ev_vis = nullptr, ev_chunk[HOST_FINAL_CHUNKS + 1] = {};
+};
+static int host_ctx(HostCtx** out) {
+    static thread_local HostCtx ctx[64];
+    int dev = 0;
+    SGC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
+    HostCtx& c = ctx[dev];
+    if (!c.ready) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        SGC_CUDA(cudaMemPoolCreate(&c.pool, &props));
+        uint64_t keep = UINT64_MAX;
+        SGC_CUDA(cudaMemPoolSetAttribute(c.pool, cudaMemPoolAttrReleaseThreshold, &keep));
+        SGC_CUDA(cudaStreamCreateWithFlags(&c.cs, cudaStreamNonBlocking));
+        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_alloc, cudaEventDisableTiming));
+        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_vis, cudaEventDisableTiming));
+        for (int i = 0; i <= HOST_FINAL_CHUNKS; i++) SGC_CUDA(cudaEventCreateWithFlags(&c.ev_chunk[i], cudaEventDisableTiming));
+        c.ready = true;
+    }
+    *out = &c;
+    return SAGECAL_OK;
+}
+// after a range of time slots of the residual is final: its copy to the host starts on the copy stream
+struct HostFinal {
+    HostCtx* c;
+    cudaStream_t st;
+    const char* dev_res;
+    char* host_res;
+    size_t bytes_slot;
+    int n;
+};
+static int host_final_chunk(void* ctx, int t0, int t1) {
+    HostFinal* h = (HostFinal*)ctx;
+    if (!h->host_res) return SAGECAL_OK;
+    cudaEvent_t ev = h->c->ev_chunk[h->n < HOST_FINAL_CHUNKS ? h->n : HOST_FINAL_CHUNKS];
+    h->n++;
+    SGC_CUDA(cudaEventRecord(ev, h->st));
+    SGC_CUDA(cudaStreamWaitEvent(h->c->cs, ev, 0));
+    SGC_CUDA(cudaMemcpyAsync(h->host_res + (size_t)t0 * h->bytes_slot, h->dev_res + (size_t)t0 * h->bytes_slot,
+                             (size_t)(t1 - t0) * h->bytes_slot, cudaMemcpyDeviceToHost, h->c->cs));
     return SAGECAL_OK;
 }
 
@@ -427,16 +513,10 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
                  o_coh = take(coh_bytes), o_jon = take((size_t)K * N * 64), o_cpc = take(sizeof(double) * K),
                  o_trc = take(sizeof(double) * ntrace), o_wsp = take(ws_pred), o_wsc = take(ws_cal);
     char* arena = nullptr;
-    {   // keep the arena in the device's default pool between calls (intervals arrive back to back)
-        int dev = 0;
-        cudaMemPool_t pool;
-        SGC_CUDA(cudaGetDevice(&dev));
-        SGC_CUDA(cudaDeviceGetDefaultMemPool(&pool, dev));
-        uint64_t keep = UINT64_MAX;
-        SGC_CUDA(cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep));
-    }
-    SGC_CUDA(cudaMallocAsync((void**)&arena, off, st));
-    int rc = SAGECAL_OK;
+    HostCtx* hc = nullptr;
+    int rc = host_ctx(&hc);
+    if (rc) return rc;
+    SGC_CUDA(cudaMallocFromPoolAsync((void**)&arena, off, hc->pool, st));
     auto h2d_on = [&](cudaStream_t s, size_t o, const void* src, size_t n) {
         if (rc == SAGECAL_OK && src && n) {
             cudaError_t e = cudaMemcpyAsync(arena + o, src, n, cudaMemcpyHostToDevice, s);
@@ -446,13 +526,8 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     auto h2d = [&](size_t o, const void* src, size_t n) { h2d_on(st, o, src, n); };
     // the visibilities (the bulk of the input) travel on a second stream while `st` predicts the coherencies,
     // which need only uvw and the source table; `st` joins before the calibration reads them
-    cudaStream_t cs = nullptr;
-    cudaEvent_t ev_alloc = nullptr, ev_vis = nullptr;
-    if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess ||
-        cudaEventCreateWithFlags(&ev_alloc, cudaEventDisableTiming) != cudaSuccess ||
-        cudaEventCreateWithFlags(&ev_vis, cudaEventDisableTiming) != cudaSuccess) {
-        rc = cuda_fail(cudaGetLastError());
-    }
+    cudaStream_t cs = hc->cs;
+    cudaEvent_t ev_alloc = hc->ev_alloc, ev_vis = hc->ev_vis;
     if (rc == SAGECAL_OK) {
         cudaError_t e = cudaEventRecord(ev_alloc, st);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_alloc, 0);
@@ -482,11 +557,14 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
         cudaError_t e = cudaStreamWaitEvent(st, ev_vis, 0);
         if (e != cudaSuccess) rc = cuda_fail(e);
     }
+    // the last write-back runs in ranges of time slots; each range's copy to the host overlaps the next range's kernel
+    HostFinal hf = {hc, st, arena + o_res, (char*)residual_host, (size_t)B * F * 64, 0};
     if (rc == SAGECAL_OK)
-        rc = sagecal_sage_calibrate(N, T, F, K, (const sagecal_c128*)(arena + o_vis), coh_format,
-                                    (const sagecal_c128*)(arena + o_coh), (sagecal_c128*)(arena + o_jon),
-                                    (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, lm_mode, (double*)(arena + o_cpc),
-                                    cost_trace_host ? (double*)(arena + o_trc) : nullptr, arena + o_wsc, ws_cal, st);
+        rc = sage_calibrate_core(N, T, F, K, (const sagecal_c128*)(arena + o_vis), coh_format,
+                                 (const sagecal_c128*)(arena + o_coh), (sagecal_c128*)(arena + o_jon),
+                                 (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, lm_mode, (double*)(arena + o_cpc),
+                                 cost_trace_host ? (double*)(arena + o_trc) : nullptr, arena + o_wsc, ws_cal, st,
+                                 HOST_FINAL_CHUNKS, host_final_chunk, &hf);
     auto d2h = [&](void* dst, size_t o, size_t n) {
         if (rc == SAGECAL_OK && dst && n) {
             cudaError_t e = cudaMemcpyAsync(dst, arena + o, n, cudaMemcpyDeviceToHost, st);
@@ -494,15 +572,14 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
         }
     };
     d2h(jones_host, o_jon, (size_t)K * N * 64);
-    d2h(residual_host, o_res, vis_bytes);
     d2h(cost_per_cluster_host, o_cpc, sizeof(double) * K);
     d2h(cost_trace_host, o_trc, sizeof(double) * ntrace);
-    if (cs) (void)cudaStreamSynchronize(cs);      // on an error path the copy may still be in flight
+    // the residual's copies (and, on an error path, the visibilities') are on the copy stream: the arena is freed on
+    // `st` only after they are done
+    cudaError_t e0 = cudaStreamSynchronize(cs);
     cudaError_t e1 = cudaFreeAsync(arena, st);
     cudaError_t e2 = cudaStreamSynchronize(st);
-    if (ev_alloc) (void)cudaEventDestroy(ev_alloc);
-    if (ev_vis) (void)cudaEventDestroy(ev_vis);
-    if (cs) (void)cudaStreamDestroy(cs);
+    if (rc == SAGECAL_OK && e0 != cudaSuccess) rc = cuda_fail(e0);
     if (rc == SAGECAL_OK && e1 != cudaSuccess) rc = cuda_fail(e1);
     if (rc == SAGECAL_OK && e2 != cudaSuccess) rc = cuda_fail(e2);
     return rc;
