@@ -133,10 +133,11 @@ def test_pass_errors(cuda_device):
 
 def test_lm_pass_full_size_tensor_core_form(cuda_device):
     """sagecal_lm_cost_grad_jtj at configs[4]'s shape (N=512, T=20, F=8) with general 2x2 (polarised) coherencies: the
-    launch configuration of bench.py --lm direct, tensor-core form with the F = 8 fast path.  The oracle cannot run
-    130 816 baselines inside a test, so: gradient and J^H J of sampled stations against the definition evaluated by
-    the oracle's coherencies and plain numpy on those stations' 511 baselines (1e-10), and the cost against
-    ||x - J_p C J_q^H||^2 of the residual the corrupt kernel leaves (an independent kernel)."""
+    launch configuration of bench.py --lm direct, tensor-core form with the F = 8 fast path.  Against the oracle on
+    the whole array (one cluster: its own prediction of all 20.9 M samples, then one oracle_cost_grad_jtj pass): the
+    cost and the gradient and J^H J of ALL 512 stations to 1e-10; and, independently of the oracle's pass routine,
+    gradient and J^H J of sampled stations against the definition written out in numpy on those stations' 511
+    baselines."""
     import torch
     import paper_1910_13908_b200 as sg
     from sagecal_inputs import baseline_index, make_config
@@ -150,9 +151,14 @@ def test_lm_pass_full_size_tensor_core_form(cuda_device):
     J = (np.eye(2) + 0.2 * (rng.standard_normal((N, 2, 2)) + 1j * rng.standard_normal((N, 2, 2)))).astype(np.complex128)
     Jd = dev(J)
     cost, grad, jtj = sg.lm_cost_grad_jtj(N, T, F, V, coh_d[0], Jd)
-    res = sg.corrupt_subtract(N, T, F, coh_d, Jd.reshape(1, N, 2, 2), V, sign=-1.0)
-    r2 = float((res.abs() ** 2).sum())
-    assert abs(float(cost[0]) - r2) <= 1e-11 * r2
+    C_or = oracle.predict(p)[0]                                               # the oracle's coherencies, all rows
+    assert rel_l2(host(coh_d[0]), C_or) < 1e-10
+    cost_o, G_o, M_o = oracle.cost_grad_jtj(N, T, F, host(V), C_or, J)
+    assert abs(float(cost[0]) - cost_o) <= 1e-10 * cost_o
+    assert rel_l2(host(grad), G_o) < 1e-10 and rel_l2(host(jtj), M_o) < 1e-10
+    gs, ms = np.abs(G_o).max(), np.abs(M_o).max()
+    assert np.abs(host(grad) - G_o).max() <= 1e-10 * gs and np.abs(host(jtj) - M_o).max() <= 1e-10 * ms
+    del C_or
     for s in (0, 255, 511):
         others = [o for o in range(N) if o != s]
         bl = np.array([baseline_index(N, min(s, o), max(s, o)) for o in others])
@@ -175,5 +181,5 @@ def test_lm_pass_full_size_tensor_core_form(cuda_device):
                 M += np.einsum("nji,njk->ik", T1.conj(), T1)
         assert rel_l2(host(grad[s]), G) < 1e-10, s
         assert rel_l2(host(jtj[s]), M) < 1e-10, s
-    del coh_d, V, res
+    del coh_d, V
     torch.cuda.empty_cache()
