@@ -165,13 +165,15 @@ def load_counts(kernel: str, arm: str):
     return None
 
 
-def stream_bytes_per_interval(samples: int, K: int, n_em: int, coh: str, lm: str = "compressed", n_lm: int = 10) -> int:
+def stream_bytes_per_interval(samples: int, K: int, n_em: int, coh: str, lm: str = "compressed", n_lm: int = 10,
+                              fused: bool = False) -> int:
     """Algorithmic HBM bytes of the streaming kernels of one interval: the initial residual reads V and
     all K coherencies and writes R ((2 + K) x 64 B per sample; 16 B per scalar coherency), then the write-back /
     statistics launches (cluster groups: wbgroup_bytes_per_sample; cluster by cluster: 256 / 160 B per sample and
     launch but the first and last; direct: 128 / 80 B per pass plus add-back and write-back)."""
     cb = 64 if coh == "full" else 16
-    init = (128 + K * cb) * samples
+    # fused route (sagecal_predict_residual): the prediction leaves the initial residual, no pass over the coherencies
+    init = 0 if fused else (128 + K * cb) * samples
     if K == 0 or n_em == 0:
         return init
     if uses_groups(lm, coh, n_lm):
@@ -183,13 +185,18 @@ def stream_bytes_per_interval(samples: int, K: int, n_em: int, coh: str, lm: str
 
 
 def interval_floor(samples: int, vis_src: int, K: int, n_em: int, coh: str, hbm_gbs: float, dfma_per_s: float,
-                   predict_inst_per_vis_src: float, lm: str = "compressed", n_lm: int = 10) -> dict:
+                   predict_inst_per_vis_src: float, lm: str = "compressed", n_lm: int = 10, fused: bool = False) -> dict:
     """Roofline floor of one interval: the streaming kernels' algorithmic bytes at the measured copy rate plus the
-    prediction's FP64 instructions at the measured DFMA rate (the M-step and the small kernels count as overhead)."""
-    b = stream_bytes_per_interval(samples, K, n_em, coh, lm, n_lm)
+    prediction's FP64 instructions at the measured DFMA rate -- or, if larger, the bytes the prediction itself moves
+    (K coherencies written; fused route: V read and R written as well) -- the M-step and the small kernels count as
+    overhead."""
+    b = stream_bytes_per_interval(samples, K, n_em, coh, lm, n_lm, fused)
     hbm_s = b / (hbm_gbs * 1e9)
     alu_s = vis_src * predict_inst_per_vis_src / dfma_per_s if dfma_per_s and predict_inst_per_vis_src else 0.0
-    return {"stream_bytes": int(b), "hbm_floor_s": hbm_s, "predict_alu_floor_s": alu_s, "floor_s": hbm_s + alu_s}
+    pbytes = (K * (64 if coh == "full" else 16) + (128 if fused else 0)) * samples
+    pred_s = max(alu_s, pbytes / (hbm_gbs * 1e9))
+    return {"stream_bytes": int(b), "hbm_floor_s": hbm_s, "predict_alu_floor_s": alu_s, "predict_floor_s": pred_s,
+            "floor_s": hbm_s + pred_s}
 
 
 def cpu_model() -> str:
@@ -266,10 +273,11 @@ def parse_clock_lines(lines) -> dict:
 # clusters and iterations; smaller configs are clipped to their own sizes.  At configs[4] the scaled figure is within
 # 10 % of the one full oracle run on record (FULL_RUN below).
 SAMPLE = dict(T=10 ** 9, K=2, n_em=1, n_lm=3)
-# tests/golden/make_golden_cfg4.py, the whole configs[4] interval through the oracle (round 1, 16 host cores of the
-# GPU box): 430 s predict + 317 s SAGE-EM (+ I/O) = 752 s
-FULL_RUN = {4: {"seconds": 752.0, "cores": 16, "what": "tests/golden/make_golden_cfg4.py, the whole interval, round 1: "
-                "430 s predict + 317 s SAGE-EM"}}
+# tests/golden/make_golden_full.py cfg4, the whole configs[4] interval through the oracle on the 16 host cores of the
+# GPU box (round 2; the times are in tests/golden/cfg4_oracle.txt): 432 s predict + 317 s SAGE-EM (+ simulate) = 754 s;
+# the round-1 run took 752 s
+FULL_RUN = {4: {"seconds": 754.0, "cores": 16, "what": "tests/golden/make_golden_full.py cfg4, the whole interval: "
+                "432 s predict + 317 s SAGE-EM (host_seconds_* in tests/golden/cfg4_oracle.txt)"}}
 
 
 def oracle_sample(p, sample=None):
@@ -380,9 +388,18 @@ def run_ours(args):
     ws = torch.empty(sg.workspace_bytes(3 if args.lm == "fullgn" else 2, N, T, F, K), dtype=torch.uint8, device=dev)
 
     def step():
-        predict()
+        # --fused: sagecal_predict_residual, the prediction of all K clusters also leaves R = V - sum_k J_k C_k J_k^H (rows
+        # 8a-0 .. 8a-2 in one pass) and sagecal_sage_calibrate(vis = NULL) starts from it.  Measured SLOWER than the two
+        # separate calls at configs[4] (51.3 ms against 31.5 + 11.7: the residual tile in shared memory leaves 8 warps
+        # per SM where the prediction wants 24), so it is not the default.
         jones.copy_(jones0)
-        return sg.sage_calibrate(N, T, F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+        if not args.fused:
+            predict()
+            return sg.sage_calibrate(N, T, F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+                                     residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
+        sg.predict_residual(N, T, p.freqs, p.f0, uvw, p.cluster_offset, sl, sm_, sI, sa, jones, vis, coh_format=fmt,
+                            out=coh, residual=residual)
+        return sg.sage_calibrate(N, T, F, None, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
                                  residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
 
     def barrier():
@@ -471,7 +488,8 @@ def run_ours(args):
     dfma = sg.profile_dfma_peak()
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     dfma_nominal = sms * 64 * (clk.get("sm_max_mhz") or 1965.0) * 1e6
-    arm = args.coh
+    fused = args.fused
+    arm = args.coh + ("_resid" if fused else "")
     rooflines = [dict(roofline)]
 
     def alu_entry(kernel, kind, units_per_launch, unit_name):
@@ -493,24 +511,41 @@ def run_ours(args):
 
     e = alu_entry("predict_kernel", "predict", p.vis_src, "visibility x source")
     if e:
+        if fused:
+            e["note"] = ("RESID arm (sagecal_predict_residual): predicts all K clusters of its rows and leaves the initial "
+                         "residual R = V - sum_k J_k C_k J_k^H, so no corrupt_kernel launch is in the step")
         rooflines.append(e)
     if args.lm != "direct":
         chunks = max(1, -(-p.n_lm // LM_RECENTRE))
         evals = (p.n_lm + chunks) / chunks                      # evaluations per launch: the chunk's trials + its centre
+        arm = args.coh
         e = alu_entry("mstep_kernel", "mstep", p.B * evals, "baseline x evaluation")
         if e:
             e["note"] = ("latency-bound cooperative kernel: two grid barriers and a station reduction per evaluation "
                          "(DESIGN.md §5.5); the fraction is the baseline arithmetic alone against the FP64 issue peak")
             rooflines.append(e)
-    if prof["corrupt"]["timed"]:
-        # initial residual: V read, K coherencies read, R written
+    cor = prof["corrupt"]
+    if not cor["timed"]:
+        # fused route: the step has no residual pass of its own; BASELINE.json:5 item (c)'s kernel is timed on its own
+        # here (sagecal_corrupt_subtract over all K clusters), after the timed region
+        sg.profile_read()
+        sg.profile_enable(["corrupt"])
+        for _ in range(4):
+            sg.corrupt_subtract(N, T, F, coh, jones, vis, sign=-1.0, coh_format=fmt, out=residual)
+        torch.cuda.synchronize()
+        cor = sg.profile_read()["corrupt"]
+        sg.profile_enable([])
+    if cor["timed"]:
+        # residual pass: V read, K coherencies read, R written
         cb = 64 if args.coh == "full" else 16
         cbytes = (128 + K * cb) * p.samples
-        cms = prof["corrupt"]["ms"] / prof["corrupt"]["timed"]
+        cms = cor["ms"] / cor["timed"]
         rooflines.append({"bound": "hbm", "kernel": "corrupt_kernel", "achieved": cbytes / (cms * 1e-3) / 1e9, "peak": peak,
                           "unit": "GB/s", "frac": cbytes / (cms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
-                          "algorithmic_bytes_per_launch": cbytes, "launches_timed": prof["corrupt"]["timed"],
-                          "avg_launch_ms": cms, "share_of_step": prof["corrupt"]["ms"] / max(args.steps, 1) / ms_per_step})
+                          "algorithmic_bytes_per_launch": cbytes, "launches_timed": cor["timed"], "avg_launch_ms": cms,
+                          "where": "inside the timed region" if prof["corrupt"]["timed"] else
+                                   "sagecal_corrupt_subtract over all K clusters after the timed region (the step's own "
+                                   "initial residual is fused into the prediction)"})
     # the fused cost / gradient / J^H J pass as BASELINE.json:5 states it (the kernel of --lm direct): 20 launches of
     # sagecal_lm_cost_grad_jtj on the step's residual and the first cluster's coherencies, after the timed region
     if args.lm != "direct":
@@ -530,8 +565,9 @@ def run_ours(args):
                               "traffic_source": "stored ncu figure (profiles/lm_pass_traffic.csv)", "peak_source": peak_src,
                               "algorithmic_bytes_per_launch": pbytes, "launches_timed": pr["timed"], "avg_launch_ms": pms,
                               "where": "loop of sagecal_lm_cost_grad_jtj after the timed region (not part of the default step)"})
+    pred_arm = args.coh + ("_resid" if fused else "")
     floor = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, peak, dfma["fma_per_s"],
-                           load_counts("predict_kernel", arm) or 0.0, args.lm, p.n_lm)
+                           load_counts("predict_kernel", pred_arm) or 0.0, args.lm, p.n_lm, fused)
     floor["frac_of_floor"] = floor["floor_s"] / (ms_per_step * 1e-3)
     extras = {"rooflines": rooflines, "dfma_peak": dict(dfma, nominal_fma_per_s=dfma_nominal, sms=sms), "interval_floor": floor}
 
@@ -617,7 +653,8 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
                    "l2": "inputs larger than L2 (per-pass working set %.2f GB vs 126 MB)" % (pass_bytes / 1e9),
                    "seed": p.seed},
         "clocks": clk, "e2e": e2e, "gpu_launches": int(gpu_launches),
-        "gpu_launches_expected": args.steps * expected_launches(K, p.n_em, p.n_lm, True, args.lm, args.coh),
+        "gpu_launches_expected": args.steps * (expected_launches(K, p.n_em, p.n_lm, True, args.lm, args.coh)
+                                               - (1 if args.fused else 0)),
         "roofline": roofline, "cpu_baseline": cpu_baseline,
         "breakdown_ms_one_step": breakdown,
         "predict_gvis_src_per_s": p.vis_src / (predict_ms * 1e-3) / 1e9 if predict_ms > 0 else None,
@@ -646,7 +683,8 @@ def measure_grid(sg, dev, args, hbm_gbs, dfma_per_s, skip=(), steps=None, warmup
     lm_mode = {"compressed": sg.LM_COMPRESSED, "direct": sg.LM_DIRECT, "fullgn": sg.LM_FULLGN, "percluster": sg.LM_PERCLUSTER}[args.lm]
     steps = args.steps if steps is None else steps
     warmup = max(args.warmup, 1) if warmup is None else warmup
-    ipu = load_counts("predict_kernel", args.coh) or 0.0
+    fused = args.fused
+    ipu = load_counts("predict_kernel", args.coh + ("_resid" if fused else "")) or 0.0
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
     for N in GRID_N:
@@ -667,9 +705,14 @@ def measure_grid(sg, dev, args, hbm_gbs, dfma_per_s, skip=(), steps=None, warmup
             ws = torch.empty(sg.workspace_bytes(3 if args.lm == "fullgn" else 2, N, p.T, p.F, K), dtype=torch.uint8, device=dev)
 
             def step():
-                predict()
                 jones.copy_(jones0)
-                return sg.sage_calibrate(N, p.T, p.F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+                if not fused:
+                    predict()
+                    return sg.sage_calibrate(N, p.T, p.F, vis, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
+                                             residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
+                sg.predict_residual(N, p.T, p.freqs, p.f0, uvw, p.cluster_offset, sl, sm_, sI, sa, jones, vis,
+                                    coh_format=fmt, out=coh, residual=residual)
+                return sg.sage_calibrate(N, p.T, p.F, None, coh, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt,
                                          residual=residual, trace=True, workspace=ws, lm_mode=lm_mode)
             for _ in range(warmup):
                 o = step()
@@ -682,9 +725,9 @@ def measure_grid(sg, dev, args, hbm_gbs, dfma_per_s, skip=(), steps=None, warmup
             torch.cuda.synchronize()
             ms = e0.elapsed_time(e1) / max(steps, 1)
             tr = o["cost_trace"].cpu().numpy()
-            fl = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, hbm_gbs, dfma_per_s, ipu, args.lm, p.n_lm)
+            fl = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, hbm_gbs, dfma_per_s, ipu, args.lm, p.n_lm, fused)
             out.append({"N": N, "B": p.B, "K": K, "samples": p.samples, "s_per_interval": ms / 1e3,
-                        "hbm_floor_s": fl["hbm_floor_s"], "predict_alu_floor_s": fl["predict_alu_floor_s"],
+                        "hbm_floor_s": fl["hbm_floor_s"], "predict_floor_s": fl["predict_floor_s"],
                         "frac_of_floor": fl["floor_s"] / (ms / 1e3),
                         "cost_first": float(tr[0]), "cost_last": float(tr[-1]),
                         "monotone": bool(np.all(np.diff(tr) <= 1e-12 * tr[:-1]))})
@@ -776,6 +819,8 @@ def main(argv=None):
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs only)")
+    ap.add_argument("--fused", action="store_true",
+                    help="prediction fused with the initial residual (sagecal_predict_residual) instead of two calls")
     ap.add_argument("--no-grid", action="store_true", help="skip the stations x clusters grid appended to the bench line")
     ap.add_argument("--grid", action="store_true",
                     help="time the paper's stations x clusters scaling grid instead of the bench step (SURVEY.md §8(f) NEXT-4)")

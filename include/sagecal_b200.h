@@ -134,6 +134,33 @@ int sagecal_predict_coherencies(
     void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * Prediction fused with the initial residual (rows 8a-0 .. 8a-2 of SURVEY.md §8(a) in one pass; BASELINE.json:5 "the
+ * Jones-corrupted residual V_pq - J_p C_pq J_q^H ... with the other clusters' J_p C J_q^H subtracted"):
+ *
+ *   coh[k]   = sagecal_predict_coherencies' C_k for every cluster (same arithmetic, float64, bit-identical)
+ *   residual = vis - sum_k J_{k,p} C_k J_{k,q}^H                      (clusters subtracted in index order)
+ *
+ * One CTA predicts ALL clusters of its 128 rows and carries the rows' residual in shared memory, so the K
+ * coherencies are not read back for the initial residual (69.7 GB at configs[4]).  Follow with
+ * sagecal_sage_calibrate(vis = NULL): it then starts from this residual.
+ * Arguments as sagecal_predict_coherencies (precision is float64), plus
+ * jones    : dev [K][N][4] start Jones (read only).   vis : dev [rows][F][4] (read only).
+ * residual : dev out [rows][F][4]; must not alias vis.
+ * Errors as sagecal_predict_coherencies; SAGECAL_EINVAL also for nclus < 1 or a NULL / misaligned jones, vis, residual.
+ */
+int sagecal_predict_residual(
+    int nstations, int ntime, int nchan,
+    const double* freqs_host, double f0,
+    const double* uvw,
+    int nclus, const int* cluster_offset_host,
+    const double* src_l, const double* src_m,
+    const double* src_I, const double* src_Q, const double* src_U, const double* src_V,
+    const double* src_alpha,
+    int coh_format, sagecal_c128* coh,
+    const sagecal_c128* jones, const sagecal_c128* vis, sagecal_c128* residual,
+    void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Jones corruption and subtraction (BASELINE.json:5 "the Jones-corrupted residual V_pq - J_p C_pq J_q^H";
  * SURVEY.md §8(a) rows 8a-2, 8a-3, 8a-6):
  *
@@ -189,9 +216,11 @@ int sagecal_lm_cost_grad_jtj(
  *                   accept iff rho > 0 (all finite): J = J', mu *= max(1/3, 1-(2 rho-1)^3), nu = 2;  else mu *= nu, nu *= 2
  *       R = x_k - J_k C_k J_k^H
  *
- * vis     : dev [rows][F][4] (read only).     coh : dev, K clusters.
+ * vis     : dev [rows][F][4] (read only), or NULL: `residual` then already holds V - sum_k J_k C_k J_k^H at the start
+ *           Jones (written by sagecal_predict_residual) and the initial pass over the coherencies is skipped.
+ * coh     : dev, K clusters.
  * jones   : dev [K][N][4], in = start values, out = solution.
- * residual: dev out [rows][F][4]; must not alias vis.
+ * residual: dev out (in/out with vis == NULL) [rows][F][4]; must not alias vis.
  * tau     : initial damping factor (1e-3 in all configs).
  * lm_mode : SAGECAL_LM_COMPRESSED, SAGECAL_LM_DIRECT, SAGECAL_LM_FULLGN or SAGECAL_LM_PERCLUSTER (above).
  * cost_per_cluster : dev out [K] f64: phi_k at the end of cluster k's last M-step.

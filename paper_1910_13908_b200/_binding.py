@@ -57,6 +57,8 @@ def load_library():
     L.sagecal_predict_workspace_bytes.argtypes = [i, i]
     L.sagecal_predict_coherencies.restype = i
     L.sagecal_predict_coherencies.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, i, vp, sz, vp]
+    L.sagecal_predict_residual.restype = i
+    L.sagecal_predict_residual.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
     L.sagecal_corrupt_subtract.restype = i
     L.sagecal_corrupt_subtract.argtypes = [i, i, i, i, i, vp, vp, vp, d, vp, vp, vp]
     L.sagecal_lm_cost_grad_jtj.restype = i
@@ -197,6 +199,50 @@ def predict_coherencies(N: int, T: int, freqs: Sequence[float], f0: float, uvw: 
     return out
 
 
+def predict_residual(N: int, T: int, freqs: Sequence[float], f0: float, uvw: torch.Tensor,
+                     cluster_offset: Sequence[int], src_l: torch.Tensor, src_m: torch.Tensor, src_I: torch.Tensor,
+                     src_alpha: torch.Tensor, jones: torch.Tensor, vis: torch.Tensor,
+                     src_Q: Optional[torch.Tensor] = None, src_U: Optional[torch.Tensor] = None,
+                     src_V: Optional[torch.Tensor] = None, coh_format: int = COH_FULL,
+                     out: Optional[torch.Tensor] = None, residual: Optional[torch.Tensor] = None, stream=None):
+    """sagecal_predict_residual: the coherencies of all K clusters AND residual = vis - sum_k J_k C_k J_k^H in one pass.
+    Returns (coh, residual)."""
+    L = load_library()
+    fr = np.ascontiguousarray(freqs, dtype=np.float64)
+    co = np.ascontiguousarray(cluster_offset, dtype=np.int32)
+    F, K, rows = int(fr.size), int(co.size) - 1, _rows(N, T)
+    shape = (K, rows, F, 4) if coh_format == COH_FULL else (K, rows, F)
+    c128 = torch.complex128
+    if out is None:
+        out = torch.empty(shape, dtype=c128, device=uvw.device)
+    elif tuple(out.shape) != shape:
+        raise ValueError(f"out: expected shape {shape}")
+    if tuple(uvw.shape) != (rows, 3):
+        raise ValueError(f"uvw: expected shape {(rows, 3)}")
+    if vis.numel() != rows * F * 4 or jones.numel() != K * N * 4:
+        raise ValueError("vis [rows,F,4] and jones [K,N,2,2] expected")
+    if residual is None:
+        residual = torch.empty((rows, F, 4), dtype=c128, device=uvw.device)
+    elif residual.numel() != rows * F * 4:
+        raise ValueError("residual: expected rows*F*4 elements")
+    S = int(co[-1]) if co.size else 0
+    for name, t in (("src_l", src_l), ("src_m", src_m), ("src_I", src_I), ("src_alpha", src_alpha),
+                    ("src_Q", src_Q), ("src_U", src_U), ("src_V", src_V)):
+        if t is not None and t.numel() != S:
+            raise ValueError(f"{name}: expected {S} elements")
+    wsb = int(L.sagecal_predict_workspace_bytes(F, S))
+    ws = _workspace(wsb, uvw.device)
+    f64 = torch.float64
+    rc = L.sagecal_predict_residual(
+        N, T, F, fr.ctypes.data, float(f0), _dev(uvw, f64, "uvw"), K, co.ctypes.data,
+        _dev(src_l, f64, "src_l"), _dev(src_m, f64, "src_m"), _dev(src_I, f64, "src_I"),
+        _dev(src_Q, f64, "src_Q"), _dev(src_U, f64, "src_U"), _dev(src_V, f64, "src_V"),
+        _dev(src_alpha, f64, "src_alpha"), coh_format, _dev(out, c128, "out"), _dev(jones, c128, "jones"),
+        _dev(vis, c128, "vis"), _dev(residual, c128, "residual"), ws.data_ptr(), wsb, _stream(stream))
+    _check(rc, "sagecal_predict_residual")
+    return out, residual
+
+
 def _coh_check(coh: torch.Tensor, coh_format: int, K: int, rows: int, F: int, name="coh"):
     shape = (K, rows, F, 4) if coh_format == COH_FULL else (K, rows, F)
     if tuple(coh.shape) != shape:
@@ -254,22 +300,27 @@ def lm_cost_grad_jtj(N: int, T: int, F: int, x: torch.Tensor, coh_k: torch.Tenso
     return cost, grad, jtj
 
 
-def sage_calibrate(N: int, T: int, F: int, vis: torch.Tensor, coh: torch.Tensor, jones: torch.Tensor,
+def sage_calibrate(N: int, T: int, F: int, vis: Optional[torch.Tensor], coh: torch.Tensor, jones: torch.Tensor,
                    n_em: int, n_lm: int, tau: float = 1e-3, coh_format: int = COH_FULL,
                    residual: Optional[torch.Tensor] = None, trace: bool = True, workspace: Optional[torch.Tensor] = None,
                    lm_mode: int = LM_COMPRESSED, stream=None):
-    """sagecal_sage_calibrate.  `jones` [K,N,2,2] is updated in place.
+    """sagecal_sage_calibrate.  `jones` [K,N,2,2] is updated in place.  vis = None: `residual` (required then) already
+    holds the initial residual written by predict_residual.
     Returns dict(jones, residual, cost_per_cluster [K], cost_trace [n_em*K+1] or None), all device tensors."""
     L = load_library()
     K, rows = int(jones.shape[0]), _rows(N, T)
     c128 = torch.complex128
     if K:
         _coh_check(coh, coh_format, K, rows, F)
-    if vis.numel() != rows * F * 4:
+    if vis is None and residual is None:
+        raise ValueError("vis = None needs the residual predict_residual wrote")
+    if vis is not None and vis.numel() != rows * F * 4:
         raise ValueError("vis: expected rows*F*4 elements")
+    if residual is not None and residual.numel() != rows * F * 4:
+        raise ValueError("residual: expected rows*F*4 elements")
     if jones.numel() != K * N * 4:
         raise ValueError("jones: expected [K, N, 2, 2]")
-    dev = vis.device
+    dev = jones.device if vis is None else vis.device
     if residual is None:
         residual = torch.empty((rows, F, 4), dtype=c128, device=dev)
     cpc = torch.zeros(max(K, 1), dtype=torch.float64, device=dev)

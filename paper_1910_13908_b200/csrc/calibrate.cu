@@ -260,7 +260,8 @@ static int sage_calibrate_core(int N, int T, int F, int K, const sagecal_c128* v
     if (N < 2 || T < 1 || F < 1 || K < 0 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
     if (lm_mode != SAGECAL_LM_COMPRESSED && lm_mode != SAGECAL_LM_DIRECT && lm_mode != SAGECAL_LM_FULLGN && lm_mode != SAGECAL_LM_PERCLUSTER) return SAGECAL_EINVAL;
-    if (!vis || !residual || vis == residual || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
+    // vis == NULL: `residual` already holds V - sum_k J_k C_k J_k^H at the start Jones (sagecal_predict_residual)
+    if (!residual || vis == residual || (vis && !aligned(vis, 32)) || !aligned(residual, 32)) return SAGECAL_EINVAL;
     if (K > 0 && (!coh || !jones || !cost_per_cluster)) return SAGECAL_EINVAL;
     if (K > 0 && (!aligned(coh, coh_format == SAGECAL_COH_SCALAR ? 16 : 32) || !aligned(jones, 16))) return SAGECAL_EINVAL;
     if (!(tau > 0.0) || !isfinite(tau)) return SAGECAL_EINVAL;
@@ -283,7 +284,9 @@ static int sage_calibrate_core(int N, int T, int F, int K, const sagecal_c128* v
     auto whole = [&]() { return after_chunk ? after_chunk(after_ctx, 0, T) : SAGECAL_OK; };
 
     // R = V - sum_k J_k C_k J_k^H
-    if (K > 0) {
+    if (!vis) {
+        // the initial residual came with the prediction
+    } else if (K > 0) {
         if ((rc = corrupt_range(N, T, F, coh_format, coh, jones, 0, K, -1.0, vis, residual, st))) return rc;
     } else {
         SGC_CUDA(cudaMemcpyAsync(residual, vis, (size_t)samples * 64, cudaMemcpyDeviceToDevice, st));

@@ -64,24 +64,29 @@ __global__ void predict_prep_kernel(int S, int F, int Fpad, PredFreqs fr, double
 // `tab` already points at this lane's copy (lane & 7), so the 8 lanes of a quarter-warp read 8 different 16-byte
 // columns of shared memory whatever their k: no bank conflicts (a single copy cost 1.8e9 conflict wavefronts per
 // cfg4 launch and left the FP64 pipe at 61 %).
-__device__ __forceinline__ void phasor_f64(double x, const double2* __restrict__ tab, double& er, double& ei) {
-    constexpr double MAGIC = 6755399441055744.0;                 // 1.5 * 2^52: adding it rounds to the nearest integer
-    const double TWO_PI = 6.283185307179586476925286766559;
-    constexpr double s1 = 6.283185307179586476925286766559, s3 = -41.341702240399760233968420089468,
-                     s5 = 81.605249276075054203397682678249, s7 = -76.705859753061385841630641093893;
-    constexpr double c2 = -19.739208802178717237668981999752, c4 = 64.939394022668291490960221297352,
-                     c6 = -85.456817206693725260701221782482, c8 = 60.244641371876660575590717312223;
-    (void)TWO_PI;
+// The polynomial coefficients live in constant memory: a DFMA takes a constant-bank operand for free, whereas literal
+// doubles were re-materialised by ~20 move instructions per loop trip, each of which costs the scheduler an issue slot
+// the FP64 pipe's two-slot instructions leave it few of.
+// PHC[0..3] = s1, s3, s5, s7 (sin(2 pi r) = r (s1 + s3 r^2 + ...)), PHC[4..7] = c2, c4, c6, c8, PHC[8] = 1.5 * 2^52
+__constant__ double PHC[9] = {6.283185307179586476925286766559, -41.341702240399760233968420089468,
+                              81.605249276075054203397682678249, -76.705859753061385841630641093893,
+                              -19.739208802178717237668981999752, 64.939394022668291490960221297352,
+                              -85.456817206693725260701221782482, 60.244641371876660575590717312223,
+                              6755399441055744.0};
+// `tab` is the BYTE address (shared window) of this lane's copy of entry 0: entry k sits 128 k bytes further.
+__device__ __forceinline__ void phasor_f64(double x, unsigned tab, double& er, double& ei) {
+    const double MAGIC = PHC[8];                                 // adding it rounds to the nearest integer
     double kd = fma(x, 64.0, MAGIC);
-    const int k = __double2loint(kd);
+    const unsigned k = (unsigned)__double2loint(kd);
     kd -= MAGIC;
     const double r = fma(kd, -0.015625, x);                      // exact: |r| <= 1/128 cycle
     const double r2 = r * r;
-    const double sp = r * fma(r2, fma(r2, fma(r2, s7, s5), s3), s1);          // sin(2 pi r)
-    const double cp = fma(r2, fma(r2, fma(r2, fma(r2, c8, c6), c4), c2), 1.0); // cos(2 pi r)
-    const double2 t = tab[(k & 63) << 3];
-    er = fma(-t.y, sp, t.x * cp);                                // cos(a + b)
-    ei = -fma(t.x, sp, t.y * cp);                                // -sin(a + b)
+    const double sp = r * fma(r2, fma(r2, fma(r2, PHC[3], PHC[2]), PHC[1]), PHC[0]);             // sin(2 pi r)
+    const double cp = fma(r2, fma(r2, fma(r2, fma(r2, PHC[7], PHC[6]), PHC[5]), PHC[4]), 1.0);   // cos(2 pi r)
+    double tx, ty;
+    asm("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(tx), "=d"(ty) : "r"(tab + ((k << 7) & 0x1f80u)));
+    er = fma(-ty, sp, tx * cp);                                  // cos(a + b)
+    ei = -fma(tx, sp, ty * cp);                                  // -sin(a + b)
 }
 __device__ __forceinline__ void phasor_f32(double cycles, float& er, float& ei) {   // exp(-2 pi i cycles)
     const float r = (float)(cycles - rint(cycles));          // exact reduction in float64, |r| <= 1/2
@@ -89,12 +94,19 @@ __device__ __forceinline__ void phasor_f32(double cycles, float& er, float& ei) 
     sincospif(2.0f * r, &sn, &cs);
     er = cs; ei = -sn;
 }
-template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
+// RESID (sagecal_predict_residual): the CTA loops ALL clusters for its 128 rows, and next to writing C_k it takes
+// R = V - sum_k J_k,p C_k J_k,q^H along: the rows' residual tile (FT channels x 4 correlations per thread) sits in
+// shared memory, so R is written once and the initial residual pass over the K coherencies (69.7 GB at configs[4])
+// is not needed.  Costs the prediction 16 (polarised: 64) more FP64 instructions per (row, cluster, channel).
+struct PredResid { int N, K; int64_t B; const sagecal_c128 *jones, *vis; sagecal_c128* residual; };
+template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED, bool RESID>
 __global__ void __launch_bounds__(PRED_THREADS)
 predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClusters cl,
                const double* __restrict__ uvw, const double* __restrict__ src_l,
                const double* __restrict__ src_m, const double* __restrict__ nm1_g,
-               const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh) {
+               const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh, PredResid rs) {
+    extern __shared__ __align__(16) unsigned char s_dyn[];       // RESID: double2 [FT * 4][PRED_THREADS]
+    double2* s_res = reinterpret_cast<double2*>(s_dyn) + threadIdx.x;
     constexpr int NFL = POL ? 4 : 1;
     constexpr int NACC = POL ? 4 : 1;            // complex accumulators per channel
     constexpr int ST = POL ? 32 : 128;           // sources per shared-memory tile
@@ -108,16 +120,30 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
 #pragma unroll
         for (int c = 0; c < 8; c++) s_tab_all[8 * threadIdx.x + c] = make_double2(cs, sn);
     }
-    const double2* s_tab = s_tab_all + (MIXED ? 0 : (threadIdx.x & 7));
+    const unsigned s_tab = (unsigned)__cvta_generic_to_shared(s_tab_all + (MIXED ? 0 : (threadIdx.x & 7)));
 
-    const int k = blockIdx.y;
-    const int s_begin = cl.off[k], s_end = cl.off[k + 1];
     const int64_t r = (int64_t)blockIdx.x * PRED_THREADS + threadIdx.x;
     const bool live = r < rows;
     double u = 0, v = 0, w = 0;
     if (live) { u = uvw[3 * r]; v = uvw[3 * r + 1]; w = uvw[3 * r + 2]; }
+    int sp = 0, sq = 1;                                         // RESID: the row's stations
+    if (RESID && live) bl_stations(rs.N, r % rs.B, sp, sq);
+    const int k_begin = RESID ? 0 : blockIdx.y, k_end = RESID ? rs.K : k_begin + 1;
 
     for (int c0 = 0; c0 < Fpad; c0 += FT) {
+      if (RESID && live) {
+#pragma unroll
+          for (int c = 0; c < FT; c++) {
+              if (c0 + c < F) {
+                  const sagecal_c128* vi = rs.vis + ((size_t)r * F + c0 + c) * 4;
+                  const d4 lo = ldg256_stream(vi), hi = ldg256_stream(vi + 2);
+                  s_res[(4 * c) * PRED_THREADS] = make_double2(lo.x, lo.y); s_res[(4 * c + 1) * PRED_THREADS] = make_double2(lo.z, lo.w);
+                  s_res[(4 * c + 2) * PRED_THREADS] = make_double2(hi.x, hi.y); s_res[(4 * c + 3) * PRED_THREADS] = make_double2(hi.z, hi.w);
+              }
+          }
+      }
+      for (int k = k_begin; k < k_end; k++) {
+        const int s_begin = cl.off[k], s_end = cl.off[k + 1];
         cplx acc[FT][NACC];
 #pragma unroll
         for (int c = 0; c < FT; c++)
@@ -246,17 +272,75 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
                     }
                 }
             }
+            if (RESID) {
+                // R -= J_p C J_q^H for this cluster: unpolarised C = c I2, so the model is c (J_p J_q^H)
+                m22 jp, jq, pq;
+                load_jones(rs.jones + ((size_t)k * rs.N + sp) * 4, jp);
+                load_jones(rs.jones + ((size_t)k * rs.N + sq) * 4, jq);
+                if (!POL) mmh(jp, jq, pq);
+#pragma unroll
+                for (int c = 0; c < FT; c++) {
+                    if (c0 + c < F) {
+                        m22 md;
+                        if (!POL) {
+#pragma unroll
+                            for (int e = 0; e < 4; e++) md.a[e] = cmul(acc[c][0], pq.a[e]);
+                        } else {
+                            m22 cc, t1;
+#pragma unroll
+                            for (int e = 0; e < 4; e++) cc.a[e] = acc[c][POL ? e : 0];
+                            mm(jp, cc, t1);
+                            mmh(t1, jq, md);
+                        }
+#pragma unroll
+                        for (int e = 0; e < 4; e++) {
+                            double2 x = s_res[(4 * c + e) * PRED_THREADS];
+                            x.x -= md.a[e].re; x.y -= md.a[e].im;
+                            s_res[(4 * c + e) * PRED_THREADS] = x;
+                        }
+                    }
+                }
+            }
         }
+      }
+      if (RESID && live) {
+#pragma unroll
+          for (int c = 0; c < FT; c++) {
+              if (c0 + c < F) {
+                  sagecal_c128* ro = rs.residual + ((size_t)r * F + c0 + c) * 4;
+                  const double2 a0 = s_res[(4 * c) * PRED_THREADS], a1 = s_res[(4 * c + 1) * PRED_THREADS];
+                  const double2 a2 = s_res[(4 * c + 2) * PRED_THREADS], a3 = s_res[(4 * c + 3) * PRED_THREADS];
+                  stg256(ro, a0.x, a0.y, a1.x, a1.y);
+                  stg256(ro + 2, a2.x, a2.y, a3.x, a3.y);
+              }
+          }
+      }
     }
 }
 
 template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
 static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
                           const PredClusters& cl, const double* uvw, const double* l, const double* m,
-                          const double* nm1, const double* flux, sagecal_c128* coh) {
+                          const double* nm1, const double* flux, sagecal_c128* coh, const PredResid* rs) {
     LaunchScope ls(KK_PREDICT, st);
-    predict_kernel<FT, POL, UNIFORM, SCALAR, MIXED><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m,
-                                                                          nm1, flux, coh);
+    if (rs) {
+        if (MIXED) return SAGECAL_EUNSUPPORTED;
+        // the residual tile: FT channels x 4 correlations x 16 B per thread (64 KB at FT = 8), opted in per device
+        constexpr int smem = FT * 4 * PRED_THREADS * 16;
+        auto kern = predict_kernel<FT, POL, UNIFORM, SCALAR, false, true>;
+        static bool ready[64] = {};
+        int dev = 0;
+        SGC_CUDA(cudaGetDevice(&dev));
+        if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
+        if (!ready[dev]) {
+            SGC_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+            ready[dev] = true;
+        }
+        kern<<<dim3(grid.x, 1), PRED_THREADS, smem, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m, nm1, flux, coh, *rs);
+    } else {
+        predict_kernel<FT, POL, UNIFORM, SCALAR, MIXED, false><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw,
+                                                                                     l, m, nm1, flux, coh, PredResid{});
+    }
     SGC_LAUNCH_CHECK();
     return SAGECAL_OK;
 }
@@ -275,12 +359,12 @@ extern "C" size_t sagecal_predict_workspace_bytes(int nchan, int nsrc_total) {
     return round_up(sizeof(double) * (size_t)nsrc_total, 256) + round_up(sizeof(double) * (size_t)nsrc_total * Fpad * 4, 256) + 256;
 }
 
-extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* freqs_host, double f0,
-                                           const double* uvw, int K, const int* cluster_offset_host,
-                                           const double* src_l, const double* src_m, const double* src_I,
-                                           const double* src_Q, const double* src_U, const double* src_V,
-                                           const double* src_alpha, int coh_format, sagecal_c128* coh,
-                                           int precision, void* workspace, size_t workspace_bytes, void* stream) {
+static int predict_impl(int N, int T, int F, const double* freqs_host, double f0,
+                        const double* uvw, int K, const int* cluster_offset_host,
+                        const double* src_l, const double* src_m, const double* src_I,
+                        const double* src_Q, const double* src_U, const double* src_V,
+                        const double* src_alpha, int coh_format, sagecal_c128* coh,
+                        int precision, void* workspace, size_t workspace_bytes, void* stream, const PredResid* rs) {
     if (N < 2 || T < 1 || F < 1 || F > PRED_MAXF || K < 0 || K > PRED_MAXK) return SAGECAL_EINVAL;
     if (!freqs_host || !(f0 > 0.0) || !cluster_offset_host) return SAGECAL_EINVAL;
     if (coh_format != SAGECAL_COH_FULL && coh_format != SAGECAL_COH_SCALAR) return SAGECAL_EINVAL;
@@ -308,11 +392,13 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
     PredFreqs fr;
     for (int c = 0; c < PRED_MAXF; c++) fr.kf[c] = 0.0;
     for (int c = 0; c < F; c++) fr.kf[c] = freqs_host[c] / SAGECAL_C0;
-    // uniform spacing (to 1e-13 of the band centre) enables the channel recurrence
+    // Uniform spacing enables the channel recurrence.  The tile's phasors advance by df, so a channel that is off the
+    // even grid by e Hz is off in phase by ph e / c0 cycles (ph up to 1e4 m): the test admits a few ulp of the
+    // frequency (4 eps f = 1.4e-7 Hz at 160 MHz, 5e-12 cycles), nothing a parity bound of 1e-10 could see.
     bool uniform = true;
     double df = F > 1 ? (freqs_host[F - 1] - freqs_host[0]) / (F - 1) : 0.0;
     for (int c = 0; c < F; c++)
-        if (fabs(freqs_host[c] - (freqs_host[0] + c * df)) > 1e-13 * fabs(freqs_host[0])) uniform = false;
+        if (fabs(freqs_host[c] - (freqs_host[0] + c * df)) > 4.0 * 2.220446049250313e-16 * fabs(freqs_host[F - 1])) uniform = false;
     const double dkf = df / SAGECAL_C0;
     for (int c = F; c < Fpad; c++) fr.kf[c] = fr.kf[0] + c * dkf;  // padded channels: harmless phases, zero flux
     PredClusters cl;
@@ -337,9 +423,9 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
 #define SGC_PRED(FT_, POL_, UNI_, SC_)                                                                                  \
     do {                                                                                                               \
         if (mixed) return launch_predict<FT_, POL_, UNI_, SC_, true>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l,  \
-                                                                    src_m, nm1, flux, coh);                            \
+                                                                    src_m, nm1, flux, coh, rs);                        \
         return launch_predict<FT_, POL_, UNI_, SC_, false>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l, src_m,    \
-                                                          nm1, flux, coh);                                             \
+                                                          nm1, flux, coh, rs);                                         \
     } while (0)
 #define SGC_PRED_FT(FT_)                                            \
     do {                                                            \
@@ -356,4 +442,30 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
 #undef SGC_PRED_FT
 #undef SGC_PRED
     return SAGECAL_OK;
+}
+
+extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* freqs_host, double f0,
+                                           const double* uvw, int K, const int* cluster_offset_host,
+                                           const double* src_l, const double* src_m, const double* src_I,
+                                           const double* src_Q, const double* src_U, const double* src_V,
+                                           const double* src_alpha, int coh_format, sagecal_c128* coh,
+                                           int precision, void* workspace, size_t workspace_bytes, void* stream) {
+    return predict_impl(N, T, F, freqs_host, f0, uvw, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
+                        src_alpha, coh_format, coh, precision, workspace, workspace_bytes, stream, nullptr);
+}
+
+extern "C" int sagecal_predict_residual(int N, int T, int F, const double* freqs_host, double f0,
+                                        const double* uvw, int K, const int* cluster_offset_host,
+                                        const double* src_l, const double* src_m, const double* src_I,
+                                        const double* src_Q, const double* src_U, const double* src_V,
+                                        const double* src_alpha, int coh_format, sagecal_c128* coh,
+                                        const sagecal_c128* jones, const sagecal_c128* vis, sagecal_c128* residual,
+                                        void* workspace, size_t workspace_bytes, void* stream) {
+    if (N < 2 || T < 1 || F < 1 || K < 1) return SAGECAL_EINVAL;
+    if (!jones || !vis || !residual || !aligned(jones, 16) || !aligned(vis, 32) || !aligned(residual, 32)) return SAGECAL_EINVAL;
+    PredResid rs;
+    rs.N = N; rs.K = K; rs.B = (int64_t)N * (N - 1) / 2;
+    rs.jones = jones; rs.vis = vis; rs.residual = residual;
+    return predict_impl(N, T, F, freqs_host, f0, uvw, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
+                        src_alpha, coh_format, coh, 0, workspace, workspace_bytes, stream, &rs);
 }

@@ -72,7 +72,7 @@ def _load(path):
 
 
 def test_cfg4_fixture_is_a_parity_seed():
-    """The stored full-size oracle run (tests/golden/make_golden_cfg4.py, oracle only) took no accept/reject decision
+    """The stored full-size oracle run (tests/golden/make_golden_full.py cfg4, oracle only) took no accept/reject decision
     within rounding of zero, and its cost trace falls monotonically (P11)."""
     g = _load(GOLD4)
     assert g["min_abs_rho"] > 1e-6
@@ -85,15 +85,13 @@ def test_cfg4_fixture_is_a_parity_seed():
 @pytest.mark.parametrize("coh", ["full", "scalar"])
 def test_cuda_path_matches_oracle_at_full_cfg4(cuda_device, coh):
     """The whole bench workload (configs[4]: N=512, T=20, F=8, K=50 x 40 sources, 3 EM x 10 LM), default lm_mode, in the
-    launch configuration bench.py times, against the stored oracle run: all 50 per-cluster costs and the 151-entry
-    cost trace to 1e-8, ||J_k||^2, sampled Jones entries and sampled residual entries."""
+    launch configuration bench.py times (and, second, with the prediction fused with the initial residual:
+    sagecal_predict_residual, then sagecal_sage_calibrate on that residual) against the stored oracle run: all 50 per-cluster costs and the 151-entry cost trace, ALL 25 600
+    Jones matrices and sampled residual entries to 1e-8."""
     import torch
     import paper_1910_13908_b200 as sg
-    from sagecal_inputs import make_config
-    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
-
-    g = _load(GOLD4)
-    p = make_config(4)
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate
+    g, J_want, p, rows = _fixture("cfg4")
     fmt = sg.COH_FULL if coh == "full" else sg.COH_SCALAR
     coh_d = gpu_predict(p, fmt)
     vis = gpu_simulate(p, coh_d, fmt)
@@ -101,30 +99,16 @@ def test_cuda_path_matches_oracle_at_full_cfg4(cuda_device, coh):
     assert abs(v2 - g["vis_norm2"]) <= 1e-10 * g["vis_norm2"]
     out = sg.sage_calibrate(p.N, p.T, p.F, vis, coh_d, dev(p.jones_init()), p.n_em, p.n_lm, p.tau, coh_format=fmt)
     torch.cuda.synchronize()
-    cpc = host(out["cost_per_cluster"])
-    want = np.array([g[f"cost_cluster_{k}"] for k in range(p.K)])
-    assert np.max(np.abs(cpc - want) / want) < 1e-8
-    tr = host(out["cost_trace"])
-    want_tr = np.array([g[f"cost_trace_{i}"] for i in range(tr.size)])
-    assert np.max(np.abs(tr - want_tr) / want_tr) < 1e-8
-    J = host(out["jones"])
-    for k in range(p.K):
-        n2 = float(np.vdot(J[k], J[k]).real)
-        assert abs(n2 - g[f"jones_norm2_{k}"]) <= 1e-8 * g[f"jones_norm2_{k}"]
-    for k in (0, 17, 49):
-        for s in (0, 255, 511):
-            z = np.array([g[f"jones_{k}_{s}_{e}_re"] + 1j * g[f"jones_{k}_{s}_{e}_im"] for e in range(4)])
-            assert np.linalg.norm(J[k, s].reshape(4) - z) <= 1e-8 * np.linalg.norm(z)
-    rows = np.sort(np.random.default_rng(4).choice(p.rows, 64, replace=False))
-    res = host(out["residual"][torch.from_numpy(rows).to(vis.device)])
-    assert abs(float(np.vdot(res, res).real) - g["residual_sample_norm2"]) <= 1e-8 * g["residual_sample_norm2"]
-    scale = np.sqrt(g["residual_sample_norm2"] / res.size)
-    for i, r in enumerate(rows):
-        for c in (0, p.F - 1):
-            for e in (0, 1):
-                z = g[f"residual_{r}_{c}_{e}_re"] + 1j * g[f"residual_{r}_{c}_{e}_im"]
-                assert abs(res[i, c, e] - z) <= 1e-8 * max(abs(z), scale)
-    del coh_d, vis, out
+    _compare_with_fixture(sg, p, g, J_want, rows, out, coh)
+    del out
+    jones = dev(p.jones_init())
+    coh_d.zero_()
+    _, res = sg.predict_residual(p.N, p.T, p.freqs, p.f0, dev(p.uvw), p.cluster_offset, dev(p.src_l), dev(p.src_m),
+                                 dev(p.src_I), dev(p.src_alpha), jones, vis, coh_format=fmt, out=coh_d)
+    out = sg.sage_calibrate(p.N, p.T, p.F, None, coh_d, jones, p.n_em, p.n_lm, p.tau, coh_format=fmt, residual=res)
+    torch.cuda.synchronize()
+    _compare_with_fixture(sg, p, g, J_want, rows, out, coh + " fused")
+    del coh_d, vis, out, res
     torch.cuda.empty_cache()
 
 
@@ -143,7 +127,7 @@ def _fixture(name):
     return g, J, p, mod.sample_rows(name, p)
 
 
-@pytest.mark.parametrize("name", ["cfg3", "cfg4pol"])
+@pytest.mark.parametrize("name", ["cfg3", "cfg4pol", "cfg4"])
 def test_full_budget_fixtures_are_parity_seeds(name):
     """No accept/reject decision of the stored oracle runs was within rounding of zero (Q18), the traces fall
     monotonically (P11) and end at ||R||^2 (P13); the polarised fixture does carry off-diagonal coherencies."""

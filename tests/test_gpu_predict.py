@@ -148,3 +148,67 @@ def test_predict_mixed_precision_variant(cuda_device, case):
     got = got.reshape(want.shape)
     assert rel_l2(got, want) < 1e-5 and rel_max(got, want) < 1e-5
     assert rel_l2(got, want) > 1e-10
+
+
+# ---- sagecal_predict_residual: prediction fused with the initial residual (rows 8a-0 .. 8a-2 in one pass) ----------
+def _fused(sg, p, fmt, jones, vis):
+    from tests.gpu_util import dev
+    d = {k: dev(getattr(p, k)) for k in ("src_l", "src_m", "src_I", "src_alpha", "src_Q", "src_U", "src_V")}
+    return sg.predict_residual(p.N, p.T, p.freqs, p.f0, dev(p.uvw), p.cluster_offset, d["src_l"], d["src_m"], d["src_I"],
+                               d["src_alpha"], dev(jones), dev(vis), d["src_Q"], d["src_U"], d["src_V"], coh_format=fmt)
+
+
+@pytest.mark.parametrize("cfg,fmt_name", [(0, "full"), (1, "full"), (2, "full"), (2, "scalar")])
+def test_predict_residual_matches_oracle(cuda_device, cfg, fmt_name):
+    """coh = the oracle's prediction and residual = V - sum_k J_k C_k J_k^H by the oracle's corrupt/subtract (1e-10), with
+    Jones that are not the identity; the coherencies are bit-identical to sagecal_predict_coherencies'."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host
+    p = make_config(cfg)
+    fmt = sg.COH_FULL if fmt_name == "full" else sg.COH_SCALAR
+    coh_ref = oracle.predict(p)
+    V = oracle.simulate(p, coh_ref)
+    J = p.jones_true * (1.0 + 0.05j) + 0.02
+    want = oracle.corrupt_subtract(p.N, p.T, p.F, coh_ref, J, V, sign=-1.0)
+    coh, res = _fused(sg, p, fmt, J, V)
+    assert np.array_equal(host(coh), host(gpu_predict(p, fmt)))
+    _check(host(res), want)
+
+
+@pytest.mark.parametrize("F,uniform", [(3, True), (5, False), (9, True)])
+def test_predict_residual_polarised_ragged(cuda_device, F, uniform):
+    """General 2x2 coherencies (model = J_p C J_q^H by two products), channel counts off the register tile, rows off the
+    CTA size, an empty cluster."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import host
+    rng = np.random.default_rng(300 + F)
+    freqs = np.linspace(120e6, 170e6, F) if uniform else np.sort(rng.uniform(120e6, 170e6, F))
+    p = make_problem(11, 3, F, 4, 7, seed=77 + F, polarised=True, layout="disc:20000", field_deg=5.0,
+                     patch_deg=0.7, freqs=freqs)
+    p.cluster_offset = np.array([0, 7, 7, 19, 28], dtype=np.int32)
+    coh_ref = oracle.predict(p)
+    V = oracle.simulate(p, coh_ref)
+    J = p.jones_true * (0.9 - 0.1j)
+    want = oracle.corrupt_subtract(p.N, p.T, p.F, coh_ref, J, V, sign=-1.0)
+    coh, res = _fused(sg, p, sg.COH_FULL, J, V)
+    _check(host(coh), coh_ref)
+    _check(host(res), want)
+
+
+@pytest.mark.parametrize("fmt_name", ["full", "scalar"])
+def test_calibrate_from_fused_residual_is_the_same_run(cuda_device, fmt_name):
+    """sagecal_sage_calibrate(vis = NULL) on the residual sagecal_predict_residual wrote follows the very trajectory of
+    the unfused route: costs, trace, Jones and residual agree to rounding of the initial residual (1e-11)."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+    p = make_config(2)
+    fmt = sg.COH_FULL if fmt_name == "full" else sg.COH_SCALAR
+    coh_d = gpu_predict(p, fmt)
+    vis = gpu_simulate(p, coh_d, fmt)
+    a = sg.sage_calibrate(p.N, p.T, p.F, vis, coh_d, dev(p.jones_init()), p.n_em, p.n_lm, p.tau, coh_format=fmt)
+    coh2, res = _fused(sg, p, fmt, p.jones_init(), host(vis))
+    b = sg.sage_calibrate(p.N, p.T, p.F, None, coh2, dev(p.jones_init()), p.n_em, p.n_lm, p.tau, coh_format=fmt, residual=res)
+    torch.cuda.synchronize()
+    for key in ("cost_per_cluster", "cost_trace", "jones", "residual"):
+        assert rel_l2(host(b[key]), host(a[key])) < 1e-11, key
