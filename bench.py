@@ -525,7 +525,7 @@ def run_ours(args):
                          "(DESIGN.md §5.5); the fraction is the baseline arithmetic alone against the FP64 issue peak")
             rooflines.append(e)
     cor = prof["corrupt"]
-    if not cor["timed"]:
+    if cor["timed"] != args.steps:                        # none (fused route) or one per add-back / write-back (direct)
         # fused route: the step has no residual pass of its own; BASELINE.json:5 item (c)'s kernel is timed on its own
         # here (sagecal_corrupt_subtract over all K clusters), after the timed region
         sg.profile_read()
@@ -543,7 +543,7 @@ def run_ours(args):
         rooflines.append({"bound": "hbm", "kernel": "corrupt_kernel", "achieved": cbytes / (cms * 1e-3) / 1e9, "peak": peak,
                           "unit": "GB/s", "frac": cbytes / (cms * 1e-3) / 1e9 / peak, "traffic": None, "peak_source": peak_src,
                           "algorithmic_bytes_per_launch": cbytes, "launches_timed": cor["timed"], "avg_launch_ms": cms,
-                          "where": "inside the timed region" if prof["corrupt"]["timed"] else
+                          "where": "inside the timed region" if prof["corrupt"]["timed"] == args.steps else
                                    "sagecal_corrupt_subtract over all K clusters after the timed region (the step's own "
                                    "initial residual is fused into the prediction)"})
     # the fused cost / gradient / J^H J pass as BASELINE.json:5 states it (the kernel of --lm direct): 20 launches of
@@ -647,6 +647,9 @@ def _finish(args, p, world, rank, ms_per_step, clk, e2e, e2e_cost_sum, gpu_launc
     predict_ms = breakdown.get("predict", 0.0) + breakdown.get("predict_prep", 0.0)
     line = {
         "metric": METRIC, "value": seconds_per_interval(ms_per_step, world), "unit": UNIT, "n_gpus": world,
+        # replicas: every rank calibrates its own interval, so `value` (job seconds per interval) is the per-replica
+        # time / n_gpus by construction; the per-replica wall time is what a kernel change moves
+        "per_replica_s": ms_per_step / 1000.0, "intervals_per_s": max(world, 1) / (ms_per_step / 1000.0),
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms_per_step, "higher_is_better": False,
         "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": {"workload": workload_name(p, args.coh, args.lm), "parallelism": "replicas only (one interval per GPU)",
