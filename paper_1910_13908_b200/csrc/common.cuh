@@ -4,6 +4,7 @@
 #include <stdint.h>
 #include <stddef.h>
 #include "sagecal_b200.h"
+#include "sagecal_b200_debug.h"
 
 namespace sgc {
 
