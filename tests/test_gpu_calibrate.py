@@ -72,7 +72,7 @@ def test_calibrate_polarised_small(cuda_device, mode):
 @pytest.mark.parametrize("mode", ["compressed", "percluster"])
 @pytest.mark.parametrize("shape", [(37, 3, 3), (33, 2, 5), (70, 2, 8), (6, 2, 40)])
 def test_calibrate_compressed_ragged_shapes(cuda_device, shape, mode):
-    """Compressed mode on shapes that leave ragged tiles everywhere: N not a multiple of the 16 x 32 station tile,
+    """Compressed mode on shapes that leave ragged pieces everywhere: N not a multiple of the 32-station column segment,
     F not a power of two (idle lanes in a baseline's lane group) and F > 32 (a lane walks several channels);
     polarised sources so all 16 + 16 statistics of a baseline matter."""
     N, T, F = shape
@@ -95,11 +95,28 @@ def test_calibrate_grouped_ragged_groups(cuda_device, K, scalar):
 
 
 def test_calibrate_compressed_more_tiles_than_ctas(cuda_device):
-    """N = 700: 500 live station tiles for at most 296 co-resident CTAs, so CTAs of the M-step kernel walk several
-    tiles (shared-memory buffers reused, per-CTA cost summed over tiles); the last column tile is ragged
+    """N = 700: 8070 units for at most 1184 co-resident warps, so every warp of the M-step kernel owns a chunk of 7 rows
+    whose statistics are streamed through its two shared-memory slots; the last column segment is ragged
     (700 = 21*32 + 28)."""
     p = make_problem(700, 1, 2, 2, 3, seed=123, sigma=0.05, layout="disc:20000", field_deg=4.0, patch_deg=0.5)
     want, got, _, _ = _run_both(p, 1, 4, mode="compressed")
+    _compare(want, got)
+
+
+@pytest.mark.parametrize("N,what", [(64, "one thread-block cluster of 16 CTAs, every warp a row (94 chunks)"),
+                                    (65, "first shape past the cluster (158 chunks): cooperative launch, 40 CTAs of 4 warps"),
+                                    (130, "cooperative, 1 row per warp, 5 column segments, ragged last one"),
+                                    (345, "2 rows per warp, statistics resident in two slots"),
+                                    (400, "3 rows per warp: more rows than slots, statistics streamed")])
+@pytest.mark.parametrize("scalar", [False, True])
+def test_calibrate_mstep_launch_regimes(cuda_device, N, what, scalar):
+    """The M-step kernel's launch plans (mstep.cu make_plan: cluster / cooperative launch, resident / streamed
+    statistics, chunk lengths 1, 2, 3) each against the oracle: one time slot, one channel, two clusters, so that the
+    oracle's pass over N(N-1)/2 baselines stays a matter of seconds."""
+    import paper_1910_13908_b200 as sg
+    p = make_problem(N, 1, 1, 2, 3, seed=900 + N, sigma=0.05, layout="disc:20000", field_deg=4.0, patch_deg=0.5,
+                     polarised=not scalar)
+    want, got, _, _ = _run_both(p, 2, 5, coh_format=sg.COH_SCALAR if scalar else sg.COH_FULL, mode="compressed")
     _compare(want, got)
 
 
