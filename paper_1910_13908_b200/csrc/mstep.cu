@@ -25,6 +25,7 @@
 // one-flag-per-CTA schemes at 2.5 us) or the hardware cluster barrier.  Everything that crosses CTAs is read with
 // ld.cg (L2).
 #include <math.h>
+#include <cooperative_groups.h>
 #include "compress.cuh"
 
 namespace sgc {
@@ -87,15 +88,8 @@ __device__ __forceinline__ double strided_max(const Strided& r) {
     return v;
 }
 
-// ---- grid barrier.  CLUSTER: the whole grid is one thread-block cluster, hardware barrier with release/acquire at
-// cluster scope.  Otherwise an arrive counter, generation gen = 1, 2, ... (the counter is zeroed before every launch).
-template <bool CLUSTER>
+// ---- grid barrier: an arrive counter, generation gen = 1, 2, ... (the counter is zeroed before every launch) -------
 __device__ __forceinline__ void grid_barrier(unsigned* bar, unsigned gen) {
-    if (CLUSTER) {
-        asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
-        asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
-        return;
-    }
     __syncthreads();
     if (threadIdx.x == 0) {
         asm volatile("red.release.gpu.global.add.u32 [%0], 1;" ::"l"(bar) : "memory");
@@ -131,6 +125,7 @@ template <bool SCALAR> struct Slot {
     static constexpr int SCC_OFF = 32 * SRC_B;
     static constexpr int BYTES = 32 * (SRC_B + SCC_B);                            // 2816 / 12800
 };
+constexpr int MS_CLUSTER_CTAS = 16;   // the largest thread-block cluster (non-portable size)
 constexpr int PJ_DOUBLES = 24;    // per warp: J_try (8), J0 (8), D = J_try - J0 (8) of the row station
 
 template <bool SCALAR>
@@ -515,7 +510,7 @@ __device__ __forceinline__ void publish(const double* s_w, double* out, bool is_
     out[blockIdx.x] = c;
 }
 
-template <bool SCALAR, bool CLUSTER>
+template <bool SCALAR>
 __global__ void __launch_bounds__(MS_THREADS, 1)
 mstep_kernel(const MstepArgs A) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -570,7 +565,7 @@ mstep_kernel(const MstepArgs A) {
         phase_baselines<SCALAR>(A, sm, ww, e, last, j0q, seq);
         __syncthreads();
         if (threadIdx.x == 0) publish(sm.s_red, A.cost_cta, false);
-        grid_barrier<CLUSTER>(A.bar, ++gen);
+        grid_barrier(A.bar, ++gen);
 
         // Warps without a station have nothing to decide; they only keep the barriers company.
         double pred_w = 0.0;
@@ -592,7 +587,7 @@ mstep_kernel(const MstepArgs A) {
             if (lane == 0) sm.s_red[2 * MS_WARPS + warp] = mm;
             __syncthreads();
             if (threadIdx.x == 0) publish(sm.s_red + 2 * MS_WARPS, A.mm_cta, true);
-            grid_barrier<CLUSTER>(A.bar, ++gen);
+            grid_barrier(A.bar, ++gen);
             if (sp0.s < N) {
                 mu = A.tau * strided_max(strided_load(A.mm_cta, (int)gridDim.x, lane));
                 nu = 2.0;
@@ -672,7 +667,7 @@ mstep_kernel(const MstepArgs A) {
             if (lane == 0) sm.s_red[MS_WARPS + warp] = pred_w;
             __syncthreads();
             if (threadIdx.x == 0) publish(sm.s_red + MS_WARPS, A.pred_cta + (size_t)(e & 1) * MS_MAX_GRID, false);
-            grid_barrier<CLUSTER>(A.bar, ++gen);
+            grid_barrier(A.bar, ++gen);
         }
     }
     if (blockIdx.x == 0 && threadIdx.x == 0) {
@@ -680,6 +675,256 @@ mstep_kernel(const MstepArgs A) {
         if (A.cost_out) *A.cost_out = phi;
         if (A.trace_out) *A.trace_out = phi;
     }
+}
+
+// ---- the smallest arrays: ONE thread-block cluster, exchanges through distributed shared memory ---------------------
+// N <= 64 (two column segments, at most 94 units): every unit has its own warp in a cluster of up to 16 CTAs and every
+// station its own warp, so nothing of an evaluation has to travel through global memory: a warp stores its row record
+// and its 32 column records straight into the shared memory of the CTA whose warp owns that station
+// (st.shared::cluster through map_shared_rank), the owner sums them from its own shared memory, keeps the accepted
+// (G, M, J) of its station in registers for the whole launch and stores the next trial Jones into EVERY CTA's copy of
+// the Jones table; cost and predicted reduction go to every CTA as one value per CTA.  Two hardware cluster barriers
+// (release / acquire) per evaluation, no L2 round trip on the critical path.  Same sums in the same order as the grid
+// form: fixed, bit-reproducible.
+constexpr int CL_MAXN = 64, CL_MAXROWS = 63, CL_NQT = 2;
+template <bool SCALAR>
+__host__ __device__ constexpr size_t mstep_cluster_smem_bytes() {
+    return (size_t)MS_WARPS * Slot<SCALAR>::BYTES +
+           sizeof(double) * (MS_WARPS * PJ_DOUBLES + 3 * MS_WARPS + 2 * CL_MAXN * 8 + MS_WARPS * CL_NQT * MS_NV +
+                             MS_WARPS * CL_MAXROWS * MS_NV + 4 * MS_CLUSTER_CTAS);
+}
+__device__ __forceinline__ cplx sel4(const cplx* a, int i) { return i == 0 ? a[0] : i == 1 ? a[1] : i == 2 ? a[2] : a[3]; }
+
+template <bool SCALAR>
+__global__ void __launch_bounds__(MS_THREADS, 1)
+mstep_cluster_kernel(const MstepArgs A) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    using S = Slot<SCALAR>;
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    const MGeom& g = A.g;
+    const int N = g.N, G = (int)gridDim.x, rank = (int)blockIdx.x;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gw = warp * G + rank;                      // this warp's unit (m = 1) and its station
+    unsigned char* stage = smem_raw + (size_t)warp * S::BYTES;
+    double* pj = reinterpret_cast<double*>(smem_raw + (size_t)MS_WARPS * S::BYTES) + warp * PJ_DOUBLES;
+    double* s_red = reinterpret_cast<double*>(smem_raw + (size_t)MS_WARPS * S::BYTES) + MS_WARPS * PJ_DOUBLES;
+    double* cl_j = s_red + 3 * MS_WARPS;                 // [CL_MAXN][8]  trial Jones, this CTA's copy
+    double* cl_j0 = cl_j + CL_MAXN * 8;                  // [CL_MAXN][8]  centre Jones
+    double* cl_prow = cl_j0 + CL_MAXN * 8;               // [MS_WARPS][CL_NQT][12]      row records of this CTA's stations
+    double* cl_pcol = cl_prow + MS_WARPS * CL_NQT * MS_NV;         // [MS_WARPS][CL_MAXROWS][12] column records
+    double* cl_part = cl_pcol + MS_WARPS * CL_MAXROWS * MS_NV;     // [4][MS_CLUSTER_CTAS]: cost, pred (2 halves), max diag M
+
+    int qt = 0, p = 0, cnt = 0;
+    if (gw < g.nchunks) g.decode(gw, qt, p, cnt);
+    const int q = MS_TQ * qt + lane;
+    const bool qlive = q < N, has_unit = cnt > 0, has_station = gw < N;
+    if (has_unit) issue_unit<SCALAR>(A, stage, qt, p, lane);
+    cp_async_commit();
+    // every CTA reads the cluster's current Jones itself: centre and first trial point
+    for (int i = threadIdx.x; i < 4 * N; i += MS_THREADS) {
+        const cplx z = ldcg_c(A.Jk + i);
+        cl_j[2 * i] = z.re; cl_j[2 * i + 1] = z.im;
+        cl_j0[2 * i] = z.re; cl_j0[2 * i + 1] = z.im;
+        if (rank == 0) st_c(A.J0 + i, z);                // the centre of this chunk's statistics, for the write-back
+    }
+    // this warp's station: accepted G, M, J and the trial J, one complex number per lane (lane & 15)
+    const int which = lane & 15;
+    cplx mine = mk(0.0, 0.0);
+    if (has_station && which >= 8) mine = ldcg_c(A.Jk + 4 * gw + (which & 3));
+    const int nrow = has_station && gw <= N - 2 ? g.nqt - (gw + 1) / MS_TQ : 0;      // its row records: segments qt0 ..
+    const int qt0 = (gw + 1) / MS_TQ, qts = gw / MS_TQ;
+    const int ncol = has_station ? min(gw, g.nrows(qts)) : 0;                        // its column records: rows p < s
+    cp_async_wait<0>();
+    __syncthreads();
+    cluster.sync();                                      // every CTA is running before anyone stores into it
+
+    cplx j0q[4], jq[4];
+#pragma unroll
+    for (int x = 0; x < 4; x++) j0q[x] = qlive && has_unit ? lds_c(cl_j0 + 8 * q + 2 * x) : mk(0.0, 0.0);
+    double phi = 0.0, mu = A.init ? 0.0 : A.ctl->mu, nu = A.init ? 2.0 : A.ctl->nu;
+
+    for (int e = 0; e <= A.n_trial; e++) {
+        const bool last = e == A.n_trial;
+        // ---- phase A: this warp's unit ----
+        double cost = 0.0;
+        if (has_unit) {
+            QSide Q;
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                jq[x] = qlive ? lds_c(cl_j + 8 * q + 2 * x) : mk(0.0, 0.0);
+                Q.j[x] = jq[x];
+                Q.d[x] = csub(jq[x], j0q[x]);
+            }
+            gram22(Q.j, Q.h00, Q.h11, Q.h01);
+            if (lane < 8) {                              // the row station's J_try (lanes 0..3), J0 (4..7), D
+                const cplx a = lds_c((lane < 4 ? cl_j : cl_j0) + 8 * p + 2 * (lane & 3));
+                pj[2 * lane] = a.re; pj[2 * lane + 1] = a.im;
+                if (lane < 4) { const cplx b = lds_c(cl_j0 + 8 * p + 2 * lane); pj[16 + 2 * lane] = a.re - b.re; pj[17 + 2 * lane] = a.im - b.im; }
+            }
+            __syncwarp();
+            cplx gq[4] = {mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0), mk(0.0, 0.0)};
+            double mq[4] = {0.0, 0.0, 0.0, 0.0};
+            double v[16];
+#pragma unroll
+            for (int x = 0; x < 16; x++) v[x] = 0.0;
+            if (qlive && q > p)
+                baseline_task<SCALAR>(reinterpret_cast<const double*>(stage + lane * S::SRC_B),
+                                      stage + S::SCC_OFF + lane * S::SCC_B, lane, pj, Q, v, gq, mq, cost);
+            halve_sum16(v, lane);
+            const int idx = halve_index(lane);
+            if (!(lane & 1) && idx < MS_NV) {            // row record -> the CTA of the warp that owns station p
+                double* dst = cluster.map_shared_rank(cl_prow, p % G) + ((p / G) * CL_NQT + qt) * MS_NV;
+                dst[idx] = v[0];
+            }
+            if (qlive) {                                 // column record of row p -> the owner of station q
+                double2* dst = reinterpret_cast<double2*>(cluster.map_shared_rank(cl_pcol, q % G) + ((q / G) * CL_MAXROWS + p) * MS_NV);
+                dst[0] = make_double2(gq[0].re, gq[0].im); dst[1] = make_double2(gq[1].re, gq[1].im);
+                dst[2] = make_double2(gq[2].re, gq[2].im); dst[3] = make_double2(gq[3].re, gq[3].im);
+                dst[4] = make_double2(mq[0], mq[1]); dst[5] = make_double2(mq[2], mq[3]);
+            }
+        }
+        cost = wsum(cost);
+        if (lane == 0) s_red[warp] = cost;
+        __syncthreads();
+        if (warp == 0 && lane < G) {                     // the CTA's cost, to every CTA of the cluster
+            double c = s_red[0];
+#pragma unroll
+            for (int w = 1; w < MS_WARPS; w++) c += s_red[w];
+            cluster.map_shared_rank(cl_part, lane)[rank] = c;
+        }
+        cluster.sync();
+
+        // ---- phase B: this warp's station ----
+        double pred_w = 0.0, mm = 0.0;
+        StAcc r;
+        if (has_station) {
+            double acc[16];
+#pragma unroll
+            for (int x = 0; x < 16; x++) acc[x] = 0.0;
+            if (lane < nrow) {
+                const double* rec = cl_prow + (warp * CL_NQT + qt0 + lane) * MS_NV;
+#pragma unroll
+                for (int x = 0; x < MS_NV; x++) acc[x] += rec[x];
+            }
+            for (int c = lane; c < ncol; c += 32) {
+                const double* rec = cl_pcol + (warp * CL_MAXROWS + c) * MS_NV;
+#pragma unroll
+                for (int x = 0; x < MS_NV; x++) acc[x] += rec[x];
+            }
+            acc[12] = lane < G ? cl_part[lane] : 0.0;
+            acc[13] = (e > 0 && lane < G) ? cl_part[(1 + ((e + 1) & 1)) * MS_CLUSTER_CTAS + lane] : 0.0;
+            halve_sum16(acc, lane);
+            double t[14];
+#pragma unroll
+            for (int x = 0; x < 14; x++) t[x] = __shfl_sync(0xffffffffu, acc[0], 2 * x);
+#pragma unroll
+            for (int x = 0; x < 4; x++) r.g[x] = mk(t[2 * x], t[2 * x + 1]);
+            r.m[0] = mk(t[8], 0.0); r.m[1] = mk(t[10], t[11]); r.m[2] = mk(t[10], -t[11]); r.m[3] = mk(t[9], 0.0);
+            r.x0 = t[12]; r.x1 = t[13];
+        }
+        bool accept = false, take = false, step = false;
+        if (e == 0 && A.init) {
+            if (has_station) { phi = r.x0; mm = fmax(r.m[0].re, r.m[3].re); }
+            if (lane == 0) s_red[2 * MS_WARPS + warp] = mm;
+            __syncthreads();
+            if (warp == 0 && lane < G) {
+                double c = s_red[2 * MS_WARPS];
+#pragma unroll
+                for (int w = 1; w < MS_WARPS; w++) c = fmax(c, s_red[2 * MS_WARPS + w]);
+                cluster.map_shared_rank(cl_part, lane)[3 * MS_CLUSTER_CTAS + rank] = c;
+            }
+            cluster.sync();
+            double m = lane < G ? cl_part[3 * MS_CLUSTER_CTAS + lane] : 0.0;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+            mu = A.tau * m;
+            nu = 2.0;
+            take = true; step = !last;
+        } else if (has_station) {
+            const double fresh = r.x0;
+            if (e == 0) {
+                phi = fresh;
+            } else {
+                const double pred = r.x1;
+                const double rho = (phi - fresh) / pred;
+                accept = isfinite(fresh) && isfinite(pred) && isfinite(rho) && pred > 0.0 && rho > 0.0;
+                if (accept) {
+                    phi = fresh;
+                    const double t = 2.0 * rho - 1.0;
+                    mu *= fmax(1.0 / 3.0, 1.0 - t * t * t);
+                    nu = 2.0;
+                } else {
+                    mu *= nu;
+                    nu *= 2.0;
+                }
+            }
+            take = accept || e == 0; step = !last;
+        }
+        if (!(mu >= 1e-300)) mu = 1e-300;
+        if (mu > 1e300) mu = 1e300;
+        if (nu > 0x1p60) nu = 0x1p60;
+        if (has_station) {
+            cplx g4[4], m4[4], jj[4];
+#pragma unroll
+            for (int x = 0; x < 4; x++) {
+                const int jsrc = accept ? 12 + x : 8 + x;
+                const cplx go = mk(__shfl_sync(0xffffffffu, mine.re, x), __shfl_sync(0xffffffffu, mine.im, x));
+                const cplx mo = mk(__shfl_sync(0xffffffffu, mine.re, 4 + x), __shfl_sync(0xffffffffu, mine.im, 4 + x));
+                jj[x] = mk(__shfl_sync(0xffffffffu, mine.re, jsrc), __shfl_sync(0xffffffffu, mine.im, jsrc));
+                g4[x] = take ? r.g[x] : go;
+                m4[x] = take ? r.m[x] : mo;
+            }
+            // the accepted state stays in registers
+            if (which < 4) mine = sel4(g4, which);
+            else if (which < 8) mine = sel4(m4, which & 3);
+            else if (which < 12) mine = sel4(jj, which & 3);
+            if (step) {
+                // dJ = G (M + mu I)^-1, J_try = J + dJ
+                const double a = m4[0].re + mu, d = m4[3].re + mu;
+                const cplx b = m4[1];
+                const double rdet = 1.0 / (a * d - (b.re * b.re + b.im * b.im));
+                const cplx inv[4] = {mk(d * rdet, 0.0), mk(-b.re * rdet, -b.im * rdet), mk(-b.re * rdet, b.im * rdet), mk(a * rdet, 0.0)};
+                cplx dj[4], jt[4];
+                dj[0] = cfma(g4[1], inv[2], cmul(g4[0], inv[0]));
+                dj[1] = cfma(g4[1], inv[3], cmul(g4[0], inv[1]));
+                dj[2] = cfma(g4[3], inv[2], cmul(g4[2], inv[0]));
+                dj[3] = cfma(g4[3], inv[3], cmul(g4[2], inv[1]));
+#pragma unroll
+                for (int x = 0; x < 4; x++) {
+                    jt[x] = cadd(jj[x], dj[x]);
+                    pred_w += g4[x].re * dj[x].re + g4[x].im * dj[x].im;
+                    pred_w += mu * (dj[x].re * dj[x].re + dj[x].im * dj[x].im);
+                }
+                if (which >= 12) mine = sel4(jt, which & 3);
+                // the trial Jones of this station, into every CTA's table: lane -> (CTA lane % G, entries lane / G, ...)
+                for (int o = lane; o < 4 * G; o += 32) {
+                    const int dst_rank = o % G, x = o / G;
+                    const cplx z = sel4(jt, x);
+                    double2* dst = reinterpret_cast<double2*>(cluster.map_shared_rank(cl_j, dst_rank) + 8 * gw + 2 * x);
+                    *dst = make_double2(z.re, z.im);
+                }
+            }
+        }
+        if (!last) {
+            if (lane == 0) s_red[MS_WARPS + warp] = pred_w;
+            __syncthreads();
+            if (warp == 0 && lane < G) {
+                double c = s_red[MS_WARPS];
+#pragma unroll
+                for (int w = 1; w < MS_WARPS; w++) c += s_red[MS_WARPS + w];
+                cluster.map_shared_rank(cl_part, lane)[(1 + (e & 1)) * MS_CLUSTER_CTAS + rank] = c;
+            }
+            cluster.sync();
+        }
+    }
+    if (has_station && lane >= 8 && lane < 12) st_c(A.Jk + 4 * gw + (lane & 3), mine);
+    if (rank == 0 && threadIdx.x == 0) {
+        A.ctl->phi = phi; A.ctl->mu = mu; A.ctl->nu = nu;
+        if (A.cost_out) *A.cost_out = phi;
+        if (A.trace_out) *A.trace_out = phi;
+    }
+    cluster.sync();                                      // nobody leaves while others may still store into it
 }
 
 // ---- host side ----------------------------------------------------------------------------------------------------
@@ -727,7 +972,7 @@ CompressWorkspace carve_compress(int N, int K, bool scalar, void* ws) {
 // Launch plan of the M-step kernel for N stations on a device with `sms` SMs (one CTA per SM): work decomposition,
 // slots per warp, grid.  Device independent but for `sms` and `cluster_cap` (the largest thread-block cluster the
 // device schedules, 0 = none), so that the host replay below sees what the kernel does.
-constexpr int MS_CLUSTER_MAX = 16;
+
 struct MstepPlan { MGeom g; int slots, grid; bool cluster; };
 static MstepPlan make_plan(int N, bool scalar, int sms, int cluster_cap) {
     MstepPlan pl;
@@ -742,8 +987,8 @@ static MstepPlan make_plan(int N, bool scalar, int sms, int cluster_cap) {
     pl.grid = want < cap ? want : cap;
     if (pl.grid * MS_WARPS < pl.g.nchunks) pl.grid = (pl.g.nchunks + MS_WARPS - 1) / MS_WARPS;
     if (pl.grid < 1) pl.grid = 1;
-    // the smallest arrays run as ONE thread-block cluster: its hardware barrier replaces the arrive counter
-    pl.cluster = pl.g.nchunks <= cluster_cap * MS_WARPS;
+    // the smallest arrays run as ONE thread-block cluster (mstep_cluster_kernel): a warp per unit, a warp per station
+    pl.cluster = N <= CL_MAXN && pl.g.m == 1 && pl.g.nchunks <= cluster_cap * MS_WARPS;
     if (pl.cluster) {
         if (pl.grid > cluster_cap) pl.grid = cluster_cap;
         if (pl.grid * MS_WARPS < pl.g.nchunks) pl.grid = (pl.g.nchunks + MS_WARPS - 1) / MS_WARPS;
@@ -762,23 +1007,24 @@ static int mstep_prepare(MstepDevice* out) {
     MstepDevice& d = devs[dev];
     if (!d.ready) {
         const int smem = (int)mstep_smem_bytes<SCALAR>(max_slots<SCALAR>());
-        SGC_CUDA(cudaFuncSetAttribute(mstep_kernel<SCALAR, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-        SGC_CUDA(cudaFuncSetAttribute(mstep_kernel<SCALAR, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SGC_CUDA(cudaFuncSetAttribute(mstep_kernel<SCALAR>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+        SGC_CUDA(cudaFuncSetAttribute(mstep_cluster_kernel<SCALAR>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                      (int)mstep_cluster_smem_bytes<SCALAR>()));
         SGC_CUDA(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev));
         // the largest cluster (16 needs the non-portable opt-in, 8 is portable) that can be resident with the
         // shared memory of a small array (its rows are resident: one slot per warp)
         d.cluster_cap = 0;
-        const bool np = cudaFuncSetAttribute(mstep_kernel<SCALAR, true>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
-        for (int csz = np ? MS_CLUSTER_MAX : 8; csz >= 2 && !d.cluster_cap; csz >>= 1) {
+        const bool np = cudaFuncSetAttribute(mstep_cluster_kernel<SCALAR>, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) == cudaSuccess;
+        for (int csz = np ? MS_CLUSTER_CTAS : 8; csz >= 2 && !d.cluster_cap; csz >>= 1) {
             cudaLaunchConfig_t cfg = {};
             cfg.gridDim = dim3((unsigned)csz); cfg.blockDim = dim3(MS_THREADS);
-            cfg.dynamicSmemBytes = mstep_smem_bytes<SCALAR>(1);
+            cfg.dynamicSmemBytes = mstep_cluster_smem_bytes<SCALAR>();
             cudaLaunchAttribute at;
             at.id = cudaLaunchAttributeClusterDimension;
             at.val.clusterDim.x = (unsigned)csz; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
             cfg.attrs = &at; cfg.numAttrs = 1;
             int ncl = 0;
-            if (cudaOccupancyMaxActiveClusters(&ncl, mstep_kernel<SCALAR, true>, &cfg) == cudaSuccess && ncl >= 1) d.cluster_cap = csz;
+            if (cudaOccupancyMaxActiveClusters(&ncl, mstep_cluster_kernel<SCALAR>, &cfg) == cudaSuccess && ncl >= 1) d.cluster_cap = csz;
         }
         (void)cudaGetLastError();
         d.ready = true;
@@ -807,20 +1053,21 @@ int enqueue_mstep(int N, bool scalar, const CompressWorkspace& w, const double* 
     if (pl.cluster) {
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = dim3((unsigned)pl.grid); cfg.blockDim = dim3(MS_THREADS);
-        cfg.dynamicSmemBytes = smem; cfg.stream = st;
+        cfg.dynamicSmemBytes = scalar ? mstep_cluster_smem_bytes<true>() : mstep_cluster_smem_bytes<false>();
+        cfg.stream = st;
         cudaLaunchAttribute at;
         at.id = cudaLaunchAttributeClusterDimension;
         at.val.clusterDim.x = (unsigned)pl.grid; at.val.clusterDim.y = 1; at.val.clusterDim.z = 1;
         cfg.attrs = &at; cfg.numAttrs = 1;
         LaunchScope ls(KK_MSTEP, st);
-        if (scalar) SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_kernel<true, true>, A));
-        else SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_kernel<false, true>, A));
+        if (scalar) SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_cluster_kernel<true>, A));
+        else SGC_CUDA(cudaLaunchKernelEx(&cfg, mstep_cluster_kernel<false>, A));
         return SAGECAL_OK;
     }
     SGC_CUDA(cudaMemsetAsync(w.bar, 0, 256, st));
     void* args[] = {(void*)&A};
     LaunchScope ls(KK_MSTEP, st);
-    SGC_CUDA(cudaLaunchCooperativeKernel(scalar ? (const void*)mstep_kernel<true, false> : (const void*)mstep_kernel<false, false>,
+    SGC_CUDA(cudaLaunchCooperativeKernel(scalar ? (const void*)mstep_kernel<true> : (const void*)mstep_kernel<false>,
                                          dim3((unsigned)pl.grid), dim3(MS_THREADS), args, smem, st));
     return SAGECAL_OK;
 }
@@ -833,7 +1080,7 @@ using namespace sgc;
 // MGeom / make_plan the launch uses, for a device with `sms` SMs.
 extern "C" int sagecal_debug_mstep_cover(int N, int sms, int32_t* cover, int64_t* info) {
     if (N < 2 || sms < 1 || !cover || !info) return SAGECAL_EINVAL;
-    const MstepPlan pl = make_plan(N, false, sms, sms >= MS_CLUSTER_MAX ? MS_CLUSTER_MAX : 0);
+    const MstepPlan pl = make_plan(N, false, sms, sms >= MS_CLUSTER_CTAS ? MS_CLUSTER_CTAS : 0);
     const MGeom& g = pl.g;
     const size_t nP = (size_t)g.U, nQ = (size_t)g.nchunks * MS_TQ;
     // bit 0: written, bit 1: carries a baseline, bit 2: read by the station reduction
