@@ -319,12 +319,15 @@ def run_reference(args):
     from sagecal_inputs import make_config
     oracle.build()
     p = make_config(args.config)
+    # every step is one bounded sample; with many steps the sample is cut to ONE cluster (about 10 s of host time at
+    # configs[4]) so that the driver's --steps 20 --warmup 5 run still ends within a few minutes
+    sample = dict(SAMPLE, K=1) if args.steps + args.warmup > 6 else SAMPLE
     for _ in range(args.warmup):
-        oracle_sample(p)
+        oracle_sample(p, sample)
     vals, desc = [], ""
     t0 = time.perf_counter()
     for _ in range(args.steps):
-        v, desc, _ = oracle_sample(p)
+        v, desc, _ = oracle_sample(p, sample)
         vals.append(v)
     wall_ms = (time.perf_counter() - t0) * 1000.0 / max(args.steps, 1)
     value = float(np.mean(vals))
