@@ -25,6 +25,7 @@
 // one-flag-per-CTA schemes at 2.5 us) or the hardware cluster barrier.  Everything that crosses CTAs is read with
 // ld.cg (L2).
 #include <math.h>
+#include <mutex>
 #include <cooperative_groups.h>
 #include "compress.cuh"
 
@@ -1001,6 +1002,8 @@ template <bool SCALAR>
 static int mstep_prepare(MstepDevice* out) {
     // per device: the opt-in to large dynamic shared memory is a per-device function attribute
     static MstepDevice devs[64] = {};
+    static std::mutex mu;                              // two host threads may meet here on their first call
+    std::lock_guard<std::mutex> lk(mu);
     int dev = 0;
     SGC_CUDA(cudaGetDevice(&dev));
     if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;

@@ -15,6 +15,7 @@
 // float64 (phases reach 3.3e3 cycles: float32 would leave 1e-4 cycles), then sincospif, the channel recurrence and
 // the flux products run in float32; products are summed in float32 over at most 32 sources and those partial sums
 // are added to the float64 accumulators.  Error ~1e-6 relative; the parity bound is 1e-5 (BASELINE.json:5).
+#include <mutex>
 #include "common.cuh"
 
 namespace sgc {
@@ -329,6 +330,8 @@ static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int F
         constexpr int smem = FT * 4 * PRED_THREADS * 16;
         auto kern = predict_kernel<FT, POL, UNIFORM, SCALAR, false, true>;
         static bool ready[64] = {};
+        static std::mutex mu;                          // two host threads may meet here on their first call
+        std::lock_guard<std::mutex> lk(mu);
         int dev = 0;
         SGC_CUDA(cudaGetDevice(&dev));
         if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
