@@ -240,9 +240,9 @@ int sagecal_sage_calibrate(
 /*
  * Whole-interval convenience entry with HOST buffers (used for end-to-end timing): copies uvw, the source table,
  * the visibilities and the start Jones to the device, runs predict + calibrate, copies Jones, residual and costs
- * back.  Allocates and frees its own device memory, stream-ordered on `stream`, from a PRIVATE memory pool the library
- * creates once per (host thread, device) and whose blocks it keeps between calls (the arena, about 70 GB at
- * configs[4], stays reserved until the process ends; the device's default pool and its attributes are not touched).
+ * back.  Works in an arena of device memory the library allocates (cudaMalloc) on the first call and keeps, per (host
+ * thread, device), for the following ones (about 70 GB at configs[4]; grown when a larger interval arrives, handed back
+ * by sagecal_host_trim; no memory pool of the device is touched).
  * The visibilities travel on an internal copy stream while the coherencies are predicted, and the last write-back runs
  * in ranges of time slots whose copies to the host overlap the next range's kernel.  Synchronises `stream` and the
  * copy stream before returning.  All array pointers are host pointers (pinned memory recommended: pageable memory
@@ -258,6 +258,32 @@ int sagecal_calibrate_interval_host(
     const sagecal_c128* vis_host, sagecal_c128* jones_host, sagecal_c128* residual_host,
     int n_em, int n_lm, double tau, int lm_mode,
     double* cost_per_cluster_host, double* cost_trace_host, void* stream);
+
+/*
+ * The same, ASYNCHRONOUS: returns once the interval is enqueued, so that a stream of intervals overlaps the
+ * device-to-host traffic of one interval (the residual: 25 ms at configs[4], more than any kernel can hide inside its own
+ * interval) with the prediction of the next.  Consecutive intervals alternate between TWO arenas (140 GB at configs[4]); the call
+ * blocks until the interval before the previous one has finished, so never more than two are in flight per (host
+ * thread, device).  The host buffers of an interval -- inputs AND outputs -- belong to the library until
+ * sagecal_host_sync returns, or until the call after the next has returned; jones_host is both, so a caller that
+ * refills it before every call rotates THREE sets (when call i is made, interval i-3 is home, interval i-2 maybe not).
+ * sagecal_host_sync(stream): waits for everything the asynchronous entry enqueued from this host thread on `stream` and
+ * on the library's copy streams.  Returns 0 or SAGECAL_ECUDA.
+ */
+int sagecal_calibrate_interval_host_async(
+    int nstations, int ntime, int nchan,
+    const double* freqs_host, double f0, const double* uvw_host,
+    int nclus, const int* cluster_offset_host,
+    const double* src_l, const double* src_m, const double* src_I,
+    const double* src_Q, const double* src_U, const double* src_V, const double* src_alpha,
+    int coh_format,
+    const sagecal_c128* vis_host, sagecal_c128* jones_host, sagecal_c128* residual_host,
+    int n_em, int n_lm, double tau, int lm_mode,
+    double* cost_per_cluster_host, double* cost_trace_host, void* stream);
+int sagecal_host_sync(void* stream);
+/* sagecal_host_sync, then hands the arenas the host entries keep cached (one or two, about 70 GB each at configs[4])
+ * back to the device.  The next host-entry call allocates again. */
+int sagecal_host_trim(void* stream);
 
 /*
  * Measurement-set rows <-> canonical layout, and flags (SURVEY.md §8(f) NEXT-4 "per-row station index arrays

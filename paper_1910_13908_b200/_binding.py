@@ -68,6 +68,12 @@ def load_library():
     L.sagecal_calibrate_interval_host.restype = i
     L.sagecal_calibrate_interval_host.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp,
                                                   i, i, d, i, vp, vp, vp]
+    L.sagecal_calibrate_interval_host_async.restype = i
+    L.sagecal_calibrate_interval_host_async.argtypes = L.sagecal_calibrate_interval_host.argtypes
+    L.sagecal_host_sync.restype = i
+    L.sagecal_host_sync.argtypes = [vp]
+    L.sagecal_host_trim.restype = i
+    L.sagecal_host_trim.argtypes = [vp]
     i64 = ctypes.c_int64
     L.sagecal_rows_workspace_bytes.restype = sz
     L.sagecal_rows_workspace_bytes.argtypes = [i, i]
@@ -413,9 +419,12 @@ def calibrate_interval_host(N: int, T: int, freqs: Sequence[float], f0: float, u
                             cluster_offset: Sequence[int], src_l, src_m, src_I, src_alpha, vis: torch.Tensor,
                             jones: torch.Tensor, n_em: int, n_lm: int, tau: float = 1e-3, src_Q=None, src_U=None,
                             src_V=None, coh_format: int = COH_FULL, residual: Optional[torch.Tensor] = None,
-                            cost_per_cluster: Optional[torch.Tensor] = None, lm_mode: int = LM_COMPRESSED, stream=None):
+                            cost_per_cluster: Optional[torch.Tensor] = None, lm_mode: int = LM_COMPRESSED, stream=None,
+                            asynchronous: bool = False):
     """sagecal_calibrate_interval_host: predict + calibrate from HOST tensors (copies inside the call).
-    `jones` (CPU, [K,N,2,2]) is updated in place; `residual` (CPU) is filled if given."""
+    `jones` (CPU, [K,N,2,2]) is updated in place; `residual` (CPU) is filled if given.
+    asynchronous=True: sagecal_calibrate_interval_host_async -- returns once enqueued; every host tensor of the call
+    (inputs and outputs) must stay alive and untouched until host_sync() (at most two intervals in flight)."""
     L = load_library()
     fr = np.ascontiguousarray(freqs, dtype=np.float64)
     co = np.ascontiguousarray(cluster_offset, dtype=np.int32)
@@ -425,10 +434,21 @@ def calibrate_interval_host(N: int, T: int, freqs: Sequence[float], f0: float, u
         cost_per_cluster = torch.zeros(K, dtype=f64)
     ptrs = [_host(t, f64, n)[0] for n, t in (("src_l", src_l), ("src_m", src_m), ("src_I", src_I), ("src_Q", src_Q),
                                             ("src_U", src_U), ("src_V", src_V), ("src_alpha", src_alpha))]
-    rc = L.sagecal_calibrate_interval_host(
+    fn = L.sagecal_calibrate_interval_host_async if asynchronous else L.sagecal_calibrate_interval_host
+    rc = fn(
         N, T, F, fr.ctypes.data, float(f0), _host(uvw, f64, "uvw")[0], K, co.ctypes.data, *ptrs, coh_format,
         _host(vis, c128, "vis")[0], _host(jones, c128, "jones")[0], _host(residual, c128, "residual")[0],
         int(n_em), int(n_lm), float(tau), int(lm_mode), _host(cost_per_cluster, f64, "cost_per_cluster")[0], None,
         _stream(stream))
     _check(rc, "sagecal_calibrate_interval_host")
     return dict(jones=jones, residual=residual, cost_per_cluster=cost_per_cluster)
+
+
+def host_trim(stream=None) -> None:
+    """sagecal_host_trim: host_sync, then the arenas cached by the host entries go back to the device."""
+    _check(load_library().sagecal_host_trim(_stream(stream)), "sagecal_host_trim")
+
+
+def host_sync(stream=None) -> None:
+    """sagecal_host_sync: waits for every interval the asynchronous host entry enqueued from this thread."""
+    _check(load_library().sagecal_host_sync(_stream(stream)), "sagecal_host_sync")

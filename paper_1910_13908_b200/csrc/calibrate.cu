@@ -429,15 +429,19 @@ extern "C" int sagecal_sage_calibrate(int N, int T, int F, int K, const sagecal_
                                cost_per_cluster, cost_trace, workspace, workspace_bytes, stream, 1, nullptr, nullptr);
 }
 
-// Per (host thread, device) helpers of the host entry, created once: a PRIVATE memory pool that keeps the arena between
-// calls (intervals arrive back to back; the device's default pool and its release threshold are left alone), the copy
+// Per (host thread, device) helpers of the host entry, created once: TWO arenas the library keeps between calls
+// (intervals arrive back to back; consecutive intervals alternate between them, so that one interval's output copies
+// can still be in flight while the next is computed; plain cudaMalloc, no memory pool is touched), the copy
 // stream and the events that order it against the caller's stream.
 constexpr int HOST_FINAL_CHUNKS = 7;
 struct HostCtx {
     bool ready = false;
-    cudaMemPool_t pool = nullptr;
-    cudaStream_t cs = nullptr;
-    cudaEvent_t ev_alloc = nullptr, ev_vis = nullptr, ev_chunk[HOST_FINAL_CHUNKS + 1] = {};
+    char* arena[2] = {nullptr, nullptr};
+    size_t arena_bytes[2] = {0, 0};
+    cudaStream_t cs = nullptr, cs_out = nullptr;        // host-to-device / device-to-host copy streams
+    cudaEvent_t ev_vis = nullptr, ev_small = nullptr, ev_chunk[HOST_FINAL_CHUNKS + 1] = {};
+    cudaEvent_t ev_done[2] = {};                        // end of the last two intervals (asynchronous entry)
+    unsigned long long n_async = 0;
 };
 static int host_ctx(HostCtx** out) {
     static thread_local HostCtx ctx[64];
@@ -446,16 +450,11 @@ static int host_ctx(HostCtx** out) {
     if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
     HostCtx& c = ctx[dev];
     if (!c.ready) {
-        cudaMemPoolProps props = {};
-        props.allocType = cudaMemAllocationTypePinned;
-        props.handleTypes = cudaMemHandleTypeNone;
-        props.location.type = cudaMemLocationTypeDevice;
-        props.location.id = dev;
-        SGC_CUDA(cudaMemPoolCreate(&c.pool, &props));
-        uint64_t keep = UINT64_MAX;
-        SGC_CUDA(cudaMemPoolSetAttribute(c.pool, cudaMemPoolAttrReleaseThreshold, &keep));
         SGC_CUDA(cudaStreamCreateWithFlags(&c.cs, cudaStreamNonBlocking));
-        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_alloc, cudaEventDisableTiming));
+        SGC_CUDA(cudaStreamCreateWithFlags(&c.cs_out, cudaStreamNonBlocking));
+        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_small, cudaEventDisableTiming));
+        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_done[0], cudaEventDisableTiming));
+        SGC_CUDA(cudaEventCreateWithFlags(&c.ev_done[1], cudaEventDisableTiming));
         SGC_CUDA(cudaEventCreateWithFlags(&c.ev_vis, cudaEventDisableTiming));
         for (int i = 0; i <= HOST_FINAL_CHUNKS; i++) SGC_CUDA(cudaEventCreateWithFlags(&c.ev_chunk[i], cudaEventDisableTiming));
         c.ready = true;
@@ -478,20 +477,20 @@ static int host_final_chunk(void* ctx, int t0, int t1) {
     cudaEvent_t ev = h->c->ev_chunk[h->n < HOST_FINAL_CHUNKS ? h->n : HOST_FINAL_CHUNKS];
     h->n++;
     SGC_CUDA(cudaEventRecord(ev, h->st));
-    SGC_CUDA(cudaStreamWaitEvent(h->c->cs, ev, 0));
+    SGC_CUDA(cudaStreamWaitEvent(h->c->cs_out, ev, 0));
     SGC_CUDA(cudaMemcpyAsync(h->host_res + (size_t)t0 * h->bytes_slot, h->dev_res + (size_t)t0 * h->bytes_slot,
-                             (size_t)(t1 - t0) * h->bytes_slot, cudaMemcpyDeviceToHost, h->c->cs));
+                             (size_t)(t1 - t0) * h->bytes_slot, cudaMemcpyDeviceToHost, h->c->cs_out));
     return SAGECAL_OK;
 }
 
-extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double* freqs_host, double f0,
-                                               const double* uvw_host, int K, const int* cluster_offset_host,
-                                               const double* src_l, const double* src_m, const double* src_I,
-                                               const double* src_Q, const double* src_U, const double* src_V,
-                                               const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
-                                               sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
-                                               int n_lm, double tau, int lm_mode, double* cost_per_cluster_host,
-                                               double* cost_trace_host, void* stream) {
+static int host_interval(int N, int T, int F, const double* freqs_host, double f0,
+                         const double* uvw_host, int K, const int* cluster_offset_host,
+                         const double* src_l, const double* src_m, const double* src_I,
+                         const double* src_Q, const double* src_U, const double* src_V,
+                         const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
+                         sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
+                         int n_lm, double tau, int lm_mode, double* cost_per_cluster_host,
+                         double* cost_trace_host, void* stream, bool async) {
     if (N < 2 || T < 1 || F < 1 || K < 1 || n_em < 0 || n_lm < 0) return SAGECAL_EINVAL;
     if (!freqs_host || !uvw_host || !cluster_offset_host || !vis_host || !jones_host || !cost_per_cluster_host)
         return SAGECAL_EINVAL;
@@ -515,11 +514,22 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     const size_t o_uvw = take((size_t)rows * 24), o_src = take(7 * sS), o_vis = take(vis_bytes), o_res = take(vis_bytes),
                  o_coh = take(coh_bytes), o_jon = take((size_t)K * N * 64), o_cpc = take(sizeof(double) * K),
                  o_trc = take(sizeof(double) * ntrace), o_wsp = take(ws_pred), o_wsc = take(ws_cal);
-    char* arena = nullptr;
     HostCtx* hc = nullptr;
     int rc = host_ctx(&hc);
     if (rc) return rc;
-    SGC_CUDA(cudaMallocFromPoolAsync((void**)&arena, off, hc->pool, st));
+    // Consecutive intervals alternate between the two arenas; at most two are in flight: wait for the interval that
+    // used this arena last (the one before the previous one).
+    // The synchronous entry waits for everything in flight and always takes the first arena.
+    const int slot = async ? (int)(hc->n_async & 1) : 0;
+    SGC_CUDA(cudaEventSynchronize(hc->ev_done[slot]));
+    if (!async) SGC_CUDA(cudaEventSynchronize(hc->ev_done[1]));
+    if (hc->arena_bytes[slot] < off) {
+        if (hc->arena[slot]) SGC_CUDA(cudaFree(hc->arena[slot]));
+        hc->arena[slot] = nullptr; hc->arena_bytes[slot] = 0;
+        SGC_CUDA(cudaMalloc((void**)&hc->arena[slot], off));
+        hc->arena_bytes[slot] = off;
+    }
+    char* arena = hc->arena[slot];
     auto h2d_on = [&](cudaStream_t s, size_t o, const void* src, size_t n) {
         if (rc == SAGECAL_OK && src && n) {
             cudaError_t e = cudaMemcpyAsync(arena + o, src, n, cudaMemcpyHostToDevice, s);
@@ -530,12 +540,7 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
     // the visibilities (the bulk of the input) travel on a second stream while `st` predicts the coherencies,
     // which need only uvw and the source table; `st` joins before the calibration reads them
     cudaStream_t cs = hc->cs;
-    cudaEvent_t ev_alloc = hc->ev_alloc, ev_vis = hc->ev_vis;
-    if (rc == SAGECAL_OK) {
-        cudaError_t e = cudaEventRecord(ev_alloc, st);
-        if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_alloc, 0);
-        if (e != cudaSuccess) rc = cuda_fail(e);
-    }
+    cudaEvent_t ev_vis = hc->ev_vis;
     h2d(o_uvw, uvw_host, (size_t)rows * 24);
     const double* cols[7] = {src_l, src_m, src_I, src_alpha, src_Q, src_U, src_V};
     double* dcol[7];
@@ -568,22 +573,83 @@ extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double
                                  (sagecal_c128*)(arena + o_res), n_em, n_lm, tau, lm_mode, (double*)(arena + o_cpc),
                                  cost_trace_host ? (double*)(arena + o_trc) : nullptr, arena + o_wsc, ws_cal, st,
                                  HOST_FINAL_CHUNKS, host_final_chunk, &hf);
+    // All device-to-host traffic goes on the output copy stream: a copy enqueued on `st` would queue behind the residual's
+    // chunks on the copy engine and hold `st` (and with it the next interval's prediction) for their 25 ms.  The
+    // interval is over for the arena when that stream has passed the last copy; `st` itself is free for the next
+    // interval at once (the asynchronous entry).
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaEventRecord(hc->ev_small, st);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(hc->cs_out, hc->ev_small, 0);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+    }
     auto d2h = [&](void* dst, size_t o, size_t n) {
         if (rc == SAGECAL_OK && dst && n) {
-            cudaError_t e = cudaMemcpyAsync(dst, arena + o, n, cudaMemcpyDeviceToHost, st);
+            cudaError_t e = cudaMemcpyAsync(dst, arena + o, n, cudaMemcpyDeviceToHost, hc->cs_out);
             if (e != cudaSuccess) rc = cuda_fail(e);
         }
     };
     d2h(jones_host, o_jon, (size_t)K * N * 64);
     d2h(cost_per_cluster_host, o_cpc, sizeof(double) * K);
     d2h(cost_trace_host, o_trc, sizeof(double) * ntrace);
-    // the residual's copies (and, on an error path, the visibilities') are on the copy stream: the arena is freed on
-    // `st` only after they are done
+    if (rc == SAGECAL_OK) {
+        cudaError_t e = cudaEventRecord(hc->ev_done[slot], hc->cs_out);
+        if (e != cudaSuccess) rc = cuda_fail(e);
+        if (rc == SAGECAL_OK && async) { hc->n_async++; return rc; }
+    }
+    // synchronous entry, or an error: wait for every stream that may touch the arena or the host buffers
     cudaError_t e0 = cudaStreamSynchronize(cs);
-    cudaError_t e1 = cudaFreeAsync(arena, st);
+    cudaError_t e1 = cudaStreamSynchronize(hc->cs_out);
     cudaError_t e2 = cudaStreamSynchronize(st);
     if (rc == SAGECAL_OK && e0 != cudaSuccess) rc = cuda_fail(e0);
     if (rc == SAGECAL_OK && e1 != cudaSuccess) rc = cuda_fail(e1);
     if (rc == SAGECAL_OK && e2 != cudaSuccess) rc = cuda_fail(e2);
     return rc;
+}
+
+extern "C" int sagecal_calibrate_interval_host(int N, int T, int F, const double* freqs_host, double f0,
+                                               const double* uvw_host, int K, const int* cluster_offset_host,
+                                               const double* src_l, const double* src_m, const double* src_I,
+                                               const double* src_Q, const double* src_U, const double* src_V,
+                                               const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
+                                               sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
+                                               int n_lm, double tau, int lm_mode, double* cost_per_cluster_host,
+                                               double* cost_trace_host, void* stream) {
+    return host_interval(N, T, F, freqs_host, f0, uvw_host, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
+                         src_alpha, coh_format, vis_host, jones_host, residual_host, n_em, n_lm, tau, lm_mode,
+                         cost_per_cluster_host, cost_trace_host, stream, false);
+}
+
+extern "C" int sagecal_calibrate_interval_host_async(int N, int T, int F, const double* freqs_host, double f0,
+                                                     const double* uvw_host, int K, const int* cluster_offset_host,
+                                                     const double* src_l, const double* src_m, const double* src_I,
+                                                     const double* src_Q, const double* src_U, const double* src_V,
+                                                     const double* src_alpha, int coh_format, const sagecal_c128* vis_host,
+                                                     sagecal_c128* jones_host, sagecal_c128* residual_host, int n_em,
+                                                     int n_lm, double tau, int lm_mode, double* cost_per_cluster_host,
+                                                     double* cost_trace_host, void* stream) {
+    return host_interval(N, T, F, freqs_host, f0, uvw_host, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
+                         src_alpha, coh_format, vis_host, jones_host, residual_host, n_em, n_lm, tau, lm_mode,
+                         cost_per_cluster_host, cost_trace_host, stream, true);
+}
+
+extern "C" int sagecal_host_sync(void* stream) {
+    HostCtx* hc = nullptr;
+    int rc = host_ctx(&hc);
+    if (rc) return rc;
+    SGC_CUDA(cudaStreamSynchronize(hc->cs));
+    SGC_CUDA(cudaStreamSynchronize((cudaStream_t)stream));
+    SGC_CUDA(cudaStreamSynchronize(hc->cs_out));
+    return SAGECAL_OK;
+}
+
+extern "C" int sagecal_host_trim(void* stream) {
+    int rc = sagecal_host_sync(stream);
+    if (rc) return rc;
+    HostCtx* hc = nullptr;
+    if ((rc = host_ctx(&hc))) return rc;
+    for (int i = 0; i < 2; i++) {
+        if (hc->arena[i]) SGC_CUDA(cudaFree(hc->arena[i]));
+        hc->arena[i] = nullptr; hc->arena_bytes[i] = 0;
+    }
+    return SAGECAL_OK;
 }

@@ -261,6 +261,47 @@ def test_calibrate_host_entry(cuda_device):
     assert np.array_equal(out["cost_per_cluster"].numpy(), host(ref["cost_per_cluster"]))
 
 
+def test_calibrate_host_entry_async_stream_of_intervals(cuda_device):
+    """sagecal_calibrate_interval_host_async: five different intervals enqueued back to back (two sets of host buffers,
+    alternating; never more than two in flight), one sagecal_host_sync between reuse: each comes back bit-identical to
+    the synchronous entry on the same inputs."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    probs, want = [], []
+    for i in range(5):
+        p = make_config(1, seed=4000 + i)
+        V = oracle.simulate(p, oracle.predict(p))
+        args = (p.N, p.T, p.freqs, p.f0, t(p.uvw), p.cluster_offset, t(p.src_l), t(p.src_m), t(p.src_I), t(p.src_alpha), t(V))
+        J = t(p.jones_init())
+        R = torch.empty((p.rows, p.F, 4), dtype=torch.complex128).pin_memory()
+        out = sg.calibrate_interval_host(*args, J, 2, 4, p.tau, residual=R)
+        want.append((J.numpy().copy(), R.numpy().copy(), out["cost_per_cluster"].numpy().copy()))
+        probs.append((p, args))
+    sets = [dict(J=t(probs[0][0].jones_init()), R=torch.empty_like(R).pin_memory(),
+                 C=torch.zeros(1, dtype=torch.float64).pin_memory()) for _ in range(2)]
+    snap = lambda b: (b["J"].numpy().copy(), b["R"].numpy().copy(), b["C"].numpy().copy())
+    got, pending = {}, {}                                # pending: buffer set -> the interval it carries
+    for i, (p, args) in enumerate(probs):
+        k = i & 1
+        if k in pending:                                 # the set is reused: everything in flight must be home first
+            sg.host_sync()
+            for kk, ii in pending.items():
+                got[ii] = snap(sets[kk])
+            pending.clear()
+        b = sets[k]
+        b["J"].copy_(torch.from_numpy(p.jones_init()))
+        sg.calibrate_interval_host(*args, b["J"], 2, 4, p.tau, residual=b["R"], cost_per_cluster=b["C"], asynchronous=True)
+        pending[k] = i
+    sg.host_sync()
+    for kk, ii in pending.items():
+        got[ii] = snap(sets[kk])
+    assert sorted(got) == [0, 1, 2, 3, 4]
+    for i in range(5):
+        for a, w in zip(got[i], want[i]):
+            assert np.array_equal(a, w), i
+
+
 @pytest.mark.parametrize("fmt", ["full", "scalar"])
 def test_calibrate_compressed_is_bit_reproducible(cuda_device, fmt):
     """No atomics in any sum and a fixed summation order: repeated runs on the same inputs give bit-identical Jones,
