@@ -442,29 +442,63 @@ __device__ __forceinline__ void rec_load(const double* base, bool on, double2* t
 #pragma unroll
     for (int x = 0; x < MS_NV / 2; x++) t[x] = on ? __ldcg(rec + x) : make_double2(0.0, 0.0);
 }
-__device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, const StationPlan& sp, int lane, double x0, double x1) {
+// A station with many column records (up to one per chunk of its segment: 128 at N = 512, 255 at N = 256) would keep
+// its warp busy long after the others are done, and the grid barrier waits for the slowest: when every warp owns at
+// most one station, the otherwise idle warps of the CTA join a TEAM (Team: `size` warps, this warp is `member`, member
+// 0 owns the station).  The members take the 32-record batches of the column records in turn, each sums its share by
+// the same halving exchange, the helpers hand their 12 partial sums over through shared memory and a named barrier of
+// the team, and the owner adds them in member order.  Fixed order: bit-reproducible.
+struct Team { int size, member, owner_warp, stride; };   // member j of the team is warp owner_warp + j * stride
+__device__ __forceinline__ StAcc station_reduce(const MstepArgs& A, const StationPlan& sp, int lane, double x0, double x1,
+                                                const Team& tm, double* s_team) {
     const MGeom& g = A.g;
     double acc[16];
 #pragma unroll
     for (int x = 0; x < 16; x++) acc[x] = 0.0;
-    for (int i = 0; i < sp.nrow || 4 * i < sp.nc; i += 32) {
-        double2 tr[MS_NV / 2], tc[4][MS_NV / 2];
-        const int qt = sp.qt0 + i + lane;
-        rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + sp.s) * MS_NV, i + lane < sp.nrow, tr);
+    // the owner's row records (at most one per column segment) and the member's first four column batches are loaded
+    // before the first addition
+    double2 tr[MS_NV / 2];
+    {
+        const int qt = sp.qt0 + lane;
+        rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + sp.s) * MS_NV, tm.member == 0 && lane < sp.nrow, tr);
+    }
+    for (int b0 = tm.member; 32 * b0 < sp.nc; b0 += 4 * tm.size) {
+        double2 tc[4][MS_NV / 2];
 #pragma unroll
         for (int u = 0; u < 4; u++) {
-            const int c = 4 * i + 32 * u + lane;
+            const int c = 32 * (b0 + u * tm.size) + lane;
             rec_load(sp.colbase + (size_t)(c < sp.nc ? c : 0) * MS_TQ * MS_NV, c < sp.nc, tc[u]);
         }
 #pragma unroll
         for (int x = 0; x < MS_NV / 2; x++) {
-            acc[2 * x] += tr[x].x; acc[2 * x + 1] += tr[x].y;
 #pragma unroll
             for (int u = 0; u < 4; u++) { acc[2 * x] += tc[u][x].x; acc[2 * x + 1] += tc[u][x].y; }
         }
     }
-    acc[12] = x0; acc[13] = x1;
+#pragma unroll
+    for (int x = 0; x < MS_NV / 2; x++) { acc[2 * x] += tr[x].x; acc[2 * x + 1] += tr[x].y; }
+    if (tm.member == 0) {
+        for (int i = 32; i < sp.nrow; i += 32) {          // more than 32 column segments (N > 1024)
+            const int qt = sp.qt0 + i + lane;
+            rec_load(A.Ppart + (size_t)(g.ubase(qt < g.nqt ? qt : 0) + sp.s) * MS_NV, i + lane < sp.nrow, tr);
+#pragma unroll
+            for (int x = 0; x < MS_NV / 2; x++) { acc[2 * x] += tr[x].x; acc[2 * x + 1] += tr[x].y; }
+        }
+        acc[12] = x0; acc[13] = x1;
+    }
     halve_sum16(acc, lane);
+    const int idx = halve_index(lane);
+    if (tm.size > 1) {
+        const int id = 1 + tm.owner_warp, cnt = 32 * tm.size;
+        if (tm.member > 0) {
+            if (!(lane & 1) && idx < MS_NV) s_team[(tm.owner_warp + tm.member * tm.stride) * MS_NV + idx] = acc[0];
+            asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(cnt) : "memory");
+            return StAcc();
+        }
+        asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(cnt) : "memory");
+        if (idx < MS_NV)
+            for (int j = 1; j < tm.size; j++) acc[0] += s_team[(tm.owner_warp + j * tm.stride) * MS_NV + idx];
+    }
     double t[14];
 #pragma unroll
     for (int x = 0; x < 14; x++) t[x] = __shfl_sync(0xffffffffu, acc[0], 2 * x);     // lane 2x holds index x
@@ -553,6 +587,23 @@ mstep_kernel(const MstepArgs A) {
     StationPlan sp0;
     sp0.s = gw; sp0.qt0 = 0; sp0.nrow = 0; sp0.nc = 0; sp0.colbase = A.Qpart;
     if (gw < N) sp0 = make_station_plan(A, gw);
+    // teams (station_reduce): with at most one station per warp, stations sit on warps 0 .. ns_w-1 of a CTA and the
+    // warps above them help: member j of the team of owner warp o is warp o + j * ns_w
+    __shared__ double s_team[MS_WARPS * MS_NV];
+    Team tm;
+    tm.size = 1; tm.member = 0; tm.owner_warp = warp; tm.stride = 1;
+    {
+        const int ns_w = (N + (int)gridDim.x - 1) / (int)gridDim.x;
+        if (nw >= N && ns_w <= MS_WARPS / 2) {
+            tm.size = MS_WARPS / ns_w; tm.stride = ns_w; tm.owner_warp = warp % ns_w; tm.member = warp / ns_w;
+            if (tm.member > 0) {
+                const int ts = tm.owner_warp * (int)gridDim.x + (int)blockIdx.x;      // the team's station
+                sp0.s = N;
+                if (tm.member < tm.size && ts < N) sp0 = make_station_plan(A, ts);
+            }
+        }
+    }
+    const bool owner = tm.member == 0 && sp0.s < N, helper = tm.member > 0 && sp0.s < N;
 
     // LM state, identical in every thread that owns a station
     double phi = 0.0, mu = A.init ? 0.0 : A.ctl->mu, nu = A.init ? 2.0 : A.ctl->nu;
@@ -573,10 +624,11 @@ mstep_kernel(const MstepArgs A) {
         if (e == 0 && A.init) {
             // (phi, G, M) at the centre are the accepted state; mu = tau * max_p max(M_p00, M_p11)
             double mm = 0.0;
-            if (sp0.s < N) {
+            if (helper) station_reduce(A, sp0, lane, 0.0, 0.0, tm, s_team);
+            if (owner) {
                 const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
                 for (int s = sp0.s; s < N; s += nw) {
-                    const StAcc r = station_reduce(A, s == sp0.s ? sp0 : make_station_plan(A, s), lane, strided_partial(cost_l), 0.0);
+                    const StAcc r = station_reduce(A, s == sp0.s ? sp0 : make_station_plan(A, s), lane, strided_partial(cost_l), 0.0, tm, s_team);
                     if (lane == 0) {
 #pragma unroll
                         for (int x = 0; x < 4; x++) { st_c(A.G + 4 * s + x, r.g[x]); st_c(A.M + 4 * s + x, r.m[x]); }
@@ -589,7 +641,7 @@ mstep_kernel(const MstepArgs A) {
             __syncthreads();
             if (threadIdx.x == 0) publish(sm.s_red + 2 * MS_WARPS, A.mm_cta, true);
             grid_barrier(A.bar, ++gen);
-            if (sp0.s < N) {
+            if (owner) {
                 mu = A.tau * strided_max(strided_load(A.mm_cta, (int)gridDim.x, lane));
                 nu = 2.0;
                 if (!(mu >= 1e-300)) mu = 1e-300;
@@ -603,7 +655,9 @@ mstep_kernel(const MstepArgs A) {
                     }
                 }
             }
-        } else if (sp0.s < N) {
+        } else if (helper) {
+            station_reduce(A, sp0, lane, 0.0, 0.0, tm, s_team);
+        } else if (owner) {
             // All loads are issued before anything is consumed: the CTA partials, the accepted (G, M, J) and the trial
             // J of the station (16 complex numbers: lane x & 15 holds one), then its records.
             const Strided cost_l = strided_load(A.cost_cta, (int)gridDim.x, lane);
@@ -614,7 +668,7 @@ mstep_kernel(const MstepArgs A) {
                 return ldcg_c(src + 4 * s + (which & 3));
             };
             cplx mine = old_elem(sp0.s);
-            StAcc r = station_reduce(A, sp0, lane, strided_partial(cost_l), strided_partial(pred_l));
+            StAcc r = station_reduce(A, sp0, lane, strided_partial(cost_l), strided_partial(pred_l), tm, s_team);
             const double fresh = r.x0;
             bool accept = false;
             if (e == 0) {
@@ -641,7 +695,7 @@ mstep_kernel(const MstepArgs A) {
             for (int s = sp0.s; s < N; s += nw) {
                 if (s != sp0.s) {
                     mine = old_elem(s);
-                    r = station_reduce(A, make_station_plan(A, s), lane, 0.0, 0.0);
+                    r = station_reduce(A, make_station_plan(A, s), lane, 0.0, 0.0, tm, s_team);
                 }
                 cplx g4[4], m4[4], jj[4];
 #pragma unroll
