@@ -12,18 +12,20 @@
 //                  exchange over the lanes (16 additions per row instead of 60), one record per row.  Column-station
 //                  sums: one record per (chunk, column).  Cost: one sum per CTA.
 //      -- grid barrier --
-//   B  control   : every warp adds the CTA costs and the CTAs' predicted reductions in the same fixed order
-//                  (identical in all CTAs), takes the accept/reject decision and updates mu, nu.  Warp <-> station:
-//                  adds the station's records (lanes over records, butterfly), commits or discards the trial, solves
-//                  dJ_p = G_p (M_p + mu I)^-1, writes the next trial Jones; the predicted reduction is summed per CTA.
+//   B  control   : every station-owning warp adds the CTA costs and the CTAs' predicted reductions in the same fixed
+//                  order (identical everywhere), takes the accept/reject decision and updates mu, nu.  Warp <->
+//                  station: adds the station's records (all loads in flight together, one halving exchange; the
+//                  CTA's idle warps help as a team when a station has many column records), commits or discards the
+//                  trial, solves dJ_p = G_p (M_p + mu I)^-1, writes the next trial Jones; the predicted reduction
+//                  is summed per CTA.
 //      -- grid barrier --
 //
-// No atomics in the sums, fixed summation order: bit-reproducible for a given grid.  All CTAs are co-resident
-// (cooperative launch, or one thread-block cluster for small arrays); the grid barrier is an arrive counter in device
-// memory (one red.release per CTA, relaxed polling, one acquire fence: 1.25 us at 148 CTAs, measured against
-// cooperative_groups' grid.sync() at 1.2 us, which however makes every warp invalidate its L1, and against
-// one-flag-per-CTA schemes at 2.5 us) or the hardware cluster barrier.  Everything that crosses CTAs is read with
-// ld.cg (L2).
+// No atomics in the sums, fixed summation order: bit-reproducible for a given grid.  mstep_kernel: cooperative launch,
+// all CTAs co-resident, the grid barrier is an arrive counter in device memory (one red.release per CTA, relaxed
+// polling, one acquire fence: 1.25 us at 148 CTAs, measured against cooperative_groups' grid.sync() at 1.2 us, which
+// however makes every warp invalidate its L1, and against one-flag-per-CTA schemes at 2.5 us); everything that crosses
+// CTAs is read with ld.cg (L2).  mstep_cluster_kernel (N <= 64): one thread-block cluster, the same two phases with
+// every exchange in distributed shared memory and the hardware cluster barrier.
 #include <math.h>
 #include <mutex>
 #include <cooperative_groups.h>
