@@ -23,6 +23,7 @@ namespace sgc {
 constexpr int PRED_THREADS = 128;
 constexpr int PRED_MAXF = 512;
 constexpr int PRED_MAXK = 1024;
+constexpr int PRED_RPT = 2;           // rows per thread of the unpolarised float64 prediction (predict2_kernel)
 
 struct PredFreqs { double kf[PRED_MAXF]; };          // f_c / c0  [1/m]
 struct PredClusters { int off[PRED_MAXK + 1]; };
@@ -319,6 +320,109 @@ predict_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClus
     }
 }
 
+// ---- unpolarised float64 prediction, RPT rows per thread ---------------------------------------------------------------
+// The hot loop is held back by its shared-memory reads (profiles/r02_ncu_full_predict_cfg4.md): with RPT = 2 rows per
+// thread a source's position and its FT fluxes are read once for both.  Rows r, r + 128, ... of an RPT x 128-row tile, so
+// that a warp's uvw reads and coherency stores stay contiguous.  Same arithmetic per (row, source) as predict_kernel:
+// bit-identical output.
+template <int FT, bool UNIFORM, bool SCALAR, int RPT, int MINB>
+__global__ void __launch_bounds__(PRED_THREADS, MINB)
+predict2_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClusters cl,
+                const double* __restrict__ uvw, const double* __restrict__ src_l,
+                const double* __restrict__ src_m, const double* __restrict__ nm1_g,
+                const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh) {
+    constexpr int ST = 128;
+    __shared__ double s_l[ST], s_m[ST], s_n[ST];
+    __shared__ __align__(16) double s_fl[ST * FT];
+    __shared__ double2 s_tab_all[64 * 8];
+    if (threadIdx.x < 64) {
+        double sn, cs;
+        sincospi((double)threadIdx.x * 0.03125, &sn, &cs);
+#pragma unroll
+        for (int c = 0; c < 8; c++) s_tab_all[8 * threadIdx.x + c] = make_double2(cs, sn);
+    }
+    const unsigned s_tab = (unsigned)__cvta_generic_to_shared(s_tab_all + (threadIdx.x & 7));
+    const int k = blockIdx.y;
+    const int s_begin = cl.off[k], s_end = cl.off[k + 1];
+    int64_t r[RPT];
+    bool live[RPT];
+    double u[RPT], v[RPT], w[RPT];
+#pragma unroll
+    for (int t = 0; t < RPT; t++) {
+        r[t] = (int64_t)blockIdx.x * (RPT * PRED_THREADS) + t * PRED_THREADS + threadIdx.x;
+        live[t] = r[t] < rows;
+        u[t] = v[t] = w[t] = 0.0;
+        if (live[t]) { u[t] = uvw[3 * r[t]]; v[t] = uvw[3 * r[t] + 1]; w[t] = uvw[3 * r[t] + 2]; }
+    }
+    for (int c0 = 0; c0 < Fpad; c0 += FT) {
+        cplx acc[RPT][FT][1];
+#pragma unroll
+        for (int t = 0; t < RPT; t++)
+#pragma unroll
+            for (int c = 0; c < FT; c++) acc[t][c][0] = mk(0.0, 0.0);
+        for (int sb = s_begin; sb < s_end; sb += ST) {
+            const int ns = min(ST, s_end - sb);
+            __syncthreads();
+            for (int i = threadIdx.x; i < ns; i += PRED_THREADS) {
+                s_l[i] = src_l[sb + i]; s_m[i] = src_m[sb + i]; s_n[i] = nm1_g[sb + i];
+            }
+            for (int i = threadIdx.x; i < ns * FT; i += PRED_THREADS) {
+                const int s = i / FT, rem = i - s * FT;
+                s_fl[i] = flux_g[(size_t)(sb + s) * Fpad + c0 + rem];
+            }
+            __syncthreads();
+            for (int s = 0; s < ns; s++) {
+                const double sl = s_l[s], smm = s_m[s], sn = s_n[s];
+                double fl[FT];
+#pragma unroll
+                for (int c = 0; c < FT; c++) fl[c] = s_fl[s * FT + c];
+#pragma unroll
+                for (int t = 0; t < RPT; t++) {
+                    const double ph = fma(w[t], sn, fma(v[t], smm, u[t] * sl));  // metres
+                    double er, ei, dr = 1.0, di = 0.0;
+                    double pr = 0.0, pi_ = 0.0, twodr = 2.0;
+                    if (UNIFORM) {
+                        phasor_f64(ph * fr.kf[c0], s_tab, er, ei);
+                        if (FT > 1) { phasor_f64(ph * dkf, s_tab, dr, di); twodr = dr + dr; }
+                    }
+#pragma unroll
+                    for (int c = 0; c < FT; c++) {
+                        if (!UNIFORM) phasor_f64(ph * fr.kf[min(c0 + c, PRED_MAXF - 1)], s_tab, er, ei);
+                        acc[t][c][0].re = fma(fl[c], er, acc[t][c][0].re);
+                        acc[t][c][0].im = fma(fl[c], ei, acc[t][c][0].im);
+                        if (UNIFORM && c + 1 < FT) {
+                            double nr, ni;
+                            if (c == 0) { nr = fma(-ei, di, er * dr); ni = fma(ei, dr, er * di); }
+                            else { nr = fma(twodr, er, -pr); ni = fma(twodr, ei, -pi_); }
+                            pr = er; pi_ = ei;
+                            er = nr; ei = ni;
+                        }
+                    }
+                }
+            }
+        }
+#pragma unroll
+        for (int t = 0; t < RPT; t++) {
+            if (!live[t]) continue;
+            if (SCALAR) {
+                sagecal_c128* o = coh + ((size_t)k * rows + r[t]) * F + c0;
+#pragma unroll
+                for (int c = 0; c < FT; c++)
+                    if (c0 + c < F) { o[c].re = acc[t][c][0].re; o[c].im = acc[t][c][0].im; }
+            } else {
+                sagecal_c128* o = coh + (((size_t)k * rows + r[t]) * F + c0) * 4;
+#pragma unroll
+                for (int c = 0; c < FT; c++) {
+                    if (c0 + c < F) {
+                        stg256(o + 4 * c, acc[t][c][0].re, acc[t][c][0].im, 0.0, 0.0);
+                        stg256(o + 4 * c + 2, 0.0, 0.0, acc[t][c][0].re, acc[t][c][0].im);
+                    }
+                }
+            }
+        }
+    }
+}
+
 template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
 static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
                           const PredClusters& cl, const double* uvw, const double* l, const double* m,
@@ -340,6 +444,12 @@ static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int F
             ready[dev] = true;
         }
         kern<<<dim3(grid.x, 1), PRED_THREADS, smem, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m, nm1, flux, coh, *rs);
+    } else if (!POL && !MIXED) {
+        // two rows per thread at four CTAs per SM (127 registers, no spills): 28.8 ms at configs[4] against 31.4 for
+        // one row per thread, 29.1 at three CTAs per SM, 30.2 with three rows per thread
+        const dim3 g2((unsigned)((rows + PRED_RPT * PRED_THREADS - 1) / (PRED_RPT * PRED_THREADS)), grid.y);
+        predict2_kernel<FT, UNIFORM, SCALAR, PRED_RPT, 4><<<g2, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m, nm1,
+                                                                                  flux, coh);
     } else {
         predict_kernel<FT, POL, UNIFORM, SCALAR, MIXED, false><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw,
                                                                                      l, m, nm1, flux, coh, PredResid{});
