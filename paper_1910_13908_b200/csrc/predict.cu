@@ -12,9 +12,10 @@
 // sin/cos(2 pi r) from degree-7/8 Taylor polynomials in r (remainders 5e-18 / 2e-20): 16 FP64 instructions per phasor
 // against ~29 for sincospi(), same accuracy (a few 1e-16 absolute).
 // precision = 1 (MIXED): the phase in cycles and its range reduction x - rint(x) stay in
-// float64 (phases reach 3.3e3 cycles: float32 would leave 1e-4 cycles), then sincospif, the channel recurrence and
-// the flux products run in float32; products are summed in float32 over at most 32 sources and those partial sums
-// are added to the float64 accumulators.  Error ~1e-6 relative; the parity bound is 1e-5 (BASELINE.json:5).
+// float64 (phases reach 3.3e3 cycles: float32 would leave 1e-4 cycles), then the phasor (sin.approx / cos.approx),
+// the channel recurrence and the flux products run in float32; products are summed in float32 over at most 32 sources
+// and those partial sums are added to the float64 accumulators.  Error ~2e-6 relative; the parity bound is 1e-5
+// (BASELINE.json:5).
 #include <mutex>
 #include "common.cuh"
 
@@ -90,11 +91,15 @@ __device__ __forceinline__ void phasor_f64(double x, unsigned tab, double& er, d
     er = fma(-ty, sp, tx * cp);                                  // cos(a + b)
     ei = -fma(tx, sp, ty * cp);                                  // -sin(a + b)
 }
+// float32 phasor of the MIXED arm: exact reduction to |r| <= 1/2 cycle in float64 (magic-number rounding: three DADDs,
+// no FRND.F64), then the hardware approximations sin.approx / cos.approx (MUFU) on 2 pi r in [-pi, pi], where their
+// absolute error is 2^-21.4 / 2^-21.2: configs[4] 20.9 ms with 1.7e-6 relative error against 25.7 ms / 5.8e-7 with
+// sincospif (only the first channel's phasor from MUFU: 23.6 ms / 6.8e-7); the parity bound is 1e-5.
 __device__ __forceinline__ void phasor_f32(double cycles, float& er, float& ei) {   // exp(-2 pi i cycles)
-    const float r = (float)(cycles - rint(cycles));          // exact reduction in float64, |r| <= 1/2
-    float sn, cs;
-    sincospif(2.0f * r, &sn, &cs);
-    er = cs; ei = -sn;
+    const double MAGIC = PHC[8];
+    const double kd = (cycles + MAGIC) - MAGIC;              // rint(cycles) for |cycles| < 2^51
+    const float a = 6.283185307179586f * (float)(cycles - kd);
+    er = __cosf(a); ei = -__sinf(a);
 }
 // RESID (sagecal_predict_residual): the CTA loops ALL clusters for its 128 rows, and next to writing C_k it takes
 // R = V - sum_k J_k,p C_k J_k,q^H along: the rows' residual tile (FT channels x 4 correlations per thread) sits in

@@ -124,7 +124,7 @@ def test_predict_errors(cuda_device):
 
 @pytest.mark.parametrize("case", ["cfg1", "cfg2-scalar", "polarised", "nonuniform"])
 def test_predict_mixed_precision_variant(cuda_device, case):
-    """precision=1 (float64 phase and range reduction, float32 sincos / recurrence / flux products, float64
+    """precision=1 (float64 phase and range reduction, float32 phasor (sin.approx / cos.approx) / recurrence / flux products, float64
     accumulation of 32-source partial sums): 1e-5 relative against the float64 oracle (BASELINE.json:5), and
     clearly not the float64 path (error above 1e-10)."""
     import paper_1910_13908_b200 as sg
