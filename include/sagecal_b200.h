@@ -53,6 +53,7 @@ typedef struct { double re, im; } sagecal_c128;
 #define SAGECAL_EWORKSPACE   (-2)  /* workspace NULL or smaller than sagecal_workspace_bytes() */
 #define SAGECAL_ECUDA        (-3)  /* a CUDA call failed: see sagecal_last_cuda_error() */
 #define SAGECAL_EUNSUPPORTED (-4)  /* valid request this build does not implement */
+#define SAGECAL_ESTATICLIMIT (-5)  /* request exceeds the fixed device scratch of a no-allocation entry point */
 
 #define SAGECAL_COH_FULL   0
 #define SAGECAL_COH_SCALAR 1
@@ -132,6 +133,31 @@ int sagecal_predict_coherencies(
     const double* src_alpha,
     int coh_format, sagecal_c128* coh, int precision,
     void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * sagecal_predict_coherencies for callers that cannot allocate device memory (code under CUDA graph capture, serving
+ * loops, harnesses that forbid cudaMalloc): same arguments without the workspace, same kernels, same result bit for
+ * bit.  The prepared source table lives in a fixed device array of SAGECAL_PREDICT_STATIC_BYTES that every GPU which
+ * loads the library holds until the process exits; the call allocates and frees nothing (no cudaMalloc / cudaFree, no
+ * allocating library routine) and makes no host<->device copy.
+ * Limit: sagecal_predict_workspace_bytes(nchan, S_tot) <= sagecal_predict_static_bytes() (2 MiB: e.g. 7 900 sources
+ * x 8 channels, almost 4 times configs[4]'s sky model); beyond it the call returns SAGECAL_ESTATICLIMIT and launches nothing.
+ * All calls on a device share the one array, which keeps the previous call's table; every call rewrites the part it
+ * reads, so nothing needs clearing.  Calls that may overlap on the GPU (different streams, or two host threads) RACE
+ * on it: serialise them on one stream, or use sagecal_predict_coherencies with a workspace per stream.
+ */
+#define SAGECAL_PREDICT_STATIC_BYTES (2 * 1024 * 1024)
+size_t sagecal_predict_static_bytes(void);
+int sagecal_predict_coherencies_static(
+    int nstations, int ntime, int nchan,
+    const double* freqs_host, double f0,
+    const double* uvw,
+    int nclus, const int* cluster_offset_host,
+    const double* src_l, const double* src_m,
+    const double* src_I, const double* src_Q, const double* src_U, const double* src_V,
+    const double* src_alpha,
+    int coh_format, sagecal_c128* coh, int precision,
+    void* stream);
 
 /*
  * Prediction fused with the initial residual (rows 8a-0 .. 8a-2 of SURVEY.md §8(a) in one pass; BASELINE.json:5 "the

@@ -57,6 +57,10 @@ def load_library():
     L.sagecal_predict_workspace_bytes.argtypes = [i, i]
     L.sagecal_predict_coherencies.restype = i
     L.sagecal_predict_coherencies.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, i, vp, sz, vp]
+    L.sagecal_predict_static_bytes.restype = sz
+    L.sagecal_predict_static_bytes.argtypes = []
+    L.sagecal_predict_coherencies_static.restype = i
+    L.sagecal_predict_coherencies_static.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, i, vp]
     L.sagecal_predict_residual.restype = i
     L.sagecal_predict_residual.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, vp, vp, vp, vp, sz, vp]
     L.sagecal_corrupt_subtract.restype = i
@@ -202,6 +206,43 @@ def predict_coherencies(N: int, T: int, freqs: Sequence[float], f0: float, uvw: 
         _dev(src_alpha, f64, "src_alpha"), coh_format, _dev(out, torch.complex128, "out"), precision,
         ws.data_ptr(), wsb, _stream(stream))
     _check(rc, "sagecal_predict_coherencies")
+    return out
+
+
+def predict_static_bytes() -> int:
+    """sagecal_predict_static_bytes: size of the fixed device scratch of sagecal_predict_coherencies_static."""
+    return int(load_library().sagecal_predict_static_bytes())
+
+
+def predict_coherencies_static(N: int, T: int, freqs: Sequence[float], f0: float, uvw: torch.Tensor,
+                               cluster_offset: Sequence[int], src_l: torch.Tensor, src_m: torch.Tensor,
+                               src_I: torch.Tensor, src_alpha: torch.Tensor, out: torch.Tensor,
+                               src_Q: Optional[torch.Tensor] = None, src_U: Optional[torch.Tensor] = None,
+                               src_V: Optional[torch.Tensor] = None, coh_format: int = COH_FULL, precision: int = 0,
+                               stream=None) -> torch.Tensor:
+    """sagecal_predict_coherencies_static: the prediction with its scratch in a fixed device array of the library; the
+    call allocates nothing, so `out` ([K, rows, F, 4] or [K, rows, F], complex128) is the caller's."""
+    L = load_library()
+    fr = np.ascontiguousarray(freqs, dtype=np.float64)
+    co = np.ascontiguousarray(cluster_offset, dtype=np.int32)
+    F, K, rows = int(fr.size), int(co.size) - 1, _rows(N, T)
+    shape = (K, rows, F, 4) if coh_format == COH_FULL else (K, rows, F)
+    if tuple(out.shape) != shape:
+        raise ValueError(f"out: expected shape {shape}")
+    if tuple(uvw.shape) != (rows, 3):
+        raise ValueError(f"uvw: expected shape {(rows, 3)}")
+    S = int(co[-1]) if co.size else 0
+    for name, t in (("src_l", src_l), ("src_m", src_m), ("src_I", src_I), ("src_alpha", src_alpha),
+                    ("src_Q", src_Q), ("src_U", src_U), ("src_V", src_V)):
+        if t is not None and t.numel() != S:
+            raise ValueError(f"{name}: expected {S} elements")
+    f64 = torch.float64
+    rc = L.sagecal_predict_coherencies_static(
+        N, T, F, fr.ctypes.data, float(f0), _dev(uvw, f64, "uvw"), K, co.ctypes.data,
+        _dev(src_l, f64, "src_l"), _dev(src_m, f64, "src_m"), _dev(src_I, f64, "src_I"),
+        _dev(src_Q, f64, "src_Q"), _dev(src_U, f64, "src_U"), _dev(src_V, f64, "src_V"),
+        _dev(src_alpha, f64, "src_alpha"), coh_format, _dev(out, torch.complex128, "out"), precision, _stream(stream))
+    _check(rc, "sagecal_predict_coherencies_static")
     return out
 
 

@@ -229,6 +229,7 @@ extern "C" const char* sagecal_strerror(int code) {
         case SAGECAL_EWORKSPACE: return "workspace missing, misaligned or too small";
         case SAGECAL_ECUDA: return "CUDA call failed (see sagecal_last_cuda_error)";
         case SAGECAL_EUNSUPPORTED: return "valid request not implemented by this build";
+        case SAGECAL_ESTATICLIMIT: return "request exceeds the fixed device scratch of a no-allocation entry point";
         default: return "unknown sagecal error code";
     }
 }

@@ -572,6 +572,53 @@ extern "C" int sagecal_predict_coherencies(int N, int T, int F, const double* fr
                         src_alpha, coh_format, coh, precision, workspace, workspace_bytes, stream, nullptr);
 }
 
+// ---- no-allocation entry point (README "Callers that cannot allocate") ------------------------------------------------
+// Same prediction as sagecal_predict_coherencies, with the prepared source table (nm1[S], flux[S][Fpad][NFL]: what
+// predict_prep_kernel writes and the predict kernels read) in a file-scope device array instead of a caller's
+// workspace.  Every device that loads the library holds SAGECAL_PREDICT_STATIC_BYTES of it until the process exits.
+// The name `g_predict_scratch` is only a stand-in in host code: the device address comes from cudaGetSymbolAddress, once
+// per device, with that device current.
+static __device__ __align__(256) unsigned char g_predict_scratch[SAGECAL_PREDICT_STATIC_BYTES];
+
+static int predict_static_scratch(void** out) {
+    static void* addr[64] = {};
+    static std::mutex mu;                              // two host threads may meet here on their first call
+    std::lock_guard<std::mutex> lk(mu);
+    int dev = 0;
+    SGC_CUDA(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
+    if (!addr[dev]) {
+        void* ptr = nullptr;
+        SGC_CUDA(cudaGetSymbolAddress(&ptr, g_predict_scratch));
+        if (!ptr || !aligned(ptr, 256)) return SAGECAL_EUNSUPPORTED;
+        addr[dev] = ptr;
+    }
+    *out = addr[dev];
+    return SAGECAL_OK;
+}
+
+extern "C" size_t sagecal_predict_static_bytes(void) { return (size_t)SAGECAL_PREDICT_STATIC_BYTES; }
+
+extern "C" int sagecal_predict_coherencies_static(int N, int T, int F, const double* freqs_host, double f0,
+                                                  const double* uvw, int K, const int* cluster_offset_host,
+                                                  const double* src_l, const double* src_m, const double* src_I,
+                                                  const double* src_Q, const double* src_U, const double* src_V,
+                                                  const double* src_alpha, int coh_format, sagecal_c128* coh,
+                                                  int precision, void* stream) {
+    if (F < 1 || F > PRED_MAXF || K < 0 || K > PRED_MAXK || !cluster_offset_host) return SAGECAL_EINVAL;
+    const int S = cluster_offset_host[K];
+    if (S < 0) return SAGECAL_EINVAL;
+    // the source table must fit the fixed array: nothing is allocated here, so a larger sky model is refused
+    const size_t need = sagecal_predict_workspace_bytes(F, S);
+    if (need == 0 || need > (size_t)SAGECAL_PREDICT_STATIC_BYTES) return SAGECAL_ESTATICLIMIT;
+    void* scratch = nullptr;
+    int rc;
+    if ((rc = predict_static_scratch(&scratch))) return rc;
+    // predict_prep_kernel writes every entry of the table the predict kernel reads: nothing has to start at zero
+    return predict_impl(N, T, F, freqs_host, f0, uvw, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
+                        src_alpha, coh_format, coh, precision, scratch, (size_t)SAGECAL_PREDICT_STATIC_BYTES, stream, nullptr);
+}
+
 extern "C" int sagecal_predict_residual(int N, int T, int F, const double* freqs_host, double f0,
                                         const double* uvw, int K, const int* cluster_offset_host,
                                         const double* src_l, const double* src_m, const double* src_I,
