@@ -123,6 +123,18 @@ size_t sagecal_workspace_bytes(int what, int nstations, int ntime, int nchan, in
  * Limits: F <= 512, K <= 1024 (descriptors travel as kernel parameters, so the call needs no host->device copy).
  */
 size_t sagecal_predict_workspace_bytes(int nchan, int nsrc_total);
+/* The workspace that lets unpolarised float64 predictions run in station form (below): the size above plus room for the
+ * station phasors of as many time slots as fit 2 GiB (at least one; the slots are then predicted in chunks).  With
+ * the smaller workspace the call still works and predicts per baseline. */
+size_t sagecal_predict_workspace_bytes_station(int nstations, int ntime, int nchan, int nclus, int nsrc_total);
+/* How unpolarised float64 predictions are computed (process-wide):
+ *   0 (default): in STATION form on the FP64 tensor cores whenever the uvw are differences of station coordinates
+ *      (u_pq = u_0q - u_0p to rounding, checked on the device in the same call: true for any interferometer) and the
+ *      workspace has room for one time slot's station phasors (sagecal_predict_workspace_bytes_station), else as
+ *      below;
+ *   1: always one phasor per (baseline, source).
+ * Both agree with the definition above to the parity bound.  Returns SAGECAL_EINVAL for any other value. */
+int sagecal_predict_set_form(int form);
 int sagecal_predict_coherencies(
     int nstations, int ntime, int nchan,
     const double* freqs_host, double f0,

@@ -57,6 +57,10 @@ def load_library():
     L.sagecal_predict_workspace_bytes.argtypes = [i, i]
     L.sagecal_predict_coherencies.restype = i
     L.sagecal_predict_coherencies.argtypes = [i, i, i, vp, d, vp, i, vp, vp, vp, vp, vp, vp, vp, vp, i, vp, i, vp, sz, vp]
+    L.sagecal_predict_workspace_bytes_station.restype = sz
+    L.sagecal_predict_workspace_bytes_station.argtypes = [i, i, i, i, i]
+    L.sagecal_predict_set_form.restype = i
+    L.sagecal_predict_set_form.argtypes = [i]
     L.sagecal_predict_static_bytes.restype = sz
     L.sagecal_predict_static_bytes.argtypes = []
     L.sagecal_predict_coherencies_static.restype = i
@@ -196,7 +200,8 @@ def predict_coherencies(N: int, T: int, freqs: Sequence[float], f0: float, uvw: 
                     ("src_Q", src_Q), ("src_U", src_U), ("src_V", src_V)):
         if t is not None and t.numel() != S:
             raise ValueError(f"{name}: expected {S} elements")
-    wsb = int(L.sagecal_predict_workspace_bytes(F, S))
+    wsb = int(L.sagecal_predict_workspace_bytes_station(N, T, F, K, S) if (src_Q is None and precision == 0)
+              else L.sagecal_predict_workspace_bytes(F, S))
     ws = _workspace(wsb, uvw.device)
     f64 = torch.float64
     rc = L.sagecal_predict_coherencies(
@@ -207,6 +212,11 @@ def predict_coherencies(N: int, T: int, freqs: Sequence[float], f0: float, uvw: 
         ws.data_ptr(), wsb, _stream(stream))
     _check(rc, "sagecal_predict_coherencies")
     return out
+
+
+def predict_set_form(form: int) -> None:
+    """sagecal_predict_set_form: 0 = station form when the uvw allow it (default), 1 = always per baseline."""
+    _check(load_library().sagecal_predict_set_form(int(form)), "sagecal_predict_set_form")
 
 
 def predict_static_bytes() -> int:

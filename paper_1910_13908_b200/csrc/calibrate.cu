@@ -503,7 +503,8 @@ static int host_interval(int N, int T, int F, const double* freqs_host, double f
     const int64_t B = (int64_t)N * (N - 1) / 2, rows = (int64_t)T * B, samples = rows * F;
     const size_t vis_bytes = (size_t)samples * 64;
     const size_t coh_bytes = (size_t)K * samples * (coh_format == SAGECAL_COH_SCALAR ? 16 : 64);
-    const size_t ws_pred = sagecal_predict_workspace_bytes(F, S);
+    // unpolarised sky models predict in station form: room for the station phasors of as many time slots as fit 2 GiB
+    const size_t ws_pred = pol ? sagecal_predict_workspace_bytes(F, S) : sagecal_predict_workspace_bytes_station(N, T, F, K, S);
     const size_t ws_cal = sagecal_workspace_bytes(lm_mode == SAGECAL_LM_FULLGN ? SAGECAL_WS_CALIBRATE_FULLGN : SAGECAL_WS_CALIBRATE,
                                                   N, T, F, K);
     const size_t ntrace = (size_t)n_em * K + 1;

@@ -24,6 +24,8 @@ namespace sgc {
 constexpr int PRED_THREADS = 128;
 constexpr int PRED_MAXF = 512;
 constexpr int PRED_MAXK = 1024;
+// sagecal_predict_set_form: 0 = station form when the uvw allow it (default), 1 = always one phasor per (baseline, source)
+static int g_predict_form = 0;
 constexpr int PRED_RPT = 2;           // rows per thread of the unpolarised float64 prediction (predict2_kernel)
 
 struct PredFreqs { double kf[PRED_MAXF]; };          // f_c / c0  [1/m]
@@ -335,7 +337,10 @@ __global__ void __launch_bounds__(PRED_THREADS, MINB)
 predict2_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClusters cl,
                 const double* __restrict__ uvw, const double* __restrict__ src_l,
                 const double* __restrict__ src_m, const double* __restrict__ nm1_g,
-                const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh) {
+                const double* __restrict__ flux_g, sagecal_c128* __restrict__ coh,
+                const int* __restrict__ only_if_flag) {
+    // launched behind predict_station_kernel: runs only if the uvw were found not to be station differences
+    if (only_if_flag && *only_if_flag == 0) return;
     constexpr int ST = 128;
     __shared__ double s_l[ST], s_m[ST], s_n[ST];
     __shared__ __align__(16) double s_fl[ST * FT];
@@ -428,10 +433,318 @@ predict2_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClu
     }
 }
 
+// ---- unpolarised float64 prediction in STATION form: a dense contraction on the FP64 tensor cores -------------------
+// An interferometer's uvw are differences of station coordinates: u_pq = x_q - x_p with x_s = u_0s (the rows of the
+// baselines (0, s); x_0 = 0), whichever sign convention the caller's uvw follow.  Then
+//     exp(-2 pi i kappa (x_q - x_p).s) = e_q,s conj(e_p,s),   e_p,s = exp(-2 pi i kappa x_p.s)
+//     C_pq[c] = sum_s conj(e_p,s[c]) (f_s[c] e_q,s[c])
+// i.e. per (time slot, cluster, channel) a rank-S_k Hermitian update -- 4 real FMAs per (visibility, source) instead of
+// the 8.8 FP64 instructions of a phasor per (baseline, source), and N S phasors per time slot instead of B S.  In real
+// form C = A B with A = [Re e_p | Im e_p] (stations x 2 S_k) for the real and A' = [-Im e_p | Re e_p] for the imaginary
+// part, B = [Re f e_q ; Im f e_q]: DMMA m8n8k4, one k-step = two sources.
+//
+// A CTA takes a 32 x 32 tile of station pairs (p-tile <= q-tile) of one (time slot, cluster): its 256 threads evaluate
+// the phasors of the tile's 64 stations for PG_SC sources at a time into shared memory (same phasor_f64 and channel
+// recurrence as predict_kernel), then every warp accumulates its 8 p x 16 q x FT channels (64 accumulator doubles per
+// lane) with 4 DMMAs per 4 LDS.64.  A lane ends up with all FT channels of its 2 x 2 (p, q) pairs x {Re, Im} and
+// stores the rows whole.  Warp tiles that lie entirely at or below the diagonal do no arithmetic.
+//
+// uvw_station_check_kernel decides on the device whether the caller's uvw ARE station-consistent (every row within
+// 8 eps of u_0q - u_0p, relative to the 1-norms of the three vectors: rounding, nothing a parity bound of 1e-10 sees
+// since the phase error is 2 pi kappa |d| |s| < 1e-11 rad for 20 km baselines and a 5 degree field); if
+// not, this kernel returns at once and predict2_kernel (launched after it, told to return in the other case) does the
+// work: no host synchronisation either way.
+constexpr int PG_TP = 16, PG_TQ = 32;   // CTA tile: 16 row stations x 32 column stations
+#ifndef PG_KZ_
+#define PG_KZ_ 5
+#endif
+#ifndef PG_KSS_
+#define PG_KSS_ 2
+#endif
+#ifndef PG_NSTG_
+#define PG_NSTG_ 4
+#endif
+constexpr int PG_KZ = PG_KZ_;                // the clusters are dealt to this many CTAs per (tile, time slot)
+constexpr int PG_KSS = PG_KSS_;               // k-steps (source pairs) per pipeline stage
+constexpr int PG_NSTG = PG_NSTG_;              // stages in flight
+constexpr int PG_THREADS = 256;
+struct PredPairs { int off[PRED_MAXK + 1]; };            // first source PAIR of every cluster (a cluster with an odd
+                                                         // count ends in a padding source of zero flux)
+template <int FT> constexpr size_t pg_smem_bytes() {
+    // the operand stages; the epilogue's [c][p][q] tile (padded) re-uses them
+    constexpr size_t stages = sizeof(double) * (size_t)(PG_NSTG * PG_KSS * FT * (PG_TP + PG_TQ) * 4);
+    constexpr size_t tile = sizeof(double) * 2 * (size_t)FT * (PG_TP * (PG_TQ + 1) + 1);
+    return stages > tile ? stages : tile;
+}
+// bytes of station phasors (both operands) per time slot
+static size_t pg_bytes_per_slot(int N, int npairs, int Fpad) { return (size_t)2 * npairs * Fpad * N * 4 * sizeof(double); }
+// tiles of one time slot: p-tile pi meets the q-tiles from the one that holds its first station on
+static int64_t pg_tiles(int N) {
+    const int ntp = (N + PG_TP - 1) / PG_TP, ntq = (N + PG_TQ - 1) / PG_TQ;
+    int64_t n = 0;
+    for (int pi = 0; pi < ntp; pi++) n += ntq - (pi * PG_TP) / PG_TQ;
+    return n;
+}
+__device__ __forceinline__ void pg_cp_async16(void* smem, const void* gmem) {
+    const unsigned s = (unsigned)__cvta_generic_to_shared(smem);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem) : "memory");
+}
+__device__ __forceinline__ void pg_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N_> __device__ __forceinline__ void pg_cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N_) : "memory"); }
+
+// Station phasors of nt time slots from t0: E[t][pair][c][station][2 sources x (re, im)] = e_p,s[c] and FE = f_s[c] e.
+// One thread per (t, pair, station, source of the pair), all FT-channel tiles; adjacent lanes write adjacent 16 bytes.
+template <int FT, bool UNIFORM>
+__global__ void __launch_bounds__(128)
+station_phasor_kernel(int N, int64_t B, int F, int Fpad, int K, int npairs, int t0, PredFreqs fr, double dkf, PredClusters cl,
+                      PredPairs pp, const double* __restrict__ uvw, const double* __restrict__ src_l,
+                      const double* __restrict__ src_m, const double* __restrict__ nm1_g,
+                      const double* __restrict__ flux_g, double* __restrict__ E, double* __restrict__ FE,
+                      const int* __restrict__ flag) {
+    if (*flag) return;
+    __shared__ double2 s_tab_all[64 * 8];
+    if (threadIdx.x < 64) {
+        double sn, cs;
+        sincospi((double)threadIdx.x * 0.03125, &sn, &cs);
+#pragma unroll
+        for (int c = 0; c < 8; c++) s_tab_all[8 * threadIdx.x + c] = make_double2(cs, sn);
+    }
+    __syncthreads();
+    const unsigned s_tab = (unsigned)__cvta_generic_to_shared(s_tab_all + (threadIdx.x & 7));
+    const int e = blockIdx.x * 128 + threadIdx.x;        // (station, h) within the pair
+    const int pair = blockIdx.y, tl = blockIdx.z;
+    if (e >= 2 * N) return;
+    const int st = e >> 1, h = e & 1;
+    // the pair's cluster: the last k with pp.off[k] <= pair
+    int lo = 0, hi = K;
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (pp.off[mid] <= pair) lo = mid; else hi = mid; }
+    const int s = cl.off[lo] + 2 * (pair - pp.off[lo]) + h;
+    const bool live = s < cl.off[lo + 1];                // else the padding source of an odd cluster
+    double u = 0.0, v = 0.0, w = 0.0;
+    if (st >= 1) {
+        const double* x = uvw + 3 * ((int64_t)(t0 + tl) * B + (st - 1));      // x_s = u_0s, x_0 = 0
+        u = x[0]; v = x[1]; w = x[2];
+    }
+    const double ph = live ? fma(w, nm1_g[s], fma(v, src_m[s], u * src_l[s])) : 0.0;   // metres
+    for (int c0 = 0; c0 < Fpad; c0 += FT) {
+        double er, ei, dr = 1.0, di = 0.0;
+        double pr = 0.0, pi_ = 0.0, twodr = 2.0;
+        if (UNIFORM) {
+            phasor_f64(ph * fr.kf[c0], s_tab, er, ei);
+            if (FT > 1) { phasor_f64(ph * dkf, s_tab, dr, di); twodr = dr + dr; }
+        }
+#pragma unroll
+        for (int c = 0; c < FT; c++) {
+            if (!UNIFORM) phasor_f64(ph * fr.kf[min(c0 + c, PRED_MAXF - 1)], s_tab, er, ei);
+            const double f = live ? flux_g[(size_t)s * Fpad + c0 + c] : 0.0;
+            const size_t o = ((((size_t)tl * npairs + pair) * Fpad + c0 + c) * N + st) * 4 + 2 * h;
+            *reinterpret_cast<double2*>(E + o) = make_double2(er, ei);
+            *reinterpret_cast<double2*>(FE + o) = make_double2(f * er, f * ei);
+            if (UNIFORM && c + 1 < FT) {
+                double nr, ni;
+                if (c == 0) { nr = fma(-ei, di, er * dr); ni = fma(ei, dr, er * di); }
+                else { nr = fma(twodr, er, -pr); ni = fma(twodr, ei, -pi_); }
+                pr = er; pi_ = ei;
+                er = nr; ei = ni;
+            }
+        }
+    }
+}
+
+__global__ void uvw_station_check_kernel(int N, int64_t B, int64_t rows, const double* __restrict__ uvw, int* flag) {
+    const int64_t r = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (r >= rows) return;
+    const int64_t t = r / B;
+    int p, q;
+    bl_stations(N, r - t * B, p, q);
+    if (p == 0) return;                                  // these rows DEFINE the station coordinates
+    const double* x = uvw + 3 * r;
+    const double* a = uvw + 3 * (t * B + (p - 1));       // bl_index(N, 0, s) = s - 1
+    const double* c = uvw + 3 * (t * B + (q - 1));
+    // uvw components are sums of products of coordinates that may cancel: the rounding of a component scales with the
+    // vectors' size, not with its own (measured on the generator's tracks: up to 1.25 eps of the 1-norms below)
+    double scale = 0.0;
+#pragma unroll
+    for (int d = 0; d < 3; d++) scale += fabs(x[d]) + fabs(c[d]) + fabs(a[d]);
+    const double tol = 8.0 * 2.220446049250313e-16 * scale;
+    bool bad = false;
+#pragma unroll
+    for (int d = 0; d < 3; d++)
+        if (!(fabs(x[d] - (c[d] - a[d])) <= tol)) bad = true;     // NaN is inconsistent
+    if (bad) *flag = 1;                                  // every writer stores the same value
+}
+
+__device__ __forceinline__ void dmma884(double& d0, double& d1, double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(d0), "+d"(d1) : "d"(a), "d"(b));
+}
+
+template <int FT, bool SCALAR>
+__global__ void __launch_bounds__(PG_THREADS, 2)
+predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, int npairs, int t0, PredPairs pp,
+                       const double* __restrict__ E, const double* __restrict__ FE, sagecal_c128* __restrict__ coh,
+                       const int* __restrict__ flag) {
+    if (*flag) return;                                   // uvw are not station differences: predict2_kernel's job
+    extern __shared__ __align__(16) unsigned char pg_smem[];
+    constexpr int SZA = PG_KSS * FT * PG_TP * 4;         // doubles per stage: [ks][c][station][2 sources x (re, im)]
+    constexpr int SZB = PG_KSS * FT * PG_TQ * 4;
+    constexpr int SZS = SZA + SZB;
+    // a warp takes ONE channel, all 16 p and NT n-tiles of 8 q (8 fragment loads per 16 DMMAs at FT = 8, 32
+    // accumulator doubles per lane: 16 warps per SM)
+    constexpr int NQW = 8 / FT < 4 ? 8 / FT : 4, NT = 4 / NQW;
+    double* smem = reinterpret_cast<double*>(pg_smem);
+    double2* s_stage = reinterpret_cast<double2*>(pg_smem);              // epilogue: [c][p][q] of the tile, padded
+    // tile (pi, qi) of this CTA: p-tiles of PG_TP stations, q-tiles of PG_TQ; only tiles with some q > p
+    const int ntq = (N + PG_TQ - 1) / PG_TQ;
+    int pi = 0, rem = (int)blockIdx.x;
+    while (rem >= ntq - (pi * PG_TP) / PG_TQ) { rem -= ntq - (pi * PG_TP) / PG_TQ; pi++; }
+    const int qi = (pi * PG_TP) / PG_TQ + rem;
+    const int p0 = PG_TP * pi, q0 = PG_TQ * qi;
+    const int tl = blockIdx.y, t = t0 + tl;
+
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int g = lane >> 2, j = lane & 3;
+    const int cw = warp % FT, qw = warp / FT;            // channel, q group of this warp
+    const bool w_work = qw < NQW;                        // FT = 1: four of the eight warps contract
+    const int qb = qw * (NT * 8);                        // first q of the warp within the tile
+    unsigned act = 0;                                    // (m-tile, n-tile) blocks with some q > p (bit mt * NT + nt)
+    if (w_work) {
+#pragma unroll
+        for (int mt = 0; mt < 2; mt++)
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++)
+                if (q0 + qb + nt * 8 + 7 > p0 + mt * 8 && p0 + mt * 8 < N && q0 + qb + nt * 8 < N) act |= 1u << (mt * NT + nt);
+    }
+    const int a_off = (cw * PG_TP + g) * 4 + j;
+    const int b_off = SZA + (cw * PG_TQ + qb + g) * 4 + j;
+    const int jx = (j ^ 1) - j;                          // the partner entry (s, 1 - ri) of this lane's (s, ri)
+    const int sgn = (j & 1) ? 0 : (int)0x80000000;       // Im part: A'[(s, 0)] = -Im e, A'[(s, 1)] = +Re e
+
+    // operand copies: threads 0..191 copy two (pair, channel) rows per pass, 96 16-byte pieces each (32 of the p
+    // stations from E, 64 of the q stations from FE); everything that does not depend on the stage is fixed here
+    const bool cp_thread = threadIdx.x < 192;
+    const int cp_rp = threadIdx.x >= 96 ? 1 : 0, cp_u = threadIdx.x - 96 * cp_rp;
+    const bool cp_p = cp_u < 2 * PG_TP;
+    const int cp_st = cp_p ? cp_u >> 1 : (cp_u - 2 * PG_TP) >> 1;
+    const double* cp_src = (cp_p ? E + (size_t)min(p0 + cp_st, N - 1) * 4 : FE + (size_t)min(q0 + cp_st, N - 1) * 4) + 2 * (cp_u & 1);
+    const int cp_dst = (cp_p ? 0 : SZA) + cp_st * 4 + 2 * (cp_u & 1);
+    const int cp_rstride = (cp_p ? PG_TP : PG_TQ) * 4;
+    const size_t rowlen = (size_t)N * 4;                 // doubles per (pair, channel) row
+
+    for (int k = blockIdx.z; k < K; k += gridDim.z) {
+      const int pb = pp.off[k], np = pp.off[k + 1] - pb;
+      const int nstage = (np + PG_KSS - 1) / PG_KSS;
+      for (int c0 = 0; c0 < Fpad; c0 += FT) {
+        double acc[2][NT][4];                            // [m-tile][n-tile][Re q, Re q+1, Im q, Im q+1]
+#pragma unroll
+        for (int mt = 0; mt < 2; mt++)
+#pragma unroll
+            for (int nt = 0; nt < NT; nt++)
+#pragma unroll
+                for (int x = 0; x < 4; x++) acc[mt][nt][x] = 0.0;
+
+        // stage sg of this (cluster, channel tile): pairs pb + sg KSS ..; 16-byte pieces, 96 per (pair, channel)
+        auto issue = [&](int sg) {
+            if (sg < nstage && cp_thread) {
+                double* dstg = smem + (sg % PG_NSTG) * SZS + cp_dst;
+                const int nrow = min(PG_KSS, np - sg * PG_KSS) * FT;
+                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * PG_KSS) * Fpad + c0) * rowlen;
+#pragma unroll
+                for (int r0 = 0; r0 < PG_KSS * FT; r0 += 2) {
+                    const int r = r0 + cp_rp;            // row (ks, c) = (r / FT, r % FT) of the stage
+                    if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + ((size_t)(r / FT) * Fpad + (r % FT)) * rowlen);
+                }
+            }
+            pg_cp_async_commit();                        // always: the group count per stage stays uniform
+        };
+        __syncthreads();                                 // every warp is done with the shared memory of the previous tile
+#pragma unroll
+        for (int sg = 0; sg < PG_NSTG - 1; sg++) issue(sg);
+        for (int sg = 0; sg < nstage; sg++) {
+            pg_cp_async_wait<PG_NSTG - 2>();             // stage sg has landed (this thread's part)
+            __syncthreads();                             // ... everyone's; and stage sg - 1 has been consumed
+            issue(sg + PG_NSTG - 1);
+            if (act) {
+                const double* sb_ = smem + (sg % PG_NSTG) * SZS;
+                const int nk = min(PG_KSS, np - sg * PG_KSS);
+#pragma unroll
+                for (int ks = 0; ks < PG_KSS; ks++) {
+                    if (ks > 0 && ks >= nk) break;       // only a cluster's last stage can be short
+                    const double* ak = sb_ + a_off + ks * FT * PG_TP * 4;
+                    const double* bk = sb_ + b_off + ks * FT * PG_TQ * 4;
+                    double a[2], a2[2], b[NT];
+#pragma unroll
+                    for (int mt = 0; mt < 2; mt++) {
+                        a[mt] = ak[mt * 32];
+                        const double x = ak[mt * 32 + jx];
+                        a2[mt] = __hiloint2double(__double2hiint(x) ^ sgn, __double2loint(x));
+                    }
+#pragma unroll
+                    for (int nt = 0; nt < NT; nt++) b[nt] = bk[nt * 32];
+#pragma unroll
+                    for (int mt = 0; mt < 2; mt++)
+#pragma unroll
+                        for (int nt = 0; nt < NT; nt++)
+                            if (act & (1u << (mt * NT + nt))) {
+                                dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                                dmma884(acc[mt][nt][2], acc[mt][nt][3], a2[mt], b[nt]);
+                            }
+                }
+            }
+        }
+        // epilogue: the tile goes through shared memory (the operand buffers, free now) as [c][p][q] complex, padded so
+        // that neither side has bank conflicts, and leaves in the order of global memory: consecutive threads store
+        // consecutive 32-byte pieces (2x2 format: (v, 0) and (0, v) of a (row, channel)) -- whole lines, 8 wavefronts
+        // per store instruction where a lane-owns-its-rows store needs 32
+        constexpr int PSTR = PG_TQ + 1, CSTR = PG_TP * PSTR + 1;         // strides in complex numbers
+        __syncthreads();                                 // every warp has finished the last stage
+        if (w_work) {
+#pragma unroll
+            for (int mt = 0; mt < 2; mt++)
+#pragma unroll
+                for (int nt = 0; nt < NT; nt++)
+#pragma unroll
+                    for (int b = 0; b < 2; b++)
+                        s_stage[cw * CSTR + (mt * 8 + g) * PSTR + qb + nt * 8 + 2 * j + b] = make_double2(acc[mt][nt][b], acc[mt][nt][2 + b]);
+        }
+        __syncthreads();
+        // pieces per (p, q): 16 bytes per channel (scalar) / 32 bytes per half of a channel; a thread keeps its piece
+        // index and walks the tile's (p, q)
+        constexpr int PCS = SCALAR ? FT : 2 * FT;
+        constexpr int QPT = PG_THREADS / PCS;            // q's covered by the CTA per trip
+        {
+            const int pc = threadIdx.x % PCS, qoff = threadIdx.x / PCS;
+            const int c = SCALAR ? pc : pc >> 1;
+            const bool c_ok = c0 + c < F;
+            const double2* sc = s_stage + c * CSTR;
+            sagecal_c128* ok = coh + ((size_t)k * rows + (size_t)t * B) * F * (SCALAR ? 1 : 4);
+            const int inner = SCALAR ? (c0 + c) : (c0 + c) * 4 + 2 * (pc & 1);     // complex numbers into a row
+#pragma unroll 2
+            for (int pl = 0; pl < PG_TP; pl++) {
+                const int p = p0 + pl;
+                if (p >= N - 1) break;
+                const int64_t rs = row_start(N, p) - p - 1;          // bl_index(N, p, q) = rs + q
+#pragma unroll
+                for (int ql = qoff; ql < PG_TQ; ql += QPT) {
+                    const int q = q0 + ql;
+                    if (!(p < q && q < N && c_ok)) continue;
+                    const double2 v = sc[pl * PSTR + ql];
+                    sagecal_c128* o = ok + (size_t)(rs + q) * F * (SCALAR ? 1 : 4) + inner;
+                    if (SCALAR) *reinterpret_cast<double2*>(o) = v;
+                    else if (pc & 1) stg256(o, 0.0, 0.0, v.x, v.y);
+                    else stg256(o, v.x, v.y, 0.0, 0.0);
+                }
+            }
+        }
+      }
+    }
+}
+
 template <int FT, bool POL, bool UNIFORM, bool SCALAR, bool MIXED>
 static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int Fpad, const PredFreqs& fr, double dkf,
                           const PredClusters& cl, const double* uvw, const double* l, const double* m,
-                          const double* nm1, const double* flux, sagecal_c128* coh, const PredResid* rs) {
+                          const double* nm1, const double* flux, sagecal_c128* coh, const PredResid* rs, int N, int T,
+                          int* flag, void* extra, size_t extra_bytes) {
     LaunchScope ls(KK_PREDICT, st);
     if (rs) {
         if (MIXED) return SAGECAL_EUNSUPPORTED;
@@ -453,8 +766,54 @@ static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int F
         // two rows per thread at four CTAs per SM (127 registers, no spills): 28.8 ms at configs[4] against 31.4 for
         // one row per thread, 29.1 at three CTAs per SM, 30.2 with three rows per thread
         const dim3 g2((unsigned)((rows + PRED_RPT * PRED_THREADS - 1) / (PRED_RPT * PRED_THREADS)), grid.y);
+        const int64_t B = (int64_t)N * (N - 1) / 2;
+        const int64_t ntile = pg_tiles(N);
+        const int K = (int)grid.y;
+        // source pairs: a k-step of the contraction is two sources; a cluster with an odd count is padded
+        PredPairs pp;
+        int npairs = 0;
+        for (int k = 0; k <= PRED_MAXK; k++) {
+            pp.off[k] = npairs;
+            if (k < K) npairs += (cl.off[k + 1] - cl.off[k] + 1) / 2;
+        }
+        const size_t per_slot = pg_bytes_per_slot(N, npairs, Fpad);
+        const int64_t tchunk = per_slot ? (int64_t)(extra_bytes / per_slot) : 0;
+        const bool station_form = g_predict_form == 0 && extra && tchunk >= 1 && npairs >= 1 && npairs <= 65535 &&
+                                  ntile <= 0x7fffffff && 2 * (int64_t)N <= 0x7fffffff;
+        if (station_form) {
+            // station form first (returns at once if the uvw are not station differences), the per-baseline form behind
+            // it (returns at once if they are): the choice is made on the device, nothing waits for the host
+            constexpr int smem = (int)pg_smem_bytes<FT>();
+            auto kern = predict_station_kernel<FT, SCALAR>;
+            {
+                static bool ready[64] = {};
+                static std::mutex mu;                  // two host threads may meet here on their first call
+                std::lock_guard<std::mutex> lk(mu);
+                int dev = 0;
+                SGC_CUDA(cudaGetDevice(&dev));
+                if (dev < 0 || dev >= 64) return SAGECAL_EUNSUPPORTED;
+                if (!ready[dev]) {
+                    SGC_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+                    SGC_CUDA(cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, 100));
+                    ready[dev] = true;
+                }
+            }
+            SGC_CUDA(cudaMemsetAsync(flag, 0, sizeof(int), st));
+            uvw_station_check_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(N, B, rows, uvw, flag);
+            const int kz = K < PG_KZ ? K : PG_KZ;      // a CTA keeps its tile for several clusters
+            const int tstep = (int)(tchunk < 32768 ? tchunk : 32768);
+            for (int t0 = 0; t0 < T; t0 += tstep) {
+                const int nt = T - t0 < tstep ? T - t0 : tstep;
+                double* E = (double*)extra;
+                double* FE = E + (size_t)nt * npairs * Fpad * N * 4;
+                station_phasor_kernel<FT, UNIFORM><<<dim3((unsigned)((2 * N + 127) / 128), (unsigned)npairs, (unsigned)nt), 128, 0, st>>>(
+                    N, B, F, Fpad, K, npairs, t0, fr, dkf, cl, pp, uvw, l, m, nm1, flux, E, FE, flag);
+                kern<<<dim3((unsigned)ntile, (unsigned)nt, (unsigned)kz), PG_THREADS, smem, st>>>(
+                    N, B, rows, F, Fpad, K, npairs, t0, pp, E, FE, coh, flag);
+            }
+        }
         predict2_kernel<FT, UNIFORM, SCALAR, PRED_RPT, 4><<<g2, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw, l, m, nm1,
-                                                                                  flux, coh);
+                                                                                  flux, coh, station_form ? flag : nullptr);
     } else {
         predict_kernel<FT, POL, UNIFORM, SCALAR, MIXED, false><<<grid, PRED_THREADS, 0, st>>>(rows, F, Fpad, fr, dkf, cl, uvw,
                                                                                      l, m, nm1, flux, coh, PredResid{});
@@ -468,6 +827,25 @@ static int pick_ft(int F) { return F >= 8 ? 8 : F >= 4 ? 4 : F >= 2 ? 2 : 1; }
 }  // namespace sgc
 
 using namespace sgc;
+
+extern "C" int sagecal_predict_set_form(int form) {
+    if (form != 0 && form != 1) return SAGECAL_EINVAL;
+    g_predict_form = form;
+    return SAGECAL_OK;
+}
+
+extern "C" size_t sagecal_predict_workspace_bytes_station(int nstations, int ntime, int nchan, int nclus, int nsrc_total) {
+    const size_t base = sagecal_predict_workspace_bytes(nchan, nsrc_total);
+    if (base == 0 || nstations < 2 || ntime < 1 || nclus < 0) return base;
+    const int ft = pick_ft(nchan);
+    const int Fpad = (int)round_up((size_t)nchan, ft);
+    const int npairs = nsrc_total / 2 + nclus;         // an upper bound: every cluster may end in a padding source
+    const size_t per_slot = pg_bytes_per_slot(nstations, npairs, Fpad);
+    const size_t cap = (size_t)2 << 30;                // the time slots are predicted in chunks of what fits 2 GiB
+    size_t extra = per_slot * (size_t)ntime;
+    if (extra > cap) extra = per_slot * (cap / per_slot > 0 ? cap / per_slot : 1);
+    return base + round_up(extra, 256);
+}
 
 extern "C" size_t sagecal_predict_workspace_bytes(int nchan, int nsrc_total) {
     if (nchan < 1 || nchan > PRED_MAXF || nsrc_total < 0) return 0;
@@ -524,6 +902,12 @@ static int predict_impl(int N, int T, int F, const double* freqs_host, double f0
 
     double* nm1 = (double*)workspace;
     double* flux = (double*)((char*)workspace + round_up(sizeof(double) * (size_t)S, 256));
+    // the last 256 bytes of the workspace: the device-side flag "uvw are not station differences"
+    int* flag = (int*)((char*)flux + round_up(sizeof(double) * (size_t)S * Fpad * 4, 256));
+    // whatever the caller gave beyond sagecal_predict_workspace_bytes(): room for the station phasors (station form)
+    const size_t base_bytes = sagecal_predict_workspace_bytes(F, S);
+    void* extra = workspace_bytes > base_bytes ? (void*)((char*)workspace + base_bytes) : nullptr;
+    const size_t extra_bytes = extra ? workspace_bytes - base_bytes : 0;
     if (S > 0) {
         const int n = S * Fpad, tb = 256;
         LaunchScope ls(KK_PREP, st);
@@ -541,9 +925,9 @@ static int predict_impl(int N, int T, int F, const double* freqs_host, double f0
 #define SGC_PRED(FT_, POL_, UNI_, SC_)                                                                                  \
     do {                                                                                                               \
         if (mixed) return launch_predict<FT_, POL_, UNI_, SC_, true>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l,  \
-                                                                    src_m, nm1, flux, coh, rs);                        \
+                                                                    src_m, nm1, flux, coh, rs, N, T, flag, extra, extra_bytes); \
         return launch_predict<FT_, POL_, UNI_, SC_, false>(grid, st, rows, F, Fpad, fr, dkf, cl, uvw, src_l, src_m,    \
-                                                          nm1, flux, coh, rs);                                         \
+                                                          nm1, flux, coh, rs, N, T, flag, extra, extra_bytes);        \
     } while (0)
 #define SGC_PRED_FT(FT_)                                            \
     do {                                                            \
@@ -616,7 +1000,7 @@ extern "C" int sagecal_predict_coherencies_static(int N, int T, int F, const dou
     if ((rc = predict_static_scratch(&scratch))) return rc;
     // predict_prep_kernel writes every entry of the table the predict kernel reads: nothing has to start at zero
     return predict_impl(N, T, F, freqs_host, f0, uvw, K, cluster_offset_host, src_l, src_m, src_I, src_Q, src_U, src_V,
-                        src_alpha, coh_format, coh, precision, scratch, (size_t)SAGECAL_PREDICT_STATIC_BYTES, stream, nullptr);
+                        src_alpha, coh_format, coh, precision, scratch, need, stream, nullptr);   // `need`: no room for station phasors -> per baseline
 }
 
 extern "C" int sagecal_predict_residual(int N, int T, int F, const double* freqs_host, double f0,

@@ -14,6 +14,16 @@ def host(t):
     return t.detach().cpu().numpy()
 
 
+class per_baseline_form:
+    """with per_baseline_form(): predictions use one phasor per (baseline, source) -- the arithmetic the fused RESID arm
+    shares bit for bit -- instead of the station form (sagecal_predict_set_form)."""
+    def __enter__(self):
+        sg.predict_set_form(1)
+
+    def __exit__(self, *exc):
+        sg.predict_set_form(0)
+
+
 def gpu_predict(prob, coh_format=sg.COH_FULL, precision=0, freqs=None):
     src = {k: dev(getattr(prob, k)) for k in ("src_l", "src_m", "src_I", "src_alpha", "src_Q", "src_U", "src_V")}
     return sg.predict_coherencies(prob.N, prob.T, prob.freqs if freqs is None else freqs, prob.f0, dev(prob.uvw),

@@ -163,7 +163,7 @@ def test_predict_residual_matches_oracle(cuda_device, cfg, fmt_name):
     """coh = the oracle's prediction and residual = V - sum_k J_k C_k J_k^H by the oracle's corrupt/subtract (1e-10), with
     Jones that are not the identity; the coherencies are bit-identical to sagecal_predict_coherencies'."""
     import paper_1910_13908_b200 as sg
-    from tests.gpu_util import gpu_predict, host
+    from tests.gpu_util import gpu_predict, host, per_baseline_form
     p = make_config(cfg)
     fmt = sg.COH_FULL if fmt_name == "full" else sg.COH_SCALAR
     coh_ref = oracle.predict(p)
@@ -171,7 +171,10 @@ def test_predict_residual_matches_oracle(cuda_device, cfg, fmt_name):
     J = p.jones_true * (1.0 + 0.05j) + 0.02
     want = oracle.corrupt_subtract(p.N, p.T, p.F, coh_ref, J, V, sign=-1.0)
     coh, res = _fused(sg, p, fmt, J, V)
-    assert np.array_equal(host(coh), host(gpu_predict(p, fmt)))
+    with per_baseline_form():                                 # the fused arm predicts per baseline
+        assert np.array_equal(host(coh), host(gpu_predict(p, fmt)))
+    _check(host(coh).reshape(coh_ref[..., 0].shape if fmt == sg.COH_SCALAR else coh_ref.shape),
+           coh_ref[..., 0] if fmt == sg.COH_SCALAR else coh_ref)
     _check(host(res), want)
 
 
@@ -201,10 +204,11 @@ def test_calibrate_from_fused_residual_is_the_same_run(cuda_device, fmt_name):
     the unfused route: costs, trace, Jones and residual agree to rounding of the initial residual (1e-11)."""
     import torch
     import paper_1910_13908_b200 as sg
-    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host
+    from tests.gpu_util import dev, gpu_predict, gpu_simulate, host, per_baseline_form
     p = make_config(2)
     fmt = sg.COH_FULL if fmt_name == "full" else sg.COH_SCALAR
-    coh_d = gpu_predict(p, fmt)
+    with per_baseline_form():                                 # the same coherencies, bit for bit, on both routes
+        coh_d = gpu_predict(p, fmt)
     vis = gpu_simulate(p, coh_d, fmt)
     a = sg.sage_calibrate(p.N, p.T, p.F, vis, coh_d, dev(p.jones_init()), p.n_em, p.n_lm, p.tau, coh_format=fmt)
     coh2, res = _fused(sg, p, fmt, p.jones_init(), host(vis))
@@ -212,3 +216,80 @@ def test_calibrate_from_fused_residual_is_the_same_run(cuda_device, fmt_name):
     torch.cuda.synchronize()
     for key in ("cost_per_cluster", "cost_trace", "jones", "residual"):
         assert rel_l2(host(b[key]), host(a[key])) < 1e-11, key
+
+
+# ---- station form (DMMA contraction of station phasors) and its fall-backs ------------------------------------------
+@pytest.mark.parametrize("shape", [(2, 1, 1, 1, 1), (3, 2, 3, 2, 5), (17, 2, 8, 3, 7), (33, 3, 5, 2, 9), (50, 2, 9, 4, 6),
+                                   (70, 1, 13, 2, 11)])
+@pytest.mark.parametrize("fmt_name", ["full", "scalar"])
+def test_predict_station_form_ragged_shapes(cuda_device, shape, fmt_name):
+    """Station counts off the 16 x 32 tile, channel counts off the register tile (and several channel tiles), odd source
+    counts (a padding source per cluster), an empty cluster: both forms against the oracle, and against each other."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host, per_baseline_form
+    N, T, F, K, S = shape
+    p = make_problem(N, T, F, K, S, seed=500 + N, layout="disc:20000", field_deg=5.0, patch_deg=0.7)
+    if K >= 3:
+        off = p.cluster_offset.copy()
+        off[2] = off[1]                                       # cluster 1 is empty
+        p.cluster_offset = off
+    fmt = sg.COH_FULL if fmt_name == "full" else sg.COH_SCALAR
+    want = oracle.predict(p)
+    if fmt == sg.COH_SCALAR:
+        want = want[..., 0]
+    got = host(gpu_predict(p, fmt)).reshape(want.shape)
+    with per_baseline_form():
+        got_b = host(gpu_predict(p, fmt)).reshape(want.shape)
+    _check(got, want)
+    _check(got_b, want)
+    assert not np.array_equal(got, got_b) or N <= 2           # two different computations (the station form DID run)
+    if K >= 3:
+        assert np.all(got[1] == 0)
+
+
+def test_predict_falls_back_when_uvw_are_not_station_differences(cuda_device):
+    """One baseline's uvw moved by a metre: the rows are no longer differences of station coordinates, the device-side
+    check sends the call to the per-baseline form, and the answer is the definition's (the station form would be off by
+    a whole phase turn on that row)."""
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import gpu_predict, host, per_baseline_form
+    p = make_problem(20, 2, 8, 3, 9, seed=611, layout="disc:20000", field_deg=5.0, patch_deg=0.7)
+    uvw = p.uvw.copy()
+    uvw[p.B + 57] += np.array([1.0, -2.0, 0.5])               # (t = 1, baseline 57), not a (0, q) row
+    p.uvw = uvw
+    want = oracle.predict(p)
+    got = host(gpu_predict(p, sg.COH_FULL))
+    _check(got, want)
+    with per_baseline_form():
+        assert np.array_equal(got, host(gpu_predict(p, sg.COH_FULL)))      # it WAS the per-baseline form
+    # NaN anywhere in the uvw: inconsistent, never the station form
+    uvw[3, 1] = np.nan
+    p.uvw = uvw
+    got = host(gpu_predict(p, sg.COH_FULL))
+    with per_baseline_form():
+        assert np.array_equal(got, host(gpu_predict(p, sg.COH_FULL)), equal_nan=True)
+
+
+def test_predict_with_the_small_workspace_predicts_per_baseline(cuda_device):
+    """sagecal_predict_workspace_bytes() (no room for station phasors) still works: per-baseline form, same bits."""
+    import torch
+    import paper_1910_13908_b200 as sg
+    from tests.gpu_util import dev, gpu_predict, host, per_baseline_form
+    p = make_config(1)
+    L = sg.load_library()
+    S = int(p.cluster_offset[-1])
+    wsb = int(L.sagecal_predict_workspace_bytes(p.F, S))
+    assert int(L.sagecal_predict_workspace_bytes_station(p.N, p.T, p.F, p.K, S)) > wsb
+    ws = torch.empty(wsb, dtype=torch.uint8, device=cuda_device)
+    out = torch.empty((p.K, p.rows, p.F, 4), dtype=torch.complex128, device=cuda_device)
+    fr = np.ascontiguousarray(p.freqs, dtype=np.float64)
+    co = np.ascontiguousarray(p.cluster_offset, dtype=np.int32)
+    d = {k: dev(getattr(p, k)) for k in ("uvw", "src_l", "src_m", "src_I", "src_alpha")}
+    rc = L.sagecal_predict_coherencies(p.N, p.T, p.F, fr.ctypes.data, float(p.f0), d["uvw"].data_ptr(), p.K, co.ctypes.data,
+                                       d["src_l"].data_ptr(), d["src_m"].data_ptr(), d["src_I"].data_ptr(), None, None,
+                                       None, d["src_alpha"].data_ptr(), sg.COH_FULL, out.data_ptr(), 0, ws.data_ptr(), wsb,
+                                       torch.cuda.current_stream().cuda_stream)
+    assert rc == 0
+    with per_baseline_form():
+        assert np.array_equal(host(out), host(gpu_predict(p, sg.COH_FULL)))
+    _check(host(gpu_predict(p, sg.COH_FULL)), oracle.predict(p))

@@ -37,7 +37,7 @@ def _static(sg, p, d, fmt, out):
 def test_static_scratch_predict_matches_the_workspace_path_on_calls_in_a_row(cuda_device):
     import torch
     import paper_1910_13908_b200 as sg
-    from tests.gpu_util import gpu_predict, host
+    from tests.gpu_util import gpu_predict, host, per_baseline_form
 
     # three different sky models one after the other through the ONE shared array: a large unpolarised table, then a
     # smaller polarised one with non-uniform channels (the first call's entries are still behind it), then scalar output
@@ -46,7 +46,8 @@ def test_static_scratch_predict_matches_the_workspace_path_on_calls_in_a_row(cud
                      freqs=np.array([120e6, 131e6, 150e6, 151e6, 178e6]))
     c = make_config(2, K=5)
     cases = [(a, sg.COH_FULL), (b, sg.COH_FULL), (c, sg.COH_SCALAR), (a, sg.COH_FULL)]
-    want = [host(gpu_predict(p, fmt)) for p, fmt in cases]                  # the existing path, its own workspace
+    with per_baseline_form():                                               # the static entry predicts per baseline
+        want = [host(gpu_predict(p, fmt)) for p, fmt in cases]              # the existing path, its own workspace
     outs = [torch.full(w.shape, float("nan"), dtype=torch.complex128, device=cuda_device) for w in want]
     ins = [_inputs(p) for p, _ in cases]
     torch.cuda.synchronize()
