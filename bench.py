@@ -187,7 +187,8 @@ def stream_bytes_per_interval(samples: int, K: int, n_em: int, coh: str, lm: str
 def interval_floor(samples: int, vis_src: int, K: int, n_em: int, coh: str, hbm_gbs: float, dfma_per_s: float,
                    predict_inst_per_vis_src: float, lm: str = "compressed", n_lm: int = 10, fused: bool = False) -> dict:
     """Roofline floor of one interval: the streaming kernels' algorithmic bytes at the measured copy rate plus the
-    prediction's FP64 instructions at the measured DFMA rate -- or, if larger, the bytes the prediction itself moves
+    prediction's arithmetic (station form: 4 FMAs per visibility x source at the measured DMMA rate; fused route: its
+    FP64 instructions at the measured DFMA rate) -- or, if larger, the bytes the prediction itself moves
     (K coherencies written; fused route: V read and R written as well) -- the M-step and the small kernels count as
     overhead."""
     b = stream_bytes_per_interval(samples, K, n_em, coh, lm, n_lm, fused)
@@ -501,6 +502,7 @@ def run_ours(args):
     # ALU-bound kernels: FP64 thread-instructions (ncu count per unit of work, profiles/kernel_counts.csv) per second
     # of CUDA-event time inside the timed region, against the DFMA-chain peak measured NOW on this device.
     dfma = sg.profile_dfma_peak()
+    dmma = sg.profile_dmma_peak()
     sms = torch.cuda.get_device_properties(dev).multi_processor_count
     dfma_nominal = sms * 64 * (clk.get("sm_max_mhz") or 1965.0) * 1e6
     fused = args.fused
@@ -524,12 +526,33 @@ def run_ours(args):
                 "launches_timed": n, "avg_launch_ms": ms, "sm_mhz_under_load": clk.get("sm_mhz"),
                 "share_of_step": prof[kind]["ms"] / max(args.steps, 1) / ms_per_step}
 
-    e = alu_entry("predict_kernel", "predict", p.vis_src, "visibility x source")
-    if e:
-        if fused:
+    if fused:
+        e = alu_entry("predict_kernel", "predict", p.vis_src, "visibility x source")
+        if e:
             e["note"] = ("RESID arm (sagecal_predict_residual): predicts all K clusters of its rows and leaves the initial "
                          "residual R = V - sum_k J_k C_k J_k^H, so no corrupt_kernel launch is in the step")
-        rooflines.append(e)
+            rooflines.append(e)
+    elif prof["predict"]["timed"]:
+        # station form: a rank-S_k Hermitian update per (time slot, cluster, channel) on the FP64 tensor
+        # cores: 4 real FMAs per visibility x source (one complex multiply-add), against the DMMA-chain peak measured
+        # NOW on this device; the call also writes the K coherencies once (its HBM bound)
+        n = prof["predict"]["timed"]
+        ms = prof["predict"]["ms"] / n
+        fma = 4.0 * p.vis_src
+        cbytes = K * (64 if args.coh == "full" else 16) * p.samples
+        rooflines.append({"bound": "tensor", "kernel": "predict_station_kernel", "achieved": fma / (ms * 1e-3) / 1e12,
+                          "peak": dmma["fma_per_s"] / 1e12, "unit": "T FP64 FMA/s", "frac": fma / (ms * 1e-3) / dmma["fma_per_s"],
+                          "traffic": None,
+                          "peak_source": "DMMA-chain kernel measured in this run (sagecal_profile_dmma_peak: 8 chains x 16 "
+                                         "warps x %d SMs, 256 FMAs per m8n8k4); DFMA chains in the same run: %.3e/s"
+                                         % (sms, dfma["fma_per_s"]),
+                          "fma_per_unit": 4.0, "unit_of_work": "visibility x source", "units_per_launch": p.vis_src,
+                          "hbm_write_bytes": cbytes, "hbm_write_frac": cbytes / (ms * 1e-3) / 1e9 / peak,
+                          "launches_timed": n, "avg_launch_ms": ms, "sm_mhz_under_load": clk.get("sm_mhz"),
+                          "share_of_step": prof["predict"]["ms"] / max(args.steps, 1) / ms_per_step,
+                          "note": "one sagecal_predict_coherencies call = uvw check + station phasors + contraction "
+                                  "(+ the per-baseline kernel, which returns at once); the per-baseline form "
+                                  "(sagecal_predict_set_form(1)) runs 8.77 FP64 instructions per visibility x source"})
     if args.lm != "direct":
         chunks = max(1, -(-p.n_lm // LM_RECENTRE))
         evals = (p.n_lm + chunks) / chunks                      # evaluations per launch: the chunk's trials + its centre
@@ -581,10 +604,14 @@ def run_ours(args):
                               "algorithmic_bytes_per_launch": pbytes, "launches_timed": pr["timed"], "avg_launch_ms": pms,
                               "where": "loop of sagecal_lm_cost_grad_jtj after the timed region (not part of the default step)"})
     pred_arm = args.coh + ("_resid" if fused else "")
-    floor = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, peak, dfma["fma_per_s"],
-                           load_counts("predict_kernel", pred_arm) or 0.0, args.lm, p.n_lm, fused)
+    if fused:
+        floor = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, peak, dfma["fma_per_s"],
+                               load_counts("predict_kernel", pred_arm) or 0.0, args.lm, p.n_lm, fused)
+    else:                                                 # station form: 4 FMAs per visibility x source at the DMMA rate
+        floor = interval_floor(p.samples, p.vis_src, K, p.n_em, args.coh, peak, dmma["fma_per_s"], 4.0, args.lm, p.n_lm, fused)
     floor["frac_of_floor"] = floor["floor_s"] / (ms_per_step * 1e-3)
-    extras = {"rooflines": rooflines, "dfma_peak": dict(dfma, nominal_fma_per_s=dfma_nominal, sms=sms), "interval_floor": floor}
+    extras = {"rooflines": rooflines, "dfma_peak": dict(dfma, nominal_fma_per_s=dfma_nominal, sms=sms),
+              "dmma_peak": dmma, "interval_floor": floor}
 
     # ---- end to end: HOST buffers in, HOST buffers out, through sagecal_calibrate_interval_host ----
     if args.no_e2e:
@@ -661,7 +688,7 @@ def run_ours(args):
         del vis_host, h_res
         torch.cuda.empty_cache()
         try:
-            extras["grid"] = measure_grid(sg, dev, args, peak, extras["dfma_peak"]["fma_per_s"],
+            extras["grid"] = measure_grid(sg, dev, args, peak, extras["dfma_peak" if args.fused else "dmma_peak"]["fma_per_s"],
                                           skip=[(p.N, p.K)] if args.config == 4 else [], steps=2, warmup=1)
         except Exception as ex:                          # the bench line must not depend on the grid
             extras["grid"] = {"error": repr(ex)}
@@ -734,7 +761,8 @@ def measure_grid(sg, dev, args, hbm_gbs, dfma_per_s, skip=(), steps=None, warmup
     steps = args.steps if steps is None else steps
     warmup = max(args.warmup, 1) if warmup is None else warmup
     fused = args.fused
-    ipu = load_counts("predict_kernel", args.coh + ("_resid" if fused else "")) or 0.0
+    # prediction's floor: fused route FP64 instructions (ncu count) at the DFMA rate; else 4 FMAs at the DMMA rate
+    ipu = (load_counts("predict_kernel", args.coh + "_resid") or 0.0) if fused else 4.0
     t = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(dev)
     out = []
     for N in GRID_N:
@@ -795,12 +823,12 @@ def run_grid(args):
     dev = torch.device("cuda", int(os.environ.get("LOCAL_RANK", "0")))
     torch.cuda.set_device(dev)
     peak, peak_src = load_peaks()
-    dfma = sg.profile_dfma_peak()
+    dfma = sg.profile_dfma_peak() if args.fused else sg.profile_dmma_peak()
     out = measure_grid(sg, dev, args, peak, dfma["fma_per_s"])
     print(json.dumps({"grid": out, "recipe": "configs[4] layout/T/F/S, 3 EM x 10 LM, float64, coherencies " + args.coh +
                       ", lm " + args.lm, "steps": args.steps, "warmup": max(args.warmup, 1),
                       "floor": "streaming kernels' algorithmic bytes at %.1f GB/s (%s) + predict's FP64 instructions at "
-                               "%.3e DFMA/s (measured in this run)" % (peak, peak_src, dfma["fma_per_s"])}), flush=True)
+                               "%.3e FMA/s (DMMA chains; --fused: FP64 instructions at the DFMA-chain rate; measured in this run)" % (peak, peak_src, dfma["fma_per_s"])}), flush=True)
     return 0
 
 

@@ -388,6 +388,9 @@ int sagecal_profile_read(double* ms_host, long long* timed_host, long long* laun
  * fma_per_s_host : host out, thread-level DFMAs per second (x2 = flop/s).   ms_host : host out or NULL, kernel time.
  */
 int sagecal_profile_dfma_peak(int iters, double* fma_per_s_host, double* ms_host, void* stream);
+/* The same for the FP64 tensor-core path: 8 independent DMMA m8n8k4 chains per warp, 16 warps per SM; FMAs per second
+ * (256 per instruction).  The denominator of the station-form prediction's roofline fraction. */
+int sagecal_profile_dmma_peak(int iters, double* fma_per_s_host, double* ms_host, void* stream);
 
 /* The host-only replays of the kernels' work decompositions (test hooks) are declared in sagecal_b200_debug.h. */
 

@@ -31,6 +31,7 @@ from ._binding import (  # noqa: F401
     predict_residual,
     predict_set_form,
     profile_dfma_peak,
+    profile_dmma_peak,
     profile_enable,
     profile_read,
     sage_calibrate,
@@ -40,6 +41,6 @@ from ._binding import (  # noqa: F401
 
 __all__ = [
     "COH_FULL", "COH_SCALAR", "LM_COMPRESSED", "LM_DIRECT", "LM_FULLGN", "LM_PERCLUSTER", "SagecalError", "apply_flags", "canonical_to_rows", "rows_to_canonical", "calibrate_interval_host", "host_sync", "host_trim", "corrupt_subtract", "kernel_kinds",
-    "launch_count", "lib_path", "lm_cost_grad_jtj", "load_library", "predict_coherencies", "predict_coherencies_static", "predict_static_bytes", "predict_residual", "predict_set_form", "profile_dfma_peak", "profile_enable",
+    "launch_count", "lib_path", "lm_cost_grad_jtj", "load_library", "predict_coherencies", "predict_coherencies_static", "predict_static_bytes", "predict_residual", "predict_set_form", "profile_dfma_peak", "profile_dmma_peak", "profile_enable",
     "profile_read", "sage_calibrate", "version", "workspace_bytes",
 ]

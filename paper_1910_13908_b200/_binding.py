@@ -101,6 +101,8 @@ def load_library():
     L.sagecal_profile_read.argtypes = [vp, vp, vp]
     L.sagecal_profile_dfma_peak.restype = i
     L.sagecal_profile_dfma_peak.argtypes = [i, vp, vp, vp]
+    L.sagecal_profile_dmma_peak.restype = i
+    L.sagecal_profile_dmma_peak.argtypes = [i, vp, vp, vp]
     _lib = L
     return L
 
@@ -140,6 +142,14 @@ def profile_dfma_peak(iters: int = 20000, stream=None) -> dict:
     v = (ctypes.c_double * 2)()
     _check(load_library().sagecal_profile_dfma_peak(iters, ctypes.addressof(v), ctypes.addressof(v) + 8, _stream(stream)),
            "sagecal_profile_dfma_peak")
+    return dict(fma_per_s=float(v[0]), ms=float(v[1]))
+
+
+def profile_dmma_peak(iters: int = 4000, stream=None) -> dict:
+    """sagecal_profile_dmma_peak: the measured FP64 tensor-core (DMMA) peak of the current device, dict(fma_per_s, ms)."""
+    v = (ctypes.c_double * 2)()
+    _check(load_library().sagecal_profile_dmma_peak(iters, ctypes.addressof(v), ctypes.addressof(v) + 8, _stream(stream)),
+           "sagecal_profile_dmma_peak")
     return dict(fma_per_s=float(v[0]), ms=float(v[1]))
 
 

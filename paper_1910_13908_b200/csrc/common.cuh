@@ -34,6 +34,8 @@ struct LaunchScope {
     ~LaunchScope();
 };
 
+void count_more_launches(int kind, int n);    // a LaunchScope counts one launch; the rest of its kernels go here
+
 // ---- complex scalars and 2x2 matrices (row-major [XX, XY, YX, YY]) --------------------------------------------
 struct __align__(16) cplx { double re, im; };
 struct __align__(32) d4 { double x, y, z, w; };

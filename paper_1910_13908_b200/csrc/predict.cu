@@ -648,11 +648,24 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
             if (sg < nstage && cp_thread) {
                 double* dstg = smem + (sg % PG_NSTG) * SZS + cp_dst;
                 const int nrow = min(PG_KSS, np - sg * PG_KSS) * FT;
-                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * PG_KSS) * Fpad + c0) * rowlen;
+                // row (ks, c) of the stage sits (ks Fpad + c) rows further in global memory
+                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * PG_KSS) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
+                if (FT > 1) {
 #pragma unroll
-                for (int r0 = 0; r0 < PG_KSS * FT; r0 += 2) {
-                    const int r = r0 + cp_rp;            // row (ks, c) = (r / FT, r % FT) of the stage
-                    if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + ((size_t)(r / FT) * Fpad + (r % FT)) * rowlen);
+                    for (int ks = 0; ks < PG_KSS; ks++) {
+#pragma unroll
+                        for (int c2 = 0; c2 < FT / 2; c2++) {
+                            const int r = ks * FT + 2 * c2 + cp_rp;
+                            if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + c2 * (2 * rowlen));
+                        }
+                        src += Fpad * rowlen;
+                    }
+                } else {
+#pragma unroll
+                    for (int r0 = 0; r0 < PG_KSS; r0 += 2) {
+                        const int r = r0 + cp_rp;
+                        if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + (size_t)r * Fpad * rowlen);
+                    }
                 }
             }
             pg_cp_async_commit();                        // always: the group count per stage stays uniform
@@ -802,6 +815,7 @@ static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int F
             uvw_station_check_kernel<<<(unsigned)((rows + 255) / 256), 256, 0, st>>>(N, B, rows, uvw, flag);
             const int kz = K < PG_KZ ? K : PG_KZ;      // a CTA keeps its tile for several clusters
             const int tstep = (int)(tchunk < 32768 ? tchunk : 32768);
+            count_more_launches(KK_PREDICT, 1 + 2 * ((T + tstep - 1) / tstep));     // the check, (phasors, contraction) per chunk
             for (int t0 = 0; t0 < T; t0 += tstep) {
                 const int nt = T - t0 < tstep ? T - t0 : tstep;
                 double* E = (double*)extra;
