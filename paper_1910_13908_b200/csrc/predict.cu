@@ -615,6 +615,7 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
             for (int nt = 0; nt < NT; nt++)
                 if (q0 + qb + nt * 8 + 7 > p0 + mt * 8 && p0 + mt * 8 < N && q0 + qb + nt * 8 < N) act |= 1u << (mt * NT + nt);
     }
+    const bool all_act = act == (1u << (2 * NT)) - 1u;
     const int a_off = (cw * PG_TP + g) * 4 + j;
     const int b_off = SZA + (cw * PG_TQ + qb + g) * 4 + j;
     const int jx = (j ^ 1) - j;                          // the partner entry (s, 1 - ri) of this lane's (s, ri)
@@ -694,14 +695,24 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                     }
 #pragma unroll
                     for (int nt = 0; nt < NT; nt++) b[nt] = bk[nt * 32];
+                    if (all_act) {                       // every tile off the diagonal: no predicates in the way
 #pragma unroll
-                    for (int mt = 0; mt < 2; mt++)
+                        for (int mt = 0; mt < 2; mt++)
 #pragma unroll
-                        for (int nt = 0; nt < NT; nt++)
-                            if (act & (1u << (mt * NT + nt))) {
+                            for (int nt = 0; nt < NT; nt++) {
                                 dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
                                 dmma884(acc[mt][nt][2], acc[mt][nt][3], a2[mt], b[nt]);
                             }
+                    } else {
+#pragma unroll
+                        for (int mt = 0; mt < 2; mt++)
+#pragma unroll
+                            for (int nt = 0; nt < NT; nt++)
+                                if (act & (1u << (mt * NT + nt))) {
+                                    dmma884(acc[mt][nt][0], acc[mt][nt][1], a[mt], b[nt]);
+                                    dmma884(acc[mt][nt][2], acc[mt][nt][3], a2[mt], b[nt]);
+                                }
+                    }
                 }
             }
         }
@@ -729,24 +740,28 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
             const int pc = threadIdx.x % PCS, qoff = threadIdx.x / PCS;
             const int c = SCALAR ? pc : pc >> 1;
             const bool c_ok = c0 + c < F;
-            const double2* sc = s_stage + c * CSTR;
-            sagecal_c128* ok = coh + ((size_t)k * rows + (size_t)t * B) * F * (SCALAR ? 1 : 4);
+            const double2* sc = s_stage + c * CSTR + qoff;
+            constexpr int RC = SCALAR ? 1 : 4;           // complex numbers per (row, channel)
             const int inner = SCALAR ? (c0 + c) : (c0 + c) * 4 + 2 * (pc & 1);     // complex numbers into a row
-#pragma unroll 2
-            for (int pl = 0; pl < PG_TP; pl++) {
+            const size_t rowc = (size_t)F * RC;          // complex numbers per row
+            // row of (p, q) = t B + bl_index(N, p, q); from p to p + 1 at the same q it advances by N - p - 2
+            int64_t row = (int64_t)t * B + row_start(N, p0) - p0 - 1 + q0 + qoff;
+            sagecal_c128* o = coh + ((size_t)k * rows + (size_t)row) * rowc + inner;
+            const int pend = min(PG_TP, N - 1 - p0);     // rows p >= N - 1 have no baseline
+            for (int pl = 0; pl < pend; pl++) {
                 const int p = p0 + pl;
-                if (p >= N - 1) break;
-                const int64_t rs = row_start(N, p) - p - 1;          // bl_index(N, p, q) = rs + q
 #pragma unroll
-                for (int ql = qoff; ql < PG_TQ; ql += QPT) {
-                    const int q = q0 + ql;
-                    if (!(p < q && q < N && c_ok)) continue;
-                    const double2 v = sc[pl * PSTR + ql];
-                    sagecal_c128* o = ok + (size_t)(rs + q) * F * (SCALAR ? 1 : 4) + inner;
-                    if (SCALAR) *reinterpret_cast<double2*>(o) = v;
-                    else if (pc & 1) stg256(o, 0.0, 0.0, v.x, v.y);
-                    else stg256(o, v.x, v.y, 0.0, 0.0);
+                for (int x = 0; x < (PG_TQ + QPT - 1) / QPT; x++) {
+                    const int q = q0 + qoff + x * QPT;
+                    if (qoff + x * QPT < PG_TQ && p < q && q < N && c_ok) {
+                        const double2 v = sc[pl * PSTR + x * QPT];
+                        sagecal_c128* ox = o + (size_t)(x * QPT) * rowc;
+                        if (SCALAR) *reinterpret_cast<double2*>(ox) = v;
+                        else if (pc & 1) stg256(ox, 0.0, 0.0, v.x, v.y);
+                        else stg256(ox, v.x, v.y, 0.0, 0.0);
+                    }
                 }
+                o += (size_t)(N - p - 2) * rowc;
             }
         }
       }
