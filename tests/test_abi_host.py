@@ -51,6 +51,28 @@ def test_strerror_version_and_sizes(lib):
     assert lib.sagecal_predict_workspace_bytes(100000, 1) == 0
 
 
+def test_predict_station_workspace_and_form_switch(lib):
+    """sagecal_predict_workspace_bytes_station = the per-baseline workspace + whole time slots of station phasors
+    (E and FE: 2 x pairs x channels x stations x 32 B each), at least one slot, at most what fits 2 GiB; the form switch
+    takes 0 and 1 only; the no-allocation entry point's limit is its header's."""
+    lib.sagecal_predict_workspace_bytes_station.restype = ctypes.c_size_t
+    base = lib.sagecal_predict_workspace_bytes(8, 2000)
+    full = lib.sagecal_predict_workspace_bytes_station(512, 20, 8, 50, 2000)
+    per_slot = 2 * (2000 // 2 + 50) * 8 * 512 * 32            # the pair count's upper bound: S/2 + K
+    assert (full - base) % per_slot < 256 and 1 <= (full - base) // per_slot <= 20
+    assert full - base <= 2 * 2 ** 30 + 256
+    small = lib.sagecal_predict_workspace_bytes_station(64, 3, 4, 5, 100)
+    assert small - lib.sagecal_predict_workspace_bytes(4, 100) >= 3 * 2 * (50 + 5) * 4 * 64 * 32     # all three slots
+    huge = lib.sagecal_predict_workspace_bytes_station(4096, 5, 8, 10, 20000)                          # one slot > 2 GiB
+    assert huge - lib.sagecal_predict_workspace_bytes(8, 20000) >= 2 * (10000 + 10) * 8 * 4096 * 32
+    assert lib.sagecal_predict_workspace_bytes_station(1, 20, 8, 50, 2000) == base                     # invalid shape
+    assert lib.sagecal_predict_set_form(2) == -1 and lib.sagecal_predict_set_form(-1) == -1
+    assert lib.sagecal_predict_set_form(1) == 0 and lib.sagecal_predict_set_form(0) == 0
+    lib.sagecal_predict_static_bytes.restype = ctypes.c_size_t
+    assert lib.sagecal_predict_static_bytes() == 2 * 1024 * 1024
+    assert b"scratch" in lib.sagecal_strerror(-5)
+
+
 def test_argument_validation_needs_no_device(lib):
     """EINVAL / EWORKSPACE are decided on the host before anything is enqueued (no compute call is made)."""
     z = ctypes.c_void_p(0)
