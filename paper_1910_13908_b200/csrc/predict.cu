@@ -470,11 +470,19 @@ constexpr int PG_NSTG = PG_NSTG_;              // stages in flight
 constexpr int PG_THREADS = 256;
 struct PredPairs { int off[PRED_MAXK + 1]; };            // first source PAIR of every cluster (a cluster with an odd
                                                          // count ends in a padding source of zero flux)
-template <int FT> constexpr size_t pg_smem_bytes() {
-    // the operand stages; the epilogue's [c][p][q] tile (padded) re-uses them
-    constexpr size_t stages = sizeof(double) * (size_t)(PG_NSTG * PG_KSS * FT * (PG_TP + PG_TQ) * 4);
+// 2x2 output: the finished tile has a shared-memory buffer of its own and leaves row by row while the NEXT tile is
+// contracted (one stage = one source pair, three in flight: what fits next to the 68 KB tile at two CTAs per SM);
+// scalar output (a quarter of the bytes, whose stores cost nothing) keeps the larger stages and sends the tile out at
+// once through the operand buffers.  configs[4]: 17.8 against 19.6 ms (2x2), 14.7 against 15.7 ms (scalar).
+template <bool SCALAR> struct PgCfg {
+    static constexpr bool PIPE = !SCALAR;
+    static constexpr int KSS = PIPE ? 1 : PG_KSS;        // k-steps (source pairs) per pipeline stage
+    static constexpr int NSTG = PIPE ? 3 : PG_NSTG;      // stages in flight
+};
+template <int FT, bool SCALAR> constexpr size_t pg_smem_bytes() {
+    constexpr size_t stages = sizeof(double) * (size_t)(PgCfg<SCALAR>::NSTG * PgCfg<SCALAR>::KSS * FT * (PG_TP + PG_TQ) * 4);
     constexpr size_t tile = sizeof(double) * 2 * (size_t)FT * (PG_TP * (PG_TQ + 1) + 1);
-    return stages > tile ? stages : tile;
+    return PgCfg<SCALAR>::PIPE ? stages + tile : (stages > tile ? stages : tile);
 }
 // bytes of station phasors (both operands) per time slot
 static size_t pg_bytes_per_slot(int N, int npairs, int Fpad) { return (size_t)2 * npairs * Fpad * N * 4 * sizeof(double); }
@@ -586,14 +594,16 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                        const int* __restrict__ flag) {
     if (*flag) return;                                   // uvw are not station differences: predict2_kernel's job
     extern __shared__ __align__(16) unsigned char pg_smem[];
-    constexpr int SZA = PG_KSS * FT * PG_TP * 4;         // doubles per stage: [ks][c][station][2 sources x (re, im)]
-    constexpr int SZB = PG_KSS * FT * PG_TQ * 4;
+    constexpr bool PIPE = PgCfg<SCALAR>::PIPE;
+    constexpr int KSS = PgCfg<SCALAR>::KSS, NSTG = PgCfg<SCALAR>::NSTG;
+    constexpr int SZA = KSS * FT * PG_TP * 4;            // doubles per stage: [ks][c][station][2 sources x (re, im)]
+    constexpr int SZB = KSS * FT * PG_TQ * 4;
     constexpr int SZS = SZA + SZB;
     // a warp takes ONE channel, all 16 p and NT n-tiles of 8 q (8 fragment loads per 16 DMMAs at FT = 8, 32
     // accumulator doubles per lane: 16 warps per SM)
     constexpr int NQW = 8 / FT < 4 ? 8 / FT : 4, NT = 4 / NQW;
     double* smem = reinterpret_cast<double*>(pg_smem);
-    double2* s_stage = reinterpret_cast<double2*>(pg_smem);              // epilogue: [c][p][q] of the tile, padded
+    double2* s_stage = reinterpret_cast<double2*>(pg_smem) + (PIPE ? (NSTG * SZS) / 2 : 0);   // the finished tile: [c][p][q], padded
     // tile (pi, qi) of this CTA: p-tiles of PG_TP stations, q-tiles of PG_TQ; only tiles with some q > p
     const int ntq = (N + PG_TQ - 1) / PG_TQ;
     int pi = 0, rem = (int)blockIdx.x;
@@ -632,9 +642,41 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
     const int cp_rstride = (cp_p ? PG_TP : PG_TQ) * 4;
     const size_t rowlen = (size_t)N * 4;                 // doubles per (pair, channel) row
 
+    // the finished tile leaves while the NEXT tile is contracted: one row of it per pipeline stage
+    constexpr int PSTR = PG_TQ + 1, CSTR = PG_TP * PSTR + 1;         // strides in complex numbers
+    constexpr int PCS = SCALAR ? FT : 2 * FT;        // pieces per (p, q): 16 bytes per channel / 32 bytes per half
+    constexpr int QPT = PG_THREADS / PCS;            // q's covered by the CTA per trip
+    constexpr int RC = SCALAR ? 1 : 4;               // complex numbers per (row, channel)
+    const int pc = threadIdx.x % PCS, qoff = threadIdx.x / PCS;
+    const int so_c = SCALAR ? pc : pc >> 1;
+    const double2* so_sc = s_stage + so_c * CSTR + qoff;
+    const size_t rowc = (size_t)F * RC;              // complex numbers per row
+    const int pend = min(PG_TP, N - 1 - p0);         // rows p >= N - 1 have no baseline
+    int so_pl = 0, so_pend = 0;
+    bool so_ok = false;
+    sagecal_c128* so_o = coh;
+    auto stream_row = [&]() {
+        if (so_pl < so_pend) {
+            const int p = p0 + so_pl;
+#pragma unroll
+            for (int x = 0; x < (PG_TQ + QPT - 1) / QPT; x++) {
+                const int q = q0 + qoff + x * QPT;
+                if (qoff + x * QPT < PG_TQ && p < q && q < N && so_ok) {
+                    const double2 v = so_sc[so_pl * PSTR + x * QPT];
+                    sagecal_c128* ox = so_o + (size_t)(x * QPT) * rowc;
+                    if (SCALAR) *reinterpret_cast<double2*>(ox) = v;
+                    else if (pc & 1) stg256(ox, 0.0, 0.0, v.x, v.y);
+                    else stg256(ox, v.x, v.y, 0.0, 0.0);
+                }
+            }
+            so_o += (size_t)(N - p - 2) * rowc;
+            so_pl++;
+        }
+    };
+
     for (int k = blockIdx.z; k < K; k += gridDim.z) {
       const int pb = pp.off[k], np = pp.off[k + 1] - pb;
-      const int nstage = (np + PG_KSS - 1) / PG_KSS;
+      const int nstage = (np + KSS - 1) / KSS;
       for (int c0 = 0; c0 < Fpad; c0 += FT) {
         double acc[2][NT][4];                            // [m-tile][n-tile][Re q, Re q+1, Im q, Im q+1]
 #pragma unroll
@@ -647,13 +689,13 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
         // stage sg of this (cluster, channel tile): pairs pb + sg KSS ..; 16-byte pieces, 96 per (pair, channel)
         auto issue = [&](int sg) {
             if (sg < nstage && cp_thread) {
-                double* dstg = smem + (sg % PG_NSTG) * SZS + cp_dst;
-                const int nrow = min(PG_KSS, np - sg * PG_KSS) * FT;
+                double* dstg = smem + (sg % NSTG) * SZS + cp_dst;
+                const int nrow = min(KSS, np - sg * KSS) * FT;
                 // row (ks, c) of the stage sits (ks Fpad + c) rows further in global memory
-                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * PG_KSS) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
+                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * KSS) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
                 if (FT > 1) {
 #pragma unroll
-                    for (int ks = 0; ks < PG_KSS; ks++) {
+                    for (int ks = 0; ks < KSS; ks++) {
 #pragma unroll
                         for (int c2 = 0; c2 < FT / 2; c2++) {
                             const int r = ks * FT + 2 * c2 + cp_rp;
@@ -663,7 +705,7 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                     }
                 } else {
 #pragma unroll
-                    for (int r0 = 0; r0 < PG_KSS; r0 += 2) {
+                    for (int r0 = 0; r0 < KSS; r0 += 2) {
                         const int r = r0 + cp_rp;
                         if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + (size_t)r * Fpad * rowlen);
                     }
@@ -673,16 +715,16 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
         };
         __syncthreads();                                 // every warp is done with the shared memory of the previous tile
 #pragma unroll
-        for (int sg = 0; sg < PG_NSTG - 1; sg++) issue(sg);
+        for (int sg = 0; sg < NSTG - 1; sg++) issue(sg);
         for (int sg = 0; sg < nstage; sg++) {
-            pg_cp_async_wait<PG_NSTG - 2>();             // stage sg has landed (this thread's part)
+            pg_cp_async_wait<NSTG - 2>();             // stage sg has landed (this thread's part)
             __syncthreads();                             // ... everyone's; and stage sg - 1 has been consumed
-            issue(sg + PG_NSTG - 1);
+            issue(sg + NSTG - 1);
             if (act) {
-                const double* sb_ = smem + (sg % PG_NSTG) * SZS;
-                const int nk = min(PG_KSS, np - sg * PG_KSS);
+                const double* sb_ = smem + (sg % NSTG) * SZS;
+                const int nk = min(KSS, np - sg * KSS);
 #pragma unroll
-                for (int ks = 0; ks < PG_KSS; ks++) {
+                for (int ks = 0; ks < KSS; ks++) {
                     if (ks > 0 && ks >= nk) break;       // only a cluster's last stage can be short
                     const double* ak = sb_ + a_off + ks * FT * PG_TP * 4;
                     const double* bk = sb_ + b_off + ks * FT * PG_TQ * 4;
@@ -715,13 +757,14 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                     }
                 }
             }
+            if (PIPE) stream_row();                      // a row of the previous tile
         }
-        // epilogue: the tile goes through shared memory (the operand buffers, free now) as [c][p][q] complex, padded so
-        // that neither side has bank conflicts, and leaves in the order of global memory: consecutive threads store
-        // consecutive 32-byte pieces (2x2 format: (v, 0) and (0, v) of a (row, channel)) -- whole lines, 8 wavefronts
-        // per store instruction where a lane-owns-its-rows store needs 32
-        constexpr int PSTR = PG_TQ + 1, CSTR = PG_TP * PSTR + 1;         // strides in complex numbers
-        __syncthreads();                                 // every warp has finished the last stage
+        // the tile goes to shared memory as [c][p][q] complex, padded so that neither side has bank conflicts, and
+        // leaves in the order of global memory: consecutive threads store consecutive 32-byte pieces (2x2 format: (v, 0)
+        // and (0, v) of a (row, channel)) -- whole lines, 8 wavefronts per store instruction where lane-owns-its-rows
+        // stores need 32
+        if (PIPE) while (so_pl < so_pend) stream_row();  // what the stages did not cover
+        __syncthreads();                                 // PIPE: the previous tile has been read; else: the last stage consumed
         if (w_work) {
 #pragma unroll
             for (int mt = 0; mt < 2; mt++)
@@ -731,40 +774,22 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                     for (int b = 0; b < 2; b++)
                         s_stage[cw * CSTR + (mt * 8 + g) * PSTR + qb + nt * 8 + 2 * j + b] = make_double2(acc[mt][nt][b], acc[mt][nt][2 + b]);
         }
-        __syncthreads();
-        // pieces per (p, q): 16 bytes per channel (scalar) / 32 bytes per half of a channel; a thread keeps its piece
-        // index and walks the tile's (p, q)
-        constexpr int PCS = SCALAR ? FT : 2 * FT;
-        constexpr int QPT = PG_THREADS / PCS;            // q's covered by the CTA per trip
-        {
-            const int pc = threadIdx.x % PCS, qoff = threadIdx.x / PCS;
-            const int c = SCALAR ? pc : pc >> 1;
-            const bool c_ok = c0 + c < F;
-            const double2* sc = s_stage + c * CSTR + qoff;
-            constexpr int RC = SCALAR ? 1 : 4;           // complex numbers per (row, channel)
-            const int inner = SCALAR ? (c0 + c) : (c0 + c) * 4 + 2 * (pc & 1);     // complex numbers into a row
-            const size_t rowc = (size_t)F * RC;          // complex numbers per row
-            // row of (p, q) = t B + bl_index(N, p, q); from p to p + 1 at the same q it advances by N - p - 2
-            int64_t row = (int64_t)t * B + row_start(N, p0) - p0 - 1 + q0 + qoff;
-            sagecal_c128* o = coh + ((size_t)k * rows + (size_t)row) * rowc + inner;
-            const int pend = min(PG_TP, N - 1 - p0);     // rows p >= N - 1 have no baseline
-            for (int pl = 0; pl < pend; pl++) {
-                const int p = p0 + pl;
-#pragma unroll
-                for (int x = 0; x < (PG_TQ + QPT - 1) / QPT; x++) {
-                    const int q = q0 + qoff + x * QPT;
-                    if (qoff + x * QPT < PG_TQ && p < q && q < N && c_ok) {
-                        const double2 v = sc[pl * PSTR + x * QPT];
-                        sagecal_c128* ox = o + (size_t)(x * QPT) * rowc;
-                        if (SCALAR) *reinterpret_cast<double2*>(ox) = v;
-                        else if (pc & 1) stg256(ox, 0.0, 0.0, v.x, v.y);
-                        else stg256(ox, v.x, v.y, 0.0, 0.0);
-                    }
-                }
-                o += (size_t)(N - p - 2) * rowc;
-            }
+        {   // this tile leaves during the next one (the next tile's first barrier orders these stores before the reads)
+            const int inner = SCALAR ? (c0 + so_c) : (c0 + so_c) * 4 + 2 * (pc & 1);     // complex numbers into a row
+            const int64_t row = (int64_t)t * B + row_start(N, p0) - p0 - 1 + q0 + qoff;
+            so_o = coh + ((size_t)k * rows + (size_t)row) * rowc + inner;
+            so_ok = c0 + so_c < F;
+            so_pl = 0; so_pend = pend;
+        }
+        if (!PIPE) {                                     // the tile sits in the operand buffers: it leaves now
+            __syncthreads();
+            while (so_pl < so_pend) stream_row();
         }
       }
+    }
+    if (PIPE) {
+        __syncthreads();
+        while (so_pl < so_pend) stream_row();
     }
 }
 
@@ -811,7 +836,7 @@ static int launch_predict(dim3 grid, cudaStream_t st, int64_t rows, int F, int F
         if (station_form) {
             // station form first (returns at once if the uvw are not station differences), the per-baseline form behind
             // it (returns at once if they are): the choice is made on the device, nothing waits for the host
-            constexpr int smem = (int)pg_smem_bytes<FT>();
+            constexpr int smem = (int)pg_smem_bytes<FT, SCALAR>();
             auto kern = predict_station_kernel<FT, SCALAR>;
             {
                 static bool ready[64] = {};
