@@ -443,11 +443,20 @@ predict2_kernel(int64_t rows, int F, int Fpad, PredFreqs fr, double dkf, PredClu
 // form C = A B with A = [Re e_p | Im e_p] (stations x 2 S_k) for the real and A' = [-Im e_p | Re e_p] for the imaginary
 // part, B = [Re f e_q ; Im f e_q]: DMMA m8n8k4, one k-step = two sources.
 //
-// A CTA takes a 32 x 32 tile of station pairs (p-tile <= q-tile) of one (time slot, cluster): its 256 threads evaluate
-// the phasors of the tile's 64 stations for PG_SC sources at a time into shared memory (same phasor_f64 and channel
-// recurrence as predict_kernel), then every warp accumulates its 8 p x 16 q x FT channels (64 accumulator doubles per
-// lane) with 4 DMMAs per 4 LDS.64.  A lane ends up with all FT channels of its 2 x 2 (p, q) pairs x {Re, Im} and
-// stores the rows whole.  Warp tiles that lie entirely at or below the diagonal do no arithmetic.
+// station_phasor_kernel writes the phasors once per (time slot, station, source) -- E = e and FE = f e, as
+// [t][source pair][channel][station][2 sources x (re, im)] -- into the part of the workspace beyond
+// sagecal_predict_workspace_bytes() (the time slots are predicted in chunks of what fits there).
+// predict_station_kernel: a CTA takes a 16 x 32 tile of station pairs (p-tile <= q-tile) of one time slot and every
+// PG_KZ-th cluster.  Eight warps; a warp contracts ONE channel x 16 p x 32 q: 2 x 4 blocks of m8n8k4 x {Re, Im} = 32
+// accumulator doubles per lane (two CTAs = 16 warps per SM).  The operand rows (512 B of the p stations from E, 1 KB of
+// the q stations from FE per (pair, channel)) arrive by cp.async in a multi-stage pipeline, laid out so that every
+// fragment load is conflict-free; per k-step a warp issues 8 LDS.64 -- A for two m-tiles, A' = the partner entry with
+// its sign bit flipped, B for four n-tiles -- for 16 DMMAs.  Blocks entirely at or below the diagonal do no
+// arithmetic.  A DMMA holds its scheduler's issue port for the 16 cycles it occupies the pipe, so every other
+// instruction costs its cycle in full: the copy addresses are fixed per thread and advance by increments.
+// The finished tile goes through shared memory as [c][p][q] and leaves in the order of global memory (consecutive
+// threads store consecutive 32-byte pieces: whole lines); with 2x2 output it has a buffer of its own and leaves row by
+// row during the NEXT tile's contraction (PgCfg below).  profiles/r02_ncu_predict_station.md has the measurements.
 //
 // uvw_station_check_kernel decides on the device whether the caller's uvw ARE station-consistent (every row within
 // 8 eps of u_0q - u_0p, relative to the 1-norms of the three vectors: rounding, nothing a parity bound of 1e-10 sees
