@@ -664,13 +664,18 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
     int so_pl = 0, so_pend = 0;
     bool so_ok = false;
     sagecal_c128* so_o = coh;
+    int so_q[(PG_TQ + QPT - 1) / QPT];               // this thread's q's (-1: outside the tile or the array)
+#pragma unroll
+    for (int x = 0; x < (PG_TQ + QPT - 1) / QPT; x++) {
+        const int q = q0 + qoff + x * QPT;
+        so_q[x] = (qoff + x * QPT < PG_TQ && q < N) ? q : -1;
+    }
     auto stream_row = [&]() {
         if (so_pl < so_pend) {
             const int p = p0 + so_pl;
 #pragma unroll
             for (int x = 0; x < (PG_TQ + QPT - 1) / QPT; x++) {
-                const int q = q0 + qoff + x * QPT;
-                if (qoff + x * QPT < PG_TQ && p < q && q < N && so_ok) {
+                if (p < so_q[x] && so_ok) {
                     const double2 v = so_sc[so_pl * PSTR + x * QPT];
                     sagecal_c128* ox = so_o + (size_t)(x * QPT) * rowc;
                     if (SCALAR) *reinterpret_cast<double2*>(ox) = v;
@@ -696,19 +701,25 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
                 for (int x = 0; x < 4; x++) acc[mt][nt][x] = 0.0;
 
         // stage sg of this (cluster, channel tile): pairs pb + sg KSS ..; 16-byte pieces, 96 per (pair, channel)
-        auto issue = [&](int sg) {
-            if (sg < nstage && cp_thread) {
-                double* dstg = smem + (sg % NSTG) * SZS + cp_dst;
-                const int nrow = min(KSS, np - sg * KSS) * FT;
-                // row (ks, c) of the stage sits (ks Fpad + c) rows further in global memory
-                const double* src = cp_src + (((size_t)tl * npairs + pb + sg * KSS) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
+        // running state of the copies: the next stage to issue, its buffer and its first row in global memory
+        int isg = 0, ibuf = 0;
+        const double* isrc = cp_src + (((size_t)tl * npairs + pb) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
+        const size_t stage_rows = (size_t)KSS * Fpad * rowlen;
+        auto issue = [&]() {
+            if (isg < nstage && cp_thread) {
+                // one pair per stage: running buffer index and pointer (fewer instructions between the DMMAs); the
+                // two-pair stages of scalar output are faster with both recomputed (measured: 14.7 against 15.2 ms)
+                double* dstg = smem + (KSS == 1 ? ibuf : isg % NSTG) * SZS + cp_dst;
+                const int nrow = KSS == 1 ? FT : min(KSS, np - isg * KSS) * FT;
+                const double* src = KSS == 1 ? isrc
+                                             : cp_src + (((size_t)tl * npairs + pb + isg * KSS) * Fpad + c0 + (FT > 1 ? cp_rp : 0)) * rowlen;
                 if (FT > 1) {
 #pragma unroll
                     for (int ks = 0; ks < KSS; ks++) {
 #pragma unroll
                         for (int c2 = 0; c2 < FT / 2; c2++) {
                             const int r = ks * FT + 2 * c2 + cp_rp;
-                            if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + c2 * (2 * rowlen));
+                            if (KSS == 1 || r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + c2 * (2 * rowlen));
                         }
                         src += Fpad * rowlen;
                     }
@@ -716,21 +727,26 @@ predict_station_kernel(int N, int64_t B, int64_t rows, int F, int Fpad, int K, i
 #pragma unroll
                     for (int r0 = 0; r0 < KSS; r0 += 2) {
                         const int r = r0 + cp_rp;
-                        if (r < nrow) pg_cp_async16(dstg + r * cp_rstride, src + (size_t)r * Fpad * rowlen);
+                        if (r < nrow && r < KSS) pg_cp_async16(dstg + r * cp_rstride, src + (size_t)r * Fpad * rowlen);
                     }
                 }
             }
             pg_cp_async_commit();                        // always: the group count per stage stays uniform
+            isg++;
+            isrc += stage_rows;
+            ibuf = ibuf + 1 == NSTG ? 0 : ibuf + 1;
         };
         __syncthreads();                                 // every warp is done with the shared memory of the previous tile
 #pragma unroll
-        for (int sg = 0; sg < NSTG - 1; sg++) issue(sg);
+        for (int sg = 0; sg < NSTG - 1; sg++) issue();
+        int cbuf = 0;
         for (int sg = 0; sg < nstage; sg++) {
             pg_cp_async_wait<NSTG - 2>();             // stage sg has landed (this thread's part)
             __syncthreads();                             // ... everyone's; and stage sg - 1 has been consumed
-            issue(sg + NSTG - 1);
+            issue();
+            const double* sb_ = smem + (KSS == 1 ? cbuf : sg % NSTG) * SZS;
+            cbuf = cbuf + 1 == NSTG ? 0 : cbuf + 1;
             if (act) {
-                const double* sb_ = smem + (sg % NSTG) * SZS;
                 const int nk = min(KSS, np - sg * KSS);
 #pragma unroll
                 for (int ks = 0; ks < KSS; ks++) {
